@@ -1,0 +1,540 @@
+"""Pins P1..P11 of the CPU oracle (SURVEY.md 8(c) "What pins the oracle").
+
+No implementation exists to compare the oracle with (PAPER.md has no tests and prints no worked
+example), so it is pinned to closed forms, invariants, brute force on tiny inputs and a library
+DP5(4).  Each test names the part of the formula sheet (A1..A9) it pins.  CPU only.
+"""
+import math
+from fractions import Fraction as Fr
+
+import numpy as np
+import pytest
+
+
+def make_grid(oracle, fn, dims, origin, spacing, nslices=1, slice_dt=1.0, time_mode=0):
+    """Sample fn(X, Y, Z, t) -> (u, v, w) at the vertices; returns (OGrid, data)."""
+    nx, ny, nz = dims
+    x = origin[0] + np.arange(nx) * spacing[0]
+    y = origin[1] + np.arange(ny) * spacing[1]
+    z = origin[2] + np.arange(nz) * spacing[2]
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    data = np.empty((nslices, nz, ny, nx, 3), dtype=np.float32)
+    for s in range(nslices):
+        u, v, w = fn(X, Y, Z, s * slice_dt)
+        data[s, ..., 0] = u; data[s, ..., 1] = v; data[s, ..., 2] = w
+    return oracle.grid(data, dims, origin, spacing, nslices, slice_dt, time_mode), data
+
+
+# ------------------------------------------------------------------------------------------
+# P1: RK4 update + loop + exit count + recording (A4, A5, A6) on a constant field.
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_p1_constant_field_straight_lines(oracle, precision):
+    c = (1.0, -0.5, 0.25)
+    h = 0.375                      # h/6 = 0.0625 exactly
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (c[0] + 0 * X, c[1] + 0 * X, c[2] + 0 * X),
+                     (9, 9, 9), (0, 0, 0), (1, 1, 1))
+    seeds = np.array([[1.0, 4.0, 2.0], [0.5, 7.75, 0.125], [7.9375, 8.0, 0.0], [0.0, 0.0625, 8.0]])
+    prm = oracle.params(0, h=h, max_steps=1000, vmin=1e-6, capacity=64, stride=1)
+    r = oracle.streamlines(g, seeds, prm, precision)
+    for i, s in enumerate(seeds):
+        # closed-form count: the largest n with p0 + n h c inside [0,8]^3 (exact rationals);
+        # stage points lie on the segment, so they are inside whenever both ends are.
+        n = 0
+        while all(0 <= Fr(s[a]) + (n + 1) * Fr(h) * Fr(c[a]) <= 8 for a in range(3)):
+            n += 1
+        assert r.steps[i] == n and r.status[i] == oracle.OUT_OF_DOMAIN
+        assert r.counts[i] == n + 1
+        k = np.arange(n + 1)
+        for a in range(3):
+            assert np.array_equal(r.vertices[a, i, :n + 1], s[a] + k * h * c[a])   # exact
+            assert np.all(np.isnan(r.vertices[a, i, n + 1:]))                      # untouched
+            assert r.final[a, i] == s[a] + n * h * c[a]
+    # totals: every accepted step took 4 samples; the failing attempt fails at stage 2, 3 or 4
+    assert r.totals[1] == r.steps.sum() and r.totals[0] == r.steps.sum() + len(seeds)
+
+
+def test_p1_recording_stride_capacity(oracle):
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (1 + 0 * X, 0 * X, 0 * X), (33, 3, 3), (0, 0, 0),
+                     (1, 1, 1))
+    prm = oracle.params(0, h=0.375, max_steps=40, vmin=0.0, capacity=5, stride=3)
+    r = oracle.streamlines(g, np.array([[1.0, 1.0, 1.0]]), prm, "f32")
+    assert r.status[0] == oracle.MAX_STEPS and r.steps[0] == 40
+    assert r.counts[0] == 5                      # vertices 0,3,6,9,12 ; 15.. beyond capacity
+    assert np.array_equal(r.vertices[0, 0], 1.0 + 0.375 * np.arange(0, 15, 3))
+    assert r.final[0, 0] == 1.0 + 40 * 0.375
+
+
+def test_termination_codes(oracle):
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (0 * X, 0 * X, 0 * X), (4, 4, 4), (0, 0, 0),
+                     (1, 1, 1))
+    prm = oracle.params(0, h=0.25, max_steps=10, vmin=1e-6, capacity=4)
+    seeds = np.array([[1.5, 1.5, 1.5], [-0.1, 1, 1], [1, 3.0001, 1], [np.nan, 1, 1], [3, 3, 3]])
+    r = oracle.streamlines(g, seeds, prm, "f32")
+    assert list(r.status) == [oracle.STAGNANT, oracle.OUT_OF_DOMAIN, oracle.OUT_OF_DOMAIN,
+                              oracle.OUT_OF_DOMAIN, oracle.STAGNANT]
+    assert list(r.counts) == [1, 0, 0, 0, 1] and list(r.steps) == [0] * 5
+    # |v| floor is a strict "<" on the squared norm; max-steps is tested before stagnation
+    g2, _ = make_grid(oracle, lambda X, Y, Z, t: (0.5 + 0 * X, 0 * X, 0 * X), (4, 4, 4), (0, 0, 0),
+                      (1, 1, 1))
+    r = oracle.streamlines(g2, seeds[:1], oracle.params(0, h=0.25, max_steps=2, vmin=0.5), "f32")
+    assert r.status[0] == oracle.MAX_STEPS and r.steps[0] == 2
+    r = oracle.streamlines(g2, seeds[:1], oracle.params(0, h=0.25, max_steps=2, vmin=0.5000001),
+                           "f32")
+    assert r.status[0] == oracle.STAGNANT and r.steps[0] == 0
+    r = oracle.streamlines(g2, seeds[:1], oracle.params(0, h=0.25, max_steps=0, vmin=0.5000001),
+                           "f32")
+    assert r.status[0] == oracle.MAX_STEPS
+
+
+# ------------------------------------------------------------------------------------------
+# P2: trilinear sampler (A1, A2) reproduces a linear field exactly.
+# ------------------------------------------------------------------------------------------
+A_LIN = np.array([[1, 2, -3], [0, -1, 4], [5, 0, 2]], dtype=np.float64)
+B_LIN = np.array([1, -2, 3], dtype=np.float64)
+
+
+def lin_field(X, Y, Z, t):
+    P = np.stack([X, Y, Z], axis=-1)
+    V = P @ A_LIN.T + B_LIN
+    return V[..., 0], V[..., 1], V[..., 2]
+
+
+def test_p2_linear_field_exact(oracle):
+    dims, origin, spacing = (7, 5, 6), (-2.0, 1.0, 3.0), (1.0, 2.0, 0.5)
+    g, _ = make_grid(oracle, lin_field, dims, origin, spacing)
+    rng = np.random.default_rng(1)
+    ext = np.array([(dims[a] - 1) * spacing[a] for a in range(3)])
+    # fp32: points at multiples of 1/8 of a cell -> every lerp is exact -> bit equality
+    cells = rng.integers(0, [8 * (d - 1) + 1 for d in dims], size=(4000, 3))
+    pts = np.array(origin) + cells / 8.0 * np.array(spacing)
+    v, rc = oracle.sample(g, pts, 0.0, "f32")
+    assert np.all(rc == 0)
+    assert np.array_equal(v.astype(np.float64), pts @ A_LIN.T + B_LIN)
+    # fp64: arbitrary points, 1e-13 relative
+    pts = np.array(origin) + rng.random((4000, 3)) * ext
+    v, rc = oracle.sample(g, pts, 0.0, "f64")
+    ref = pts @ A_LIN.T + B_LIN
+    assert np.all(rc == 0) and np.max(np.abs(v - ref)) <= 1e-13 * np.max(np.abs(ref))
+    # the closed box: the top face is inside (last cell, f = 1), one ulp beyond is not
+    top = np.array(origin) + ext
+    v, rc = oracle.sample(g, top[None, :], 0.0, "f64")
+    assert rc[0] == 0 and np.allclose(v[0], top @ A_LIN.T + B_LIN, rtol=1e-14)
+    out = np.array([np.nextafter(top[0], np.inf), top[1], top[2]])
+    assert oracle.sample(g, out[None, :], 0.0, "f64")[1][0] == oracle.OUT_OF_DOMAIN
+    below = np.array([np.nextafter(origin[0], -np.inf), origin[1], origin[2]])
+    assert oracle.sample(g, below[None, :], 0.0, "f64")[1][0] == oracle.OUT_OF_DOMAIN
+
+
+# ------------------------------------------------------------------------------------------
+# P3: sampler vs the plain definition (8-term weighted sum), brute force on tiny grids.
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_p3_eight_term_sum(oracle, n):
+    rng = np.random.default_rng(n)
+    dims = (n, n + 1, n + 2)
+    data = rng.standard_normal((1, dims[2], dims[1], dims[0], 3)).astype(np.float32)
+    origin, spacing = (0.5, -1.0, 2.0), (0.25, 2.0, 0.5)   # dyadic: vertices map to f = 0 exactly
+    g = oracle.grid(data, dims, origin, spacing)
+    ext = np.array([(dims[a] - 1) * spacing[a] for a in range(3)])
+    pts = np.array(origin) + rng.random((500, 3)) * ext
+    gi = (pts - origin) / spacing
+    i = np.minimum(np.floor(gi).astype(int), np.array(dims) - 2)
+    f = gi - i
+    ref = np.zeros((500, 3))
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                w = (f[:, 0] if dx else 1 - f[:, 0]) * (f[:, 1] if dy else 1 - f[:, 1]) * \
+                    (f[:, 2] if dz else 1 - f[:, 2])
+                ref += w[:, None] * data[0, i[:, 2] + dz, i[:, 1] + dy, i[:, 0] + dx, :]
+    v64, rc = oracle.sample(g, pts, 0.0, "f64")
+    assert np.all(rc == 0) and np.max(np.abs(v64 - ref)) < 1e-13
+    v32, rc = oracle.sample(g, pts.astype(np.float32), 0.0, "f32")
+    assert np.max(np.abs(v32 - ref)) < 2e-5       # fp32 positions: a few ulp of g times gradient
+    # at a vertex (f = 0) the stored value is returned exactly
+    for (x, y, z) in [(0, 0, 0), (0, 1, 1), (dims[0] - 2, dims[1] - 2, dims[2] - 2)]:
+        p = np.array([[origin[0] + x * spacing[0], origin[1] + y * spacing[1],
+                       origin[2] + z * spacing[2]]])
+        v, rc = oracle.sample(g, p, 0.0, "f32")
+        assert rc[0] == 0 and np.array_equal(v[0], data[0, z, y, x])
+    # on the top face the last cell is used with f = 1: lerp returns b to within 1 ulp (Q5)
+    p = np.array([[origin[a] + (dims[a] - 1) * spacing[a] for a in range(3)]])
+    v, rc = oracle.sample(g, p, 0.0, "f32")
+    corner = data[0, -1, -1, -1]
+    assert rc[0] == 0 and np.all(np.abs(v[0] - corner) <= 4 * np.spacing(np.abs(data).max()))
+    assert oracle.sample(g, np.array([[np.nan, 0, 2.5]]), 0.0, "f32")[1][0] == oracle.OUT_OF_DOMAIN
+
+
+# ------------------------------------------------------------------------------------------
+# P4: RK4 on the rigid rotation v = (-y, x, 0): each step is the map
+# M = I + hJ + (hJ)^2/2 + (hJ)^3/6 + (hJ)^4/24, i.e. multiplication of x+iy by
+# (1 - h^2/2 + h^4/24) + i (h - h^3/6).
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("h", [0.1, 0.05])
+def test_p4_rigid_rotation(oracle, h):
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (-Y, X, 0 * X), (9, 9, 3), (-4, -4, -1), (1, 1, 1))
+    n = int(round(10.0 / h))
+    prm = oracle.params(0, h=h, max_steps=n, vmin=0.0, capacity=n + 1)
+    seed = np.array([[2.0, 0.5, 0.25]])
+    r = oracle.streamlines(g, seed, prm, "f64")
+    assert r.status[0] == oracle.MAX_STEPS and r.steps[0] == n
+    zc = complex(seed[0, 0], seed[0, 1]) * (complex(1 - h**2 / 2 + h**4 / 24, h - h**3 / 6) **
+                                            np.arange(n + 1))
+    assert np.max(np.abs(r.vertices[0, 0] - zc.real)) < 1e-12
+    assert np.max(np.abs(r.vertices[1, 0] - zc.imag)) < 1e-12
+    assert np.all(r.vertices[2, 0] == 0.25)
+    # radius drift and phase error of the closed form (the O(h^4) global error of RK4)
+    rn = np.hypot(r.vertices[0, 0, -1], r.vertices[1, 0, -1]) / np.hypot(2.0, 0.5)
+    assert abs(rn - (1 - h**6 / 72 + h**8 / 576) ** (n / 2)) < 1e-13
+    ang = np.unwrap(np.arctan2(r.vertices[1, 0], r.vertices[0, 0]))
+    per_step = math.atan2(h - h**3 / 6, 1 - h**2 / 2 + h**4 / 24)
+    assert abs((ang[-1] - ang[0]) - n * per_step) < 1e-11
+    assert abs((ang[-1] - ang[0]) - 10.0 - (-10.0 * h**4 / 120)) < 10 * h**6
+
+
+# ------------------------------------------------------------------------------------------
+# P5: RK4 order on a nonlinear field: ABC flow with C = 0 conserves I = B sin x + A cos z.
+# ------------------------------------------------------------------------------------------
+def _abc_drift(oracle, field, h, seeds, A, B):
+    n = int(round(10.0 / h))
+    prm = oracle.params(0, h=h, max_steps=n, vmin=0.0, capacity=1)
+    r = oracle.streamlines(field, seeds, prm, "f64")
+    assert np.all(r.status == oracle.MAX_STEPS)
+    inv = lambda p: B * np.sin(p[0]) + A * np.cos(p[2])
+    return np.max(np.abs(inv(r.final) - inv(seeds.T)))
+
+
+def test_p5_abc_invariant_order(oracle, wl):
+    A, B = math.sqrt(3.0), math.sqrt(2.0)
+    big = 1e3
+    ana = oracle.analytic(2, [A, B, 0.0], [-big] * 3, [big] * 3)
+    seeds = wl.uniform(7, 60).reshape(20, 3) * 2 * math.pi
+    d = [_abc_drift(oracle, ana, h, seeds, A, B) for h in (0.2, 0.1, 0.05)]
+    assert d[0] / d[1] >= 14 and d[1] / d[2] >= 14, d     # 4th order: 16x per halving
+    # grid sampler: the drift is dominated by the O(dx^2) interpolation error -> >= 4x per doubling
+    drifts = []
+    for N in (33, 65, 129):
+        L = 6 * math.pi
+        sp = L / (N - 1)
+        g, _ = make_grid(oracle, lambda X, Y, Z, t: (A * np.sin(Z), B * np.sin(X) + A * np.cos(Z),
+                                                     B * np.cos(X)),
+                         (N, N, N), (-2 * math.pi,) * 3, (sp,) * 3)
+        n = 100
+        prm = oracle.params(0, h=0.02, max_steps=n, vmin=0.0, capacity=1)
+        r = oracle.streamlines(g, seeds, prm, "f64")
+        assert np.all(r.status == oracle.MAX_STEPS)
+        inv = lambda p: B * np.sin(p[0]) + A * np.cos(p[2])
+        drifts.append(np.max(np.abs(inv(r.final) - inv(seeds.T))))
+    assert drifts[0] / drifts[1] > 3.5 and drifts[1] / drifts[2] > 3.5, drifts   # >= 2nd order in dx
+
+
+# ------------------------------------------------------------------------------------------
+# P6: time interpolation + stage times (A3, A4): v = a + b t, spatially uniform.
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_p6_linear_in_time_exact(oracle, precision):
+    a = np.array([1.0, -4.0, 0.25]); b = np.array([0.5, -1.5, 0.0])
+    fn = lambda X, Y, Z, t: tuple(a[c] + b[c] * t + 0 * X for c in range(3))
+    g, _ = make_grid(oracle, fn, (2, 2, 2), (-512, -512, -512), (1024, 1024, 1024), nslices=33,
+                     slice_dt=0.5)
+    prm = oracle.params(0, h=0.25, max_steps=64, vmin=0.0, capacity=65)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
+    assert r.status[0] == oracle.MAX_STEPS
+    assert list(r.final[:, 0]) == [80.0, -256.0, 4.0]                 # x0 + aT + bT^2/2, T = 16
+    t = 0.25 * np.arange(65)
+    for c in range(3):
+        assert np.array_equal(r.vertices[c, 0], a[c] * t + b[c] * t * t / 2)
+    # t0 shifts the clock: starting at t0 = 4 for 16 steps
+    prm = oracle.params(0, h=0.25, max_steps=16, vmin=0.0, t0=4.0)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
+    assert list(r.final[:, 0]) == [a[c] * 4 + b[c] * (8 * 8 - 4 * 4) / 2 for c in range(3)]
+    # beyond the last slice (t > 16) the field is frozen (Q10): v = a + 16 b
+    prm = oracle.params(0, h=0.25, max_steps=8, vmin=0.0, t0=20.0)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
+    assert list(r.final[:, 0]) == [2 * (a[c] + 16 * b[c]) for c in range(3)]
+
+
+def test_p6_hold_floor_slice_mode(oracle):
+    """time_mode = 1 is the paper's fields[(int)simTime]: piecewise constant."""
+    a = np.array([1.0, -4.0, 0.25]); b = np.array([0.5, -1.5, 0.0])
+    fn = lambda X, Y, Z, t: tuple(a[c] + b[c] * t + 0 * X for c in range(3))
+    g, _ = make_grid(oracle, fn, (2, 2, 2), (-512,) * 3, (1024,) * 3, nslices=5, slice_dt=1.0,
+                     time_mode=1)
+    prm = oracle.params(0, h=0.5, max_steps=8, vmin=0.0)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, "f64")
+    # step n covers [n/2, (n+1)/2]: stages at t_n, t_n + h/2 (twice), t_n + h use floor slices
+    x = np.zeros(3)
+    for n in range(8):
+        t = 0.5 * n
+        v = lambda tt: a + b * min(math.floor(tt), 4)
+        x = x + 0.5 / 6 * (v(t) + 2 * v(t + 0.25) + 2 * v(t + 0.25) + v(t + 0.5))
+    assert np.allclose(r.final[:, 0], x, rtol=0, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------
+# P7: the unsteady path on config 4's field (double gyre).
+# ------------------------------------------------------------------------------------------
+def test_p7_double_gyre(oracle, wl):
+    f = wl.double_gyre_field(dims=(64, 32, 16), nslices=8, dt=0.25)
+    g = oracle.grid(f.data, f.dims, f.origin, f.spacing, f.nslices, f.slice_dt)
+    # (i) particles on the wall y = 0 keep y == 0 exactly (that grid row is exactly zero)
+    seeds = np.array([[0.3, 0.0, 0.2], [1.7, 0.0, 0.9], [1.0, 0.0, 0.5]], dtype=np.float32)
+    prm = oracle.params(0, h=0.05, max_steps=200, vmin=0.0, capacity=201)
+    r = oracle.streamlines(g, seeds, prm, "f32")
+    assert np.all(r.status == oracle.MAX_STEPS) and np.all(r.vertices[1] == 0.0)
+    assert np.max(np.abs(r.vertices[0, :, -1] - seeds[:, 0])) > 1e-2   # but they do move in x
+    # (ii) analytic sampler: tan(pi z/2) = tan(pi z0/2) exp(0.05 pi t)
+    ana = oracle.analytic(4, [0.1, 0.25, 2 * math.pi / 10, 0.05], [0, 0, 0], [2, 1, 1])
+    z0 = np.array([0.1, 0.37, 0.5, 0.8])
+    seeds = np.stack([np.full(4, 0.7), np.full(4, 0.4), z0], axis=1)
+    r = oracle.streamlines(ana, seeds, oracle.params(0, h=0.05, max_steps=1000, vmin=0.0), "f64")
+    assert np.all(r.status == oracle.MAX_STEPS)
+    lhs = np.tan(math.pi * r.final[2] / 2)
+    rhs = np.tan(math.pi * z0 / 2) * math.exp(0.05 * math.pi * 50.0)
+    assert np.max(np.abs(lhs / rhs - 1)) < 1e-8
+    # (iii) eps = 0: steady, stream function A sin(pi x) sin(pi y) conserved to O(h^4)
+    psi = lambda p: 0.1 * np.sin(math.pi * p[0]) * np.sin(math.pi * p[1])
+    d = []
+    for h in (0.4, 0.2, 0.1):
+        ana0 = oracle.analytic(4, [0.1, 0.0, 2 * math.pi / 10, 0.05], [0, 0, 0], [2, 1, 1])
+        rr = oracle.streamlines(ana0, seeds, oracle.params(0, h=h, max_steps=int(round(40 / h)),
+                                                           vmin=0.0), "f64")
+        d.append(np.max(np.abs(psi(rr.final) - psi(seeds.T))))
+    assert d[0] / d[1] > 12 and d[1] / d[2] > 12, d
+
+
+# ------------------------------------------------------------------------------------------
+# P8: Dormand-Prince 5(4) (A8).
+# ------------------------------------------------------------------------------------------
+DP_C = [Fr(0), Fr(1, 5), Fr(3, 10), Fr(4, 5), Fr(8, 9), Fr(1), Fr(1)]
+
+
+def _tableau_matrix(tab):
+    A = np.zeros((7, 7))
+    k = 0
+    for s in range(1, 7):
+        for j in range(s):
+            A[s, j] = tab["a"][k]; k += 1
+    return A
+
+
+@pytest.mark.parametrize("precision,tol", [("f64", 4e-16), ("f32", 2e-7)])
+def test_p8i_tableau_identities(oracle, precision, tol):
+    tab = oracle.dp5_tableau(precision)
+    A, b, e, c = _tableau_matrix(tab), tab["b"], tab["e"], tab["c"]
+    cx = np.array([float(x) for x in DP_C])
+    assert np.max(np.abs(c - cx)) <= tol
+    assert np.max(np.abs(A.sum(axis=1) - cx)) <= 8 * tol            # row sums = c
+    assert np.max(np.abs(A[6] - b)) == 0                            # FSAL: a7 = b
+    bs = b - e                                                      # embedded 4th-order weights
+    # quadrature conditions: b to degree 4, b* to degree 3
+    for k in range(5):
+        assert abs(b @ cx**k - 1 / (k + 1)) <= 8 * tol
+    for k in range(4):
+        assert abs(bs @ cx**k - 1 / (k + 1)) <= 8 * tol
+    assert abs(bs @ cx**4 - 1 / 5) > 1e-4                           # ... and not to degree 4
+    # tree conditions of orders 3..5 for b (Butcher): b.A.c = 1/6, b.A.c^2 = 1/12,
+    # b.(c*(A.c)) = 1/8, b.A.A.c = 1/24, b.A.c^3 = 1/20, b.A.A.A.c = 1/120
+    Ac = A @ cx
+    assert abs(b @ Ac - 1 / 6) <= 8 * tol
+    assert abs(b @ (A @ cx**2) - 1 / 12) <= 8 * tol
+    assert abs(b @ (cx * Ac) - 1 / 8) <= 8 * tol
+    assert abs(b @ (A @ Ac) - 1 / 24) <= 8 * tol
+    assert abs(b @ (A @ cx**3) - 1 / 20) <= 8 * tol
+    assert abs(b @ (A @ (A @ Ac)) - 1 / 120) <= 8 * tol
+    assert abs(bs @ Ac - 1 / 6) <= 8 * tol and abs(bs @ (A @ Ac) - 1 / 24) <= 8 * tol
+    # the printed error weights (tests/golden/dp5_error_weights.txt)
+    import os
+    gold = open(os.path.join(os.path.dirname(__file__), "golden", "dp5_error_weights.txt"))
+    ex = [float(Fr(tok)) for line in gold if not line.startswith("#") for tok in line.split()]
+    assert np.max(np.abs(e - np.array(ex))) <= tol
+
+
+def test_p8ii_fixed_step_rotation_polynomial(oracle):
+    """With h_min = h_max the step map on v = (-y, x, 0) is R(hJ),
+    R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24 + z^5/120 + z^6/600."""
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (-Y, X, 0 * X), (9, 9, 3), (-4, -4, -1), (1, 1, 1))
+    h, n = 0.125, 40
+    prm = oracle.params(1, h=h, h_min=h, h_max=h, atol=1e-30, rtol=1e-30, max_steps=n, vmin=0.0,
+                        capacity=n + 1)
+    r = oracle.streamlines(g, np.array([[2.0, 0.5, 0.0]]), prm, "f64")
+    assert r.status[0] == oracle.MAX_STEPS and r.totals[0] == n      # forced accepts at the floor
+    z = 1j * h
+    R = 1 + z + z**2 / 2 + z**3 / 6 + z**4 / 24 + z**5 / 120 + z**6 / 600
+    zc = complex(2.0, 0.5) * R ** np.arange(n + 1)
+    assert np.max(np.abs(r.vertices[0, 0] - zc.real)) < 1e-13
+    assert np.max(np.abs(r.vertices[1, 0] - zc.imag)) < 1e-13
+
+
+def test_p8iii_quartic_in_time_exact(oracle):
+    """v = t^4 (uniform in space): DP5(4) integrates it exactly, x = t^5/5, for any step sizes."""
+    ana = oracle.analytic(3, [0, 0, 0, 0, 0, 0, 1.0, -2.0, 0.5], [-1e9] * 3, [1e9] * 3)
+    prm = oracle.params(1, h=0.1, h_min=0.01, h_max=0.7, atol=1e-6, rtol=1e-6, max_steps=25,
+                        vmin=0.0, t0=0.0, capacity=26)
+    r = oracle.streamlines(ana, np.zeros((1, 3)), prm, "f64")
+    x = r.vertices[0, 0]
+    t = (5 * x) ** 0.2                                               # the accepted times
+    assert np.all(np.diff(t) > 0.0099) and np.all(np.diff(t) < 0.7001) and t[-1] > 5
+    assert np.max(np.abs(r.vertices[1, 0] - (-2.0) * t**5 / 5) / (1 + t**5)) < 1e-13
+    assert np.max(np.abs(r.vertices[2, 0] - 0.5 * t**5 / 5) / (1 + t**5)) < 1e-13
+    assert abs(t[1] - 0.1) < 1e-12                                   # first step = params.h
+
+
+def test_p8iv_against_library_dp5(oracle):
+    """fp64 + analytic ABC: accepted steps equal those of scipy's RK45 (same tableau, same
+    controller constants 0.9 / 0.2 / 10 / -1/5) as long as no h_min clamp or failure occurs."""
+    from scipy.integrate import RK45
+    A, B, C = math.sqrt(3.0), math.sqrt(2.0), 1.0
+    ana = oracle.analytic(2, [A, B, C], [-1e3] * 3, [1e3] * 3)
+    fun = lambda t, p: [A * math.sin(p[2]) + C * math.cos(p[1]), B * math.sin(p[0]) + A * math.cos(p[2]),
+                        C * math.sin(p[1]) + B * math.cos(p[0])]
+    for seed, rtol, atol in [([1.0, 2.0, 3.0], 1e-5, 1e-5), ([4.0, 0.5, 5.5], 1e-8, 1e-9)]:
+        n = 300
+        prm = oracle.params(1, h=0.25, h_min=1e-12, h_max=2.0, atol=atol, rtol=rtol, max_steps=n,
+                            vmin=0.0, capacity=n + 1)
+        r = oracle.streamlines(ana, np.array([seed]), prm, "f64")
+        s = RK45(fun, 0.0, seed, 1e9, first_step=0.25, max_step=2.0, rtol=rtol, atol=atol)
+        ys, rejected = [np.array(seed)], 0
+        for _ in range(n):
+            s.step()
+            ys.append(s.y.copy())
+        ys = np.array(ys)
+        assert r.status[0] == oracle.MAX_STEPS
+        assert np.max(np.abs(r.vertices[:, 0, :].T - ys)) < 1e-7
+        # same number of rejected attempts: scipy counts 6 evaluations per attempt (+1 at start)
+        assert r.totals[2] == s.nfev and r.totals[0] > n
+
+
+def test_p8v_rp10(oracle):
+    LO, HI = 3.4867844e-11, 3405062.9
+    x = np.exp(np.linspace(math.log(LO), math.log(HI), 200001))
+    y32 = oracle.rp10(x.astype(np.float32), "f32").astype(np.float64)
+    assert np.max(np.abs(y32 * x.astype(np.float32).astype(np.float64) ** 0.1 - 1)) <= 2e-7
+    y64 = oracle.rp10(x, "f64")
+    assert np.max(np.abs(y64 * x**0.1 - 1)) <= 1e-9
+    # the clamp points of the controller: 0.9*LO^-0.1 = 10, 0.9*HI^-0.1 = 0.2
+    assert abs(0.9 * LO**-0.1 - 10) < 1e-5 and abs(0.9 * HI**-0.1 - 0.2) < 1e-7
+
+
+def test_p8_controller_paths(oracle):
+    """Constant field: the error estimate is exactly 0, so fac = 10 until h_max; forced accept at
+    h_min on a field the estimator hates; rejection shrinks h and caps the next factor at 1."""
+    g, _ = make_grid(oracle, lambda X, Y, Z, t: (1 + 0 * X, 0 * X, 0 * X), (65, 3, 3), (0, 0, 0),
+                     (1, 1, 1))
+    prm = oracle.params(1, h=0.0078125, h_min=0.0078125, h_max=1.0, atol=1e-5, rtol=1e-5,
+                        max_steps=6, vmin=0.0, capacity=7)
+    r = oracle.streamlines(g, np.array([[1.0, 1.0, 1.0]]), prm, "f32")
+    assert np.allclose(np.diff(r.vertices[0, 0]), [0.0078125, 0.078125, 0.78125, 1.0, 1.0, 1.0],
+                       rtol=1e-6, atol=0)        # sum(b) = 1 only to fp32 rounding
+    assert r.totals[0] == 6 and r.totals[2] == 1 + 6 * 6
+    # a kinked field (|x - 2.5| profile in y-velocity) forces rejections
+    g2, _ = make_grid(oracle, lambda X, Y, Z, t: (1 + 0 * X, np.abs(X - 3.0), 0 * X), (9, 65, 3),
+                      (0, 0, 0), (1, 1, 1))
+    prm = oracle.params(1, h=1.0, h_min=0.001, h_max=1.0, atol=1e-7, rtol=1e-7, max_steps=40,
+                        vmin=0.0, capacity=41)
+    r = oracle.streamlines(g2, np.array([[0.6, 1.0, 1.0]]), prm, "f64")
+    assert r.totals[0] > r.totals[1] > 0                      # some attempts were rejected
+    x = r.vertices[0, 0, :r.counts[0]]
+    y = r.vertices[1, 0, :r.counts[0]]
+    exact = 1.0 + np.where(x < 3, (2.4**2 - (3 - x)**2) / 2, 2.4**2 / 2 + (x - 3)**2 / 2)
+    assert np.max(np.abs(y - exact)) < 1e-4    # still right (kink step force-accepted at h_min)
+    # forced accept at the floor: h_min = h_max with an impossible tolerance never rejects
+    prm = oracle.params(1, h=0.5, h_min=0.5, h_max=0.5, atol=1e-30, rtol=0.0, max_steps=8,
+                        vmin=0.0)
+    r = oracle.streamlines(g2, np.array([[0.6, 1.0, 1.0]]), prm, "f64")
+    assert r.totals[0] == r.totals[1] == 8
+
+
+# ------------------------------------------------------------------------------------------
+# P9 + P10: bricks (A9) == monolithic, bit for bit; queue invariants.
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nb,N", [((2, 2, 2), 32), ((3, 2, 1), 31)])
+def test_p9_bricks_equal_monolithic(oracle, wl, nb, N):
+    f = wl.turb_field_cpu(N, 48, 1, 6, seed=2606)
+    n = 3000
+    seeds = wl.seeds_uniform(42, n, [N - 1] * 3)
+    prm = oracle.params(0, h=0.25, max_steps=400, vmin=1e-6, capacity=401)
+    mono = oracle.streamlines(oracle.grid(f.data, f.dims, f.origin, f.spacing), seeds, prm, "f32")
+    boxes = wl.brick_boxes(f.dims, nb, 1)
+    arrays = wl.cut_bricks(f, nb, 1)
+    bricks = [oracle.grid(a, None, f.origin, f.spacing, gdims=f.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(arrays, boxes)]
+    br = oracle.brick_advect(bricks, nb, seeds, prm, "f32")
+    assert np.count_nonzero(br.status == oracle.HALO_MISS) == 0
+    assert np.array_equal(br.status, mono.status) and np.array_equal(br.steps, mono.steps)
+    assert np.array_equal(br.counts, mono.counts)
+    assert np.array_equal(br.vertices, mono.vertices, equal_nan=True)
+    assert np.array_equal(br.final, mono.final)
+    assert np.array_equal(br.totals[:3], mono.totals[:3])
+    # P10 invariants
+    assert br.nrounds >= 2 and br.totals[3] == br.nlog == len(br.log)
+    B = [N // nb[a] for a in range(3)]
+    own = lambda p: sum(np.minimum(np.floor(p[:, a]).astype(int) // B[a], nb[a] - 1) *
+                        [1, nb[0], nb[0] * nb[1]][a] for a in range(3))
+    q0 = np.bincount(own(seeds), minlength=len(bricks))
+    assert np.array_equal(br.round_counts[0], q0)
+    rnd = (br.log >> np.uint64(48)).astype(int); dest = ((br.log >> np.uint64(32)) & np.uint64(0xffff)).astype(int)
+    ids = (br.log & np.uint64(0xffffffff)).astype(int)
+    for r_ in range(1, br.nrounds):
+        sel = rnd == r_
+        assert np.array_equal(np.bincount(dest[sel], minlength=len(bricks)), br.round_counts[r_])
+        assert len(np.unique(ids[sel])) == sel.sum()        # no id twice in one round
+    assert br.round_counts[1:].sum() == br.nlog
+    inside = (mono.counts > 0)
+    v = mono.vertices[:, inside, 0]
+    assert np.all(v >= 0) and np.all(v <= N - 1)
+    assert np.all(br.steps <= 400) and np.all((br.status >= 1) & (br.status <= 4))
+
+
+def test_p9_owner_and_halo_miss(oracle):
+    N, nb = 9, (2, 1, 1)
+    data = np.zeros((1, N, N, N, 3), dtype=np.float32); data[..., 0] = 1.0
+    fast = data.copy(); fast[..., 0] = 3.0
+
+    class F:  # minimal field record for cut_bricks
+        pass
+    import workloads as wl
+    for arr, expect in [(data, oracle.OUT_OF_DOMAIN), (fast, oracle.HALO_MISS)]:
+        fld = wl.Field((N, N, N), (0, 0, 0), (1, 1, 1), arr)
+        boxes = wl.brick_boxes(fld.dims, nb, 1)
+        bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+                  for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+        prm = oracle.params(0, h=1.0, max_steps=50, vmin=0.0, capacity=51)
+        seeds = np.array([[3.5, 4, 4], [4.0, 4, 4], [2.0, 4, 4]], dtype=np.float32)
+        r = oracle.brick_advect(bricks, nb, seeds, prm, "f32")
+        # B = 4: positions with floor(g) < 4 belong to brick 0, g == 4.0 (the face) to brick 1
+        assert list(r.round_counts[0]) == [2, 1]
+        if expect == oracle.OUT_OF_DOMAIN:
+            assert np.all(r.status == oracle.OUT_OF_DOMAIN)
+            assert list(r.steps) == [4, 4, 6]                 # x0 + n <= 8
+            assert r.nlog == 2                                # seeds 0 and 2 cross the face once
+        else:
+            # speed 3, h = 1: stage point p + 3 lies beyond brick 0's stored box [0, 5]
+            assert r.status[0] == oracle.HALO_MISS and r.status[2] == oracle.HALO_MISS
+            assert r.status[1] == oracle.OUT_OF_DOMAIN
+
+
+# ------------------------------------------------------------------------------------------
+# P11: streakline slot (i, j) == last vertex of the pathline from (point_i, t_j).
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_p11_streakline_is_pathline_family(oracle, wl, precision):
+    f = wl.double_gyre_field(dims=(32, 16, 8), nslices=8, dt=0.25)
+    g = oracle.grid(f.data, f.dims, f.origin, f.spacing, f.nslices, f.slice_dt)
+    pts = np.array([[0.5, 0.25, 0.3], [1.5, 0.6, 0.7], [2.5, 0.5, 0.5], [1.0, 0.999, 0.01]],
+                   dtype=np.float32)
+    h, nsteps = 0.0625, 24
+    prm = oracle.params(0, h=h, vmin=0.0, t0=0.5)
+    sk = oracle.streaklines(g, pts, nsteps, prm, precision)
+    alive = np.zeros(len(pts), dtype=int)
+    for j in range(nsteps):
+        p = oracle.params(0, h=h, max_steps=nsteps - j, vmin=0.0, t0=0.5 + j * h)
+        sl = oracle.streamlines(g, pts, p, precision)
+        assert np.array_equal(sk.vertices[:, j, :], sl.final)
+        assert np.array_equal(sk.status[j * len(pts):(j + 1) * len(pts)], sl.status)
+        alive += (sl.status == oracle.MAX_STEPS)
+    assert np.array_equal(sk.counts, alive)
+    assert sk.status[2] == oracle.OUT_OF_DOMAIN and np.array_equal(sk.vertices[:, 0, 2], pts[2])
+    # youngest release has taken exactly one step, the oldest nsteps
+    assert sk.steps[(nsteps - 1) * len(pts)] == 1 and sk.steps[0] == nsteps
