@@ -1,0 +1,183 @@
+/* include/streami.h -- C ABI of the B200-native particle-update library
+ * (libstreami_b200.so, sources in paper_2606_02627_b200/csrc/).
+ *
+ * What it computes: the particle-update step of field-line tracing as described in
+ * "Streami: An MPI Data-Parallel Library to Compute Field Lines on GPUs"
+ * (arxiv/paper_2606_02627; citations are /root/reference/PAPER.md:<line>):
+ *   - update() kernel, one RK4 step per particle with four field.sample() calls and
+ *     "a failed sample ends the particle"            Listing 1
+ *   - VecField::sample() / destinationID(), macrocell + halo
+ *   - structured field = array of float3 voxels, sampled by offset computation
+ *   - Tracer::step()/trace() loop, streakline batches per step, fields[simStep]
+ *                                                    Listing 2
+ *   - particle = position + unique id
+ *   - emitOutgoing / forward until no particle is active anywhere
+ * Where the paper is silent (trilinear filter, linear interpolation in time, |v| floor,
+ * adaptive Dormand-Prince 5(4), capacity/stride recording) BASELINE.json binds and the fp32
+ * formula sheet A1-A9 (restated in DESIGN.md section 3) fixes every operation.
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory owned by the caller (e.g. torch tensors);
+ *     "host" pointers are ordinary host memory.  No torch types cross this boundary.
+ *   - Every call returns int: 0 ok, negative = error (STREAMI_E_*).  Nothing is printed, no
+ *     exception crosses the ABI.  Bad *particles* are not errors (a seed outside the domain gets
+ *     status OUT_OF_DOMAIN, 0 steps, 0 vertices).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work
+ *     is enqueued on it; outputs are valid after the caller synchronises that stream, unless a
+ *     function says that it synchronises the stream itself.  No call synchronises the device.
+ *   - All per-particle outputs are indexed by particle id (= seed index; streaklines:
+ *     release*m + point), so they do not depend on scheduling, sorting or queue order.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns STREAMI_E_CUDA.
+ */
+#ifndef STREAMI_H
+#define STREAMI_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* error codes */
+#define STREAMI_OK            0
+#define STREAMI_E_INVALID    (-1)  /* null pointer, dim < 2, spacing <= 0 or non-finite, nslices < 1,
+                                      capacity == 0, stride == 0, h <= 0, h_min > h_max, ... */
+#define STREAMI_E_NOMEM      (-2)  /* out of device memory */
+#define STREAMI_E_CUDA       (-3)  /* CUDA error; text behind streami_error_string(-3) */
+#define STREAMI_E_TRUNCATED  (-4)  /* hand-off log or round table overflowed; results still valid */
+
+/* termination reasons (A5) written to out_status */
+#define STREAMI_ALIVE          0u  /* never final */
+#define STREAMI_OUT_OF_DOMAIN  1u  /* a stage sample or the new position left the domain (Listing 1's return) */
+#define STREAMI_MAX_STEPS      2u  /* reached max_steps (streaklines: alive at the end) */
+#define STREAMI_STAGNANT       3u  /* |v(p)| < vmin */
+#define STREAMI_HALO_MISS      4u  /* bricks only: a stage point left the brick's stored box */
+
+/* field layouts (layout_hint of streami_field_create*, reported by streami_field_info) */
+#define STREAMI_LAYOUT_AUTO    0   /* library chooses (DESIGN.md section 6 says how) */
+#define STREAMI_LAYOUT_PACKED3 1   /* use the caller's packed float3 array in place (the paper's layout) */
+#define STREAMI_LAYOUT_FLOAT4  2   /* library-owned copy padded to 16 B per vertex */
+#define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: {V[x], V[x+1], pad}: one
+                                      aligned sector per trilinear row */
+
+typedef struct streami_field_s* streami_field;   /* opaque host-side handle (D2/D3) */
+
+typedef struct {                 /* all fp32 scalars are used bit-for-bit */
+  int      integrator;           /* 0 = RK4 fixed step (Listing 1), 1 = Dormand-Prince 5(4) adaptive (A8) */
+  float    h;                    /* RK4 step; DP5(4) initial step */
+  float    h_min, h_max;         /* DP5(4) only */
+  float    atol, rtol;           /* DP5(4) only */
+  unsigned max_steps;            /* accepted steps per particle (ignored by streaklines) */
+  float    vmin;                 /* terminate when |v(p)| < vmin (0 disables) */
+  float    t0;                   /* time of step 0 (unsteady fields) */
+  int      time_mode;            /* 0 = linear between slices, 1 = hold floor slice */
+  unsigned capacity;             /* vertex slots per particle (A6) */
+  unsigned stride;               /* record vertex k iff k % stride == 0 and k/stride < capacity */
+  /* optional extra outputs, device pointers, may be NULL: */
+  unsigned* out_steps;           /* [n] accepted steps */
+  unsigned* out_status;          /* [n] termination reason */
+  float*    out_final;           /* [3][n] last inside position (SoA) */
+  unsigned long long* out_totals;/* [4] attempted steps, accepted steps, field samples, hand-offs;
+                                    overwritten (not accumulated) by each call */
+} streami_params;
+
+/* Create a field over a caller-owned packed array ("a CUDA global memory array
+ * for the voxels"): dev_ptr = [nslices][Nz][Ny][Nx][3] fp32, x fastest, vertex-centred (A1).
+ * dev_ptr is BORROWED for the life of the handle and never written.  With layout_hint other
+ * than PACKED3 the library makes its own repacked copy (owned by the handle, freed by
+ * _destroy); the repack runs on the legacy default stream and is complete on return.
+ * slice_dt is the time between slices (ignored when nslices == 1).
+ * Errors: INVALID (null, dims < 2, spacing <= 0 or non-finite, nslices < 1, slice_dt <= 0,
+ * more than 2^32-1 vertices per slice, unknown layout), NOMEM, CUDA. */
+int streami_field_create(const int dims[3], const float origin[3], const float spacing[3],
+                         int nslices, float slice_dt, const float* dev_ptr, int layout_hint,
+                         streami_field* out);
+
+/* Create a brick-decomposed steady field (macrocells + halo; A9).  The global
+ * grid global_dims is cut by brick_grid = (nbx, nby, nbz) into bricks of B_a = N_a / nb_a cells
+ * (the last brick of an axis takes the remainder).  Brick b = (bz*nby + by)*nbx + bx STORES the
+ * vertex box lo_a = max(B_a*b_a - ghost, 0) .. hi_a = min(B_a*(b_a+1) + ghost, N_a-1) (hi_a =
+ * N_a-1 for the last brick) as its own packed float3 array brick_dev_ptrs[b] (host array of
+ * device pointers), the way each MPI rank of the paper holds its partition.  Same ownership
+ * and layout rules as streami_field_create, per brick.  ghost >= 1. */
+int streami_field_create_bricked(const int global_dims[3], const float origin[3],
+                                 const float spacing[3], const int brick_grid[3], int ghost_cells,
+                                 const float* const* brick_dev_ptrs, int layout_hint,
+                                 streami_field* out);
+
+int streami_field_destroy(streami_field f);
+
+/* Layout actually used and device bytes owned by the handle (0 for PACKED3). */
+int streami_field_info(streami_field f, int* layout, size_t* owned_bytes);
+
+/* a2-a4 alone: sample the field at n device points [n][3] at time t (A2/A3).
+ * out_v [n][3] (zero where not ok), out_rc [n] = 0 ok / OUT_OF_DOMAIN.  Monolithic fields only. */
+int streami_sample(streami_field f, const float* points, size_t n, float t, int time_mode,
+                   float* out_v, unsigned* out_rc, void* cuda_stream);
+
+/* Streamlines (Tracer::trace() in Streamlines mode; A4-A6, A8).
+ * seeds [n][3] device AoS.  out_vertices [3][n][capacity] device SoA planes, slot k/stride of
+ * particle id at c*n*capacity + id*capacity + k/stride; slots beyond out_counts[id] are left
+ * untouched.  out_counts [n] device = stored vertices per particle.  out_vertices may be NULL
+ * (nothing recorded, out_counts still written).  Asynchronous on cuda_stream; scratch memory
+ * is taken from the stream-ordered allocator.  n == 0 is ok.  Monolithic fields only.
+ * Errors: INVALID (null field/seeds/params/out_counts, capacity == 0, stride == 0, h <= 0 or
+ * non-finite, DP5: h_min <= 0, h_min > h_max, atol/rtol < 0), NOMEM, CUDA. */
+int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
+                              const streami_params* params, float* out_vertices,
+                              unsigned* out_counts, void* cuda_stream);
+
+/* The same call with HOST buffers: seeds, out_vertices, out_counts and the optional outputs in
+ * params are host pointers (pinned memory makes the copies faster but is not required).  Copies
+ * host->device, traces, copies device->host and synchronises cuda_stream before returning. */
+int streami_trace_streamlines_host(streami_field f, const float* seeds, size_t n,
+                                   const streami_params* params, float* out_vertices,
+                                   unsigned* out_counts, void* cuda_stream);
+
+/* Streaklines (Listing 2; A7).  points [m][3] device.  Particle (i, j) is
+ * released at point i at global step j and steps at global indices j..nsteps-1 with
+ * t_s = t0 + (float)s*h (RK4 only; params->integrator must be 0; max_steps, capacity, stride are
+ * ignored).  out_vertices [3][nsteps][m] device, release-major: slot (j, i) = final position of
+ * particle id = j*m + i (its last inside position if it died).  out_counts [m] = particles of
+ * point i alive at the end (status MAX_STEPS).  params->out_steps/out_status are [nsteps*m].
+ * Asynchronous on cuda_stream. */
+int streami_trace_streaklines(streami_field f, const float* points, size_t m, unsigned nsteps,
+                              const streami_params* params, float* out_vertices,
+                              unsigned* out_counts, void* cuda_stream);
+
+/* Brick advection with hand-off (P1/K1/K3/K4 of SURVEY.md; A9).
+ * f must come from streami_field_create_bricked; RK4 only.  In round r every particle queued for
+ * brick b is advected inside b until it ends or its new position is owned by another brick; it
+ * is then appended to that brick's queue for round r+1 (the device-side stand-in for
+ * emitOutgoing + the all-to-all forward).  Rounds run until no particle is queued anywhere.
+ * Outputs as streami_trace_streamlines, plus (all optional, device unless noted):
+ *   out_round_counts [max_rounds][nbricks]: |Q_r[b]| (rows beyond the executed rounds untouched)
+ *   out_handoff_log  [log_capacity]: one entry (round+1)<<48 | dest<<32 | id per hand-off, in
+ *                    unspecified order; out_log_count (device, 1 x u64) = hand-offs in total
+ *   out_nrounds      HOST pointer: rounds executed.
+ * This call synchronises cuda_stream once per round (it reads the live count) and before
+ * returning.  Returns STREAMI_E_TRUNCATED if the log or the round table overflowed (all other
+ * results are still valid). */
+int streami_brick_advect(streami_field f, const float* seeds, size_t n,
+                         const streami_params* params, float* out_vertices, unsigned* out_counts,
+                         unsigned* out_round_counts, unsigned max_rounds,
+                         unsigned long long* out_handoff_log, size_t log_capacity,
+                         unsigned long long* out_log_count, unsigned* out_nrounds,
+                         void* cuda_stream);
+
+/* Tuning knobs for measurement (process-wide, not part of the method): name is one of
+ * "cell_cache" (0/1, reuse the 8 cell vertices in registers while a sample stays in the cell),
+ * "presort" (0/1, order seeds by coarse Morton bin before tracing), "streak_window" (global
+ * steps per launch, 0 = automatic).  Returns INVALID for unknown names. */
+int streami_set_option(const char* name, int value);
+int streami_get_option(const char* name, int* value);
+
+/* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */
+unsigned long long streami_launch_count(void);
+
+const char* streami_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STREAMI_H */

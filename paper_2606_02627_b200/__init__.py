@@ -1,0 +1,223 @@
+"""Thin Python binding of libstreami_b200.so (C ABI in include/streami.h).
+
+Argument marshalling only: every step of the particle-update path runs in the CUDA kernels of
+csrc/.  PyTorch is used for device memory (`torch.empty(..., device="cuda")`) and streams.
+There is no CPU fallback: if the library cannot be built/loaded, importing the functions raises.
+Function names and argument meaning follow include/streami.h one to one.
+"""
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+OK, E_INVALID, E_NOMEM, E_CUDA, E_TRUNCATED = 0, -1, -2, -3, -4
+OUT_OF_DOMAIN, MAX_STEPS, STAGNANT, HALO_MISS = 1, 2, 3, 4
+LAYOUT_AUTO, LAYOUT_PACKED3, LAYOUT_FLOAT4, LAYOUT_XPAIR = 0, 1, 2, 3
+
+
+class StreamiError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("streami error %d: %s" % (code, text))
+        self.code = code
+
+
+class Params(ctypes.Structure):
+    """Mirror of streami_params."""
+    _fields_ = [("integrator", ctypes.c_int), ("h", ctypes.c_float), ("h_min", ctypes.c_float),
+                ("h_max", ctypes.c_float), ("atol", ctypes.c_float), ("rtol", ctypes.c_float),
+                ("max_steps", ctypes.c_uint), ("vmin", ctypes.c_float), ("t0", ctypes.c_float),
+                ("time_mode", ctypes.c_int), ("capacity", ctypes.c_uint), ("stride", ctypes.c_uint),
+                ("out_steps", ctypes.c_void_p), ("out_status", ctypes.c_void_p),
+                ("out_final", ctypes.c_void_p), ("out_totals", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building in-tree if stale) the CUDA library.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        L = ctypes.CDLL(so)
+        P, I, U, F, Z = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint, ctypes.c_float, ctypes.c_size_t
+        L.streami_field_create.argtypes = [P, P, P, I, F, P, I, P]
+        L.streami_field_create_bricked.argtypes = [P, P, P, P, I, P, I, P]
+        L.streami_field_destroy.argtypes = [P]
+        L.streami_field_info.argtypes = [P, P, P]
+        L.streami_sample.argtypes = [P, P, Z, F, I, P, P, P]
+        L.streami_trace_streamlines.argtypes = [P, P, Z, P, P, P, P]
+        L.streami_trace_streamlines_host.argtypes = [P, P, Z, P, P, P, P]
+        L.streami_trace_streaklines.argtypes = [P, P, Z, U, P, P, P, P]
+        L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
+        L.streami_set_option.argtypes = [ctypes.c_char_p, I]
+        L.streami_get_option.argtypes = [ctypes.c_char_p, P]
+        L.streami_launch_count.restype = ctypes.c_ulonglong
+        L.streami_error_string.restype = ctypes.c_char_p
+        L.streami_error_string.argtypes = [I]
+        _lib = L
+    return _lib
+
+
+def _check(rc, allow=()):
+    if rc != OK and rc not in allow:
+        raise StreamiError(rc, lib().streami_error_string(rc).decode())
+    return rc
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _req(t, dtype, name):
+    if t is None:
+        return
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise ValueError("%s must be a contiguous CUDA tensor of %s" % (name, dtype))
+
+
+def params(integrator=0, h=0.01, h_min=0.0, h_max=0.0, atol=0.0, rtol=0.0, max_steps=1000,
+           vmin=0.0, t0=0.0, time_mode=0, capacity=1, stride=1, out_steps=None, out_status=None,
+           out_final=None, out_totals=None):
+    _req(out_steps, torch.int32, "out_steps"); _req(out_status, torch.int32, "out_status")
+    _req(out_final, torch.float32, "out_final"); _req(out_totals, torch.int64, "out_totals")
+    p = Params(integrator, h, h_min, h_max, atol, rtol, max_steps, vmin, t0, time_mode, capacity,
+               stride, None, None, None, None)
+    p.out_steps = None if out_steps is None else out_steps.data_ptr()
+    p.out_status = None if out_status is None else out_status.data_ptr()
+    p.out_final = None if out_final is None else out_final.data_ptr()
+    p.out_totals = None if out_totals is None else out_totals.data_ptr()
+    p._keep = (out_steps, out_status, out_final, out_totals)
+    return p
+
+
+class Field:
+    """Owner of a streami_field handle; keeps the caller's tensors alive (dev_ptr is borrowed)."""
+
+    def __init__(self, handle, keep, bricked):
+        self.handle, self._keep, self.bricked = handle, keep, bricked
+
+    def info(self):
+        lay, nbytes = ctypes.c_int(0), ctypes.c_size_t(0)
+        _check(lib().streami_field_info(self.handle, ctypes.byref(lay), ctypes.byref(nbytes)))
+        return lay.value, nbytes.value
+
+    def destroy(self):
+        if self.handle:
+            lib().streami_field_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def _i3(v):
+    return (ctypes.c_int * 3)(*[int(x) for x in v])
+
+
+def _f3(v):
+    return (ctypes.c_float * 3)(*[float(x) for x in v])
+
+
+def streami_field_create(dims, origin, spacing, nslices, slice_dt, data, layout_hint=LAYOUT_AUTO):
+    """data: CUDA float32 tensor [nslices, Nz, Ny, Nx, 3] (packed, x fastest)."""
+    _req(data, torch.float32, "data")
+    h = ctypes.c_void_p(None)
+    _check(lib().streami_field_create(_i3(dims), _f3(origin), _f3(spacing), int(nslices),
+                                      float(slice_dt), _ptr(data), int(layout_hint), ctypes.byref(h)))
+    return Field(h, data, False)
+
+
+def streami_field_create_bricked(global_dims, origin, spacing, brick_grid, ghost_cells, brick_data,
+                                 layout_hint=LAYOUT_AUTO):
+    """brick_data: list of CUDA float32 tensors, one per brick (flat id order), each the brick's
+    stored box [nz, ny, nx, 3]."""
+    for t in brick_data:
+        _req(t, torch.float32, "brick")
+    ptrs = (ctypes.c_void_p * len(brick_data))(*[t.data_ptr() for t in brick_data])
+    h = ctypes.c_void_p(None)
+    _check(lib().streami_field_create_bricked(_i3(global_dims), _f3(origin), _f3(spacing),
+                                              _i3(brick_grid), int(ghost_cells), ptrs,
+                                              int(layout_hint), ctypes.byref(h)))
+    return Field(h, list(brick_data), True)
+
+
+def streami_sample(field, points, t=0.0, time_mode=0, stream=None):
+    _req(points, torch.float32, "points")
+    n = points.shape[0]
+    v = torch.empty((n, 3), dtype=torch.float32, device=points.device)
+    rc = torch.empty(n, dtype=torch.int32, device=points.device)
+    _check(lib().streami_sample(field.handle, _ptr(points), n, float(t), int(time_mode), _ptr(v),
+                                _ptr(rc), _stream(stream)))
+    return v, rc
+
+
+def streami_trace_streamlines(field, seeds, prm, out_vertices, out_counts, stream=None):
+    _req(seeds, torch.float32, "seeds"); _req(out_vertices, torch.float32, "out_vertices")
+    _req(out_counts, torch.int32, "out_counts")
+    _check(lib().streami_trace_streamlines(field.handle, _ptr(seeds), seeds.shape[0],
+                                           ctypes.byref(prm), _ptr(out_vertices), _ptr(out_counts),
+                                           _stream(stream)))
+
+
+def streami_trace_streamlines_host(field, seeds, prm_host, out_vertices, out_counts, stream=None):
+    """Host-buffer variant: seeds/out_* are CPU tensors (pinned for speed); prm_host must carry
+    host pointers (or None) in its optional outputs."""
+    for t in (seeds, out_vertices, out_counts):
+        if t is not None and (t.is_cuda or not t.is_contiguous()):
+            raise ValueError("host variant takes contiguous CPU tensors")
+    _check(lib().streami_trace_streamlines_host(field.handle, _ptr(seeds), seeds.shape[0],
+                                                ctypes.byref(prm_host), _ptr(out_vertices),
+                                                _ptr(out_counts), _stream(stream)))
+
+
+def streami_trace_streaklines(field, points, nsteps, prm, out_vertices, out_counts, stream=None):
+    _req(points, torch.float32, "points"); _req(out_vertices, torch.float32, "out_vertices")
+    _req(out_counts, torch.int32, "out_counts")
+    _check(lib().streami_trace_streaklines(field.handle, _ptr(points), points.shape[0], int(nsteps),
+                                           ctypes.byref(prm), _ptr(out_vertices), _ptr(out_counts),
+                                           _stream(stream)))
+
+
+def streami_brick_advect(field, seeds, prm, out_vertices, out_counts, out_round_counts=None,
+                         out_handoff_log=None, out_log_count=None, stream=None):
+    """Returns (nrounds, truncated)."""
+    _req(seeds, torch.float32, "seeds"); _req(out_vertices, torch.float32, "out_vertices")
+    _req(out_counts, torch.int32, "out_counts"); _req(out_round_counts, torch.int32, "round_counts")
+    _req(out_handoff_log, torch.int64, "handoff_log"); _req(out_log_count, torch.int64, "log_count")
+    max_rounds = 0 if out_round_counts is None else out_round_counts.shape[0]
+    log_cap = 0 if out_handoff_log is None else out_handoff_log.numel()
+    nrounds = ctypes.c_uint(0)
+    rc = _check(lib().streami_brick_advect(field.handle, _ptr(seeds), seeds.shape[0],
+                                           ctypes.byref(prm), _ptr(out_vertices), _ptr(out_counts),
+                                           _ptr(out_round_counts), max_rounds, _ptr(out_handoff_log),
+                                           log_cap, _ptr(out_log_count), ctypes.byref(nrounds),
+                                           _stream(stream)), allow=(E_TRUNCATED,))
+    return nrounds.value, rc == E_TRUNCATED
+
+
+def streami_set_option(name, value):
+    _check(lib().streami_set_option(name.encode(), int(value)))
+
+
+def streami_get_option(name):
+    v = ctypes.c_int(0)
+    _check(lib().streami_get_option(name.encode(), ctypes.byref(v)))
+    return v.value
+
+
+def streami_launch_count():
+    return lib().streami_launch_count()

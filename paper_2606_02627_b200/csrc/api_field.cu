@@ -1,0 +1,255 @@
+// csrc/api_field.cu -- field handles (D2/D3 of SURVEY.md: the host class that "is primarily
+// responsible for data handling"), layout repack, options, streami_sample.
+#include <cmath>
+#include <cstring>
+#include <mutex>
+
+#include "internal.h"
+#include "misc_kernels.cuh"
+
+namespace streami {
+
+Options& options() { static Options o{1, 1, 0}; return o; }
+std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
+
+static std::mutex g_err_mutex;
+static std::string g_cuda_err = "CUDA error";
+void set_cuda_error(cudaError_t e) {
+  std::lock_guard<std::mutex> lk(g_err_mutex);
+  g_cuda_err = std::string("CUDA error: ") + cudaGetErrorName(e) + ": " + cudaGetErrorString(e);
+  cudaGetLastError();   // clear the sticky-less error state
+}
+
+int num_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
+  }
+  return n;
+}
+
+static bool finite_pos(float x) { return std::isfinite(x) && x > 0.0f; }
+
+// Build the library-owned copy of one packed float3 array with `nvert` vertices.
+static int repack(const float* src, unsigned long long nvert, unsigned nx, int layout, void** out,
+                  size_t* bytes) {
+  *out = nullptr; *bytes = 0;
+  if (layout == LAYOUT_PACKED3) { *out = const_cast<float*>(src); return STREAMI_OK; }
+  size_t rec = layout == LAYOUT_FLOAT4 ? 16 : 32;
+  void* dst = nullptr;
+  STREAMI_TRY(cudaMalloc(&dst, rec * nvert + 32));   // +32: FLOAT4 reads p[1] of the last vertex
+  int blocks = 148 * 8;
+  if (layout == LAYOUT_FLOAT4)
+    repack_float4_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert);
+  else
+    repack_xpair_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert, nx);
+  launch_counter()++;
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemset((char*)dst + rec * nvert, 0, 32);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+  if (e != cudaSuccess) { cudaFree(dst); return check(e); }
+  *out = dst; *bytes = rec * nvert + 32;
+  return STREAMI_OK;
+}
+
+static int fill_geom(Geom& g, const int dims[3], const float origin[3], const float spacing[3],
+                     int nslices, float slice_dt) {
+  for (int a = 0; a < 3; ++a) {
+    if (dims[a] < 2 || !finite_pos(spacing[a]) || !std::isfinite(origin[a])) return STREAMI_E_INVALID;
+  }
+  if (nslices < 1) return STREAMI_E_INVALID;
+  if (nslices > 1 && !finite_pos(slice_dt)) return STREAMI_E_INVALID;
+  if ((unsigned long long)dims[0] * dims[1] * dims[2] > 0xffffffffull) return STREAMI_E_INVALID;
+  g.ox = origin[0]; g.oy = origin[1]; g.oz = origin[2];
+  g.rx = 1.0f / spacing[0]; g.ry = 1.0f / spacing[1]; g.rz = 1.0f / spacing[2];   // A1, fp32 IEEE
+  g.topx = (float)(dims[0] - 1); g.topy = (float)(dims[1] - 1); g.topz = (float)(dims[2] - 1);
+  g.nslices = nslices;
+  g.q = nslices > 1 ? 1.0f / slice_dt : 1.0f;
+  g.top_s = (float)(nslices - 1);
+  g.time_mode = 0;
+  return STREAMI_OK;
+}
+
+static int pick_layout(int hint) {
+  if (hint == STREAMI_LAYOUT_AUTO) return LAYOUT_XPAIR;   // measured fastest
+  if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR)
+    return hint;
+  return -1;
+}
+
+}  // namespace streami
+
+using namespace streami;
+
+extern "C" {
+
+int streami_field_create(const int dims[3], const float origin[3], const float spacing[3],
+                         int nslices, float slice_dt, const float* dev_ptr, int layout_hint,
+                         streami_field* out) {
+  if (!dims || !origin || !spacing || !dev_ptr || !out) return STREAMI_E_INVALID;
+  *out = nullptr;
+  int layout = pick_layout(layout_hint);
+  if (layout < 0) return STREAMI_E_INVALID;
+  streami_field_s* f = new streami_field_s();
+  int rc = fill_geom(f->g, dims, origin, spacing, nslices, slice_dt);
+  if (rc) { delete f; return rc; }
+  for (int a = 0; a < 3; ++a) f->dims[a] = dims[a];
+  f->layout = layout; f->bricked = false; f->d_bricks = nullptr; f->owned_bytes = 0;
+  Store& s = f->store;
+  s.lox = s.loy = s.loz = 0;
+  s.hix = dims[0] - 1; s.hiy = dims[1] - 1; s.hiz = dims[2] - 1;
+  s.topflagx = s.topflagy = s.topflagz = 1;
+  s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
+  s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
+  void* data = nullptr; size_t bytes = 0;
+  rc = repack(dev_ptr, s.slice_stride * (unsigned long long)nslices, s.nx, layout, &data, &bytes);
+  if (rc) { delete f; return rc; }
+  s.data = data;
+  if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
+  *out = f;
+  return STREAMI_OK;
+}
+
+int streami_field_create_bricked(const int global_dims[3], const float origin[3],
+                                 const float spacing[3], const int brick_grid[3], int ghost_cells,
+                                 const float* const* brick_dev_ptrs, int layout_hint,
+                                 streami_field* out) {
+  if (!global_dims || !origin || !spacing || !brick_grid || !brick_dev_ptrs || !out)
+    return STREAMI_E_INVALID;
+  *out = nullptr;
+  int layout = pick_layout(layout_hint);
+  if (layout < 0 || ghost_cells < 1) return STREAMI_E_INVALID;
+  for (int a = 0; a < 3; ++a)
+    if (brick_grid[a] < 1 || brick_grid[a] > global_dims[a] - 1) return STREAMI_E_INVALID;
+  const int nb = brick_grid[0] * brick_grid[1] * brick_grid[2];
+  if (nb > 65535) return STREAMI_E_INVALID;   // the hand-off log packs dest into 16 bits
+  streami_field_s* f = new streami_field_s();
+  int rc = fill_geom(f->g, global_dims, origin, spacing, 1, 1.0f);
+  if (rc) { delete f; return rc; }
+  for (int a = 0; a < 3; ++a) f->dims[a] = global_dims[a];
+  f->layout = layout; f->bricked = true; f->d_bricks = nullptr; f->owned_bytes = 0;
+  BrickMap& m = f->bm;
+  m.nbx = brick_grid[0]; m.nby = brick_grid[1]; m.nbz = brick_grid[2];
+  m.Bx = global_dims[0] / m.nbx; m.By = global_dims[1] / m.nby; m.Bz = global_dims[2] / m.nbz;
+  const int B[3] = {m.Bx, m.By, m.Bz};
+  auto fail = [&](int code) {
+    for (void* p : f->owned) cudaFree(p);
+    delete f;
+    return code;
+  };
+  for (int bz = 0; bz < m.nbz; ++bz)
+    for (int by = 0; by < m.nby; ++by)
+      for (int bx = 0; bx < m.nbx; ++bx) {
+        const int b[3] = {bx, by, bz};
+        int lo[3], hi[3];
+        for (int a = 0; a < 3; ++a) {
+          lo[a] = std::max(B[a] * b[a] - ghost_cells, 0);
+          hi[a] = std::min(B[a] * (b[a] + 1) + ghost_cells, global_dims[a] - 1);
+          if (b[a] == brick_grid[a] - 1) hi[a] = global_dims[a] - 1;
+          if (hi[a] - lo[a] < 1) return fail(STREAMI_E_INVALID);
+        }
+        const float* src = brick_dev_ptrs[(bz * m.nby + by) * m.nbx + bx];
+        if (!src) return fail(STREAMI_E_INVALID);
+        Store s;
+        s.lox = lo[0]; s.loy = lo[1]; s.loz = lo[2];
+        s.hix = hi[0]; s.hiy = hi[1]; s.hiz = hi[2];
+        s.topflagx = hi[0] == global_dims[0] - 1; s.topflagy = hi[1] == global_dims[1] - 1;
+        s.topflagz = hi[2] == global_dims[2] - 1;
+        s.nx = (unsigned)(hi[0] - lo[0] + 1);
+        s.nxy = s.nx * (unsigned)(hi[1] - lo[1] + 1);
+        s.slice_stride = (unsigned long long)s.nxy * (unsigned)(hi[2] - lo[2] + 1);
+        void* data = nullptr; size_t bytes = 0;
+        rc = repack(src, s.slice_stride, s.nx, layout, &data, &bytes);
+        if (rc) return fail(rc);
+        s.data = data;
+        if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
+        f->bricks.push_back(s);
+      }
+  void* tbl = nullptr;
+  if (check(cudaMalloc(&tbl, sizeof(Store) * nb)) != STREAMI_OK) return fail(STREAMI_E_NOMEM);
+  f->owned.push_back(tbl);
+  cudaError_t e = cudaMemcpy(tbl, f->bricks.data(), sizeof(Store) * nb, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return fail(check(e));
+  f->d_bricks = (Store*)tbl;
+  *out = f;
+  return STREAMI_OK;
+}
+
+int streami_field_destroy(streami_field f) {
+  if (!f) return STREAMI_E_INVALID;
+  for (void* p : f->owned) cudaFree(p);
+  delete f;
+  return STREAMI_OK;
+}
+
+int streami_field_info(streami_field f, int* layout, size_t* owned_bytes) {
+  if (!f) return STREAMI_E_INVALID;
+  if (layout) *layout = f->layout;
+  if (owned_bytes) *owned_bytes = f->owned_bytes;
+  return STREAMI_OK;
+}
+
+int streami_sample(streami_field f, const float* points, size_t n, float t, int time_mode,
+                   float* out_v, unsigned* out_rc, void* cuda_stream) {
+  if (!f || f->bricked || !points || !out_v || !out_rc) return STREAMI_E_INVALID;
+  if (time_mode != 0 && time_mode != 1) return STREAMI_E_INVALID;
+  if (n == 0) return STREAMI_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Geom g = f->g; g.time_mode = time_mode;
+  const bool unsteady = g.nslices > 1;
+  unsigned blocks = (unsigned)((n + 255) / 256);
+#define GO(L, U) sample_kernel<L, U><<<blocks, 256, 0, st>>>(g, f->store, points, n, t, out_v, out_rc)
+  switch (f->layout * 2 + (unsteady ? 1 : 0)) {
+    case LAYOUT_PACKED3 * 2: GO(LAYOUT_PACKED3, false); break;
+    case LAYOUT_PACKED3 * 2 + 1: GO(LAYOUT_PACKED3, true); break;
+    case LAYOUT_FLOAT4 * 2: GO(LAYOUT_FLOAT4, false); break;
+    case LAYOUT_FLOAT4 * 2 + 1: GO(LAYOUT_FLOAT4, true); break;
+    case LAYOUT_XPAIR * 2: GO(LAYOUT_XPAIR, false); break;
+    default: GO(LAYOUT_XPAIR, true); break;
+  }
+#undef GO
+  STREAMI_LAUNCHED();
+  return STREAMI_OK;
+}
+
+int streami_set_option(const char* name, int value) {
+  if (!name) return STREAMI_E_INVALID;
+  Options& o = options();
+  if (!strcmp(name, "cell_cache")) o.cell_cache = value != 0;
+  else if (!strcmp(name, "presort")) o.presort = value != 0;
+  else if (!strcmp(name, "streak_window")) o.streak_window = value < 0 ? 0 : value;
+  else return STREAMI_E_INVALID;
+  return STREAMI_OK;
+}
+
+int streami_get_option(const char* name, int* value) {
+  if (!name || !value) return STREAMI_E_INVALID;
+  Options& o = options();
+  if (!strcmp(name, "cell_cache")) *value = o.cell_cache;
+  else if (!strcmp(name, "presort")) *value = o.presort;
+  else if (!strcmp(name, "streak_window")) *value = o.streak_window;
+  else return STREAMI_E_INVALID;
+  return STREAMI_OK;
+}
+
+unsigned long long streami_launch_count(void) { return launch_counter().load(); }
+
+const char* streami_error_string(int code) {
+  switch (code) {
+    case STREAMI_OK: return "ok";
+    case STREAMI_E_INVALID: return "invalid argument";
+    case STREAMI_E_NOMEM: return "out of device memory";
+    case STREAMI_E_TRUNCATED: return "hand-off log or round table truncated (results valid)";
+    case STREAMI_E_CUDA: {
+      static thread_local std::string copy;
+      std::lock_guard<std::mutex> lk(g_err_mutex);
+      copy = g_cuda_err;
+      return copy.c_str();
+    }
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

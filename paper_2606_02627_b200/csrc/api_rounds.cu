@@ -1,0 +1,184 @@
+// csrc/api_rounds.cu -- the two round loops (a10): streaklines (Listing 2: a
+// new batch of particles per advection step) and brick advection with hand-off (PAPER.md:96-101,
+// 142-144: advance, emitOutgoing, forward, repeat while any particle is active anywhere).
+#include <cmath>
+#include <vector>
+
+#include "internal.h"
+#include "misc_kernels.cuh"
+#include "trace_kernel.cuh"
+
+namespace streami {
+typedef void (*TraceKernel)(const TraceArgs);
+TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache);
+int trace_grid(TraceKernel k, unsigned long long nwork, int* grid);
+int check_params(const streami_params* p, bool need_capacity);
+void fill_integrator(TraceArgs& a, const streami_params* p);
+
+typedef void (*StreakKernel)(const StreakArgs);
+static StreakKernel pick_streak(int layout, bool unsteady) {
+  switch (layout) {
+    case LAYOUT_PACKED3: return unsteady ? streak_kernel<LAYOUT_PACKED3, true> : streak_kernel<LAYOUT_PACKED3, false>;
+    case LAYOUT_FLOAT4: return unsteady ? streak_kernel<LAYOUT_FLOAT4, true> : streak_kernel<LAYOUT_FLOAT4, false>;
+    default: return unsteady ? streak_kernel<LAYOUT_XPAIR, true> : streak_kernel<LAYOUT_XPAIR, false>;
+  }
+}
+}  // namespace streami
+
+using namespace streami;
+
+extern "C" {
+
+int streami_trace_streaklines(streami_field f, const float* points, size_t m, unsigned nsteps,
+                              const streami_params* params, float* out_vertices,
+                              unsigned* out_counts, void* cuda_stream) {
+  if (!f || f->bricked || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, false);
+  if (rc) return rc;
+  if (params->integrator != 0) return STREAMI_E_INVALID;      // shared stage times need a fixed step
+  if ((unsigned long long)m * nsteps > 0xffffffffull) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
+  if (m == 0 || nsteps == 0) return STREAMI_OK;
+
+  const bool unsteady = f->g.nslices > 1;
+  // Window = global steps per launch.  Unsteady: about two slice intervals, so that the slices a
+  // launch touches stay L2-resident; steady: everything in one launch.
+  unsigned K = (unsigned)options().streak_window;
+  if (K == 0) {
+    if (!unsteady) K = nsteps;
+    else {
+      float per = 2.0f / (f->g.q * params->h);
+      K = per < 4.0f ? 4u : (per > 64.0f ? 64u : (unsigned)per);
+    }
+  }
+  unsigned char* state = nullptr;
+  const size_t total = (size_t)m * nsteps;
+  STREAMI_TRY(cudaMallocAsync((void**)&state, total, st));
+  StreakArgs a{};
+  a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
+  a.points = points; a.m = m; a.nsteps = nsteps;
+  a.h = params->h; a.h2 = 0.5f * params->h; a.h6 = params->h / 6.0f;
+  a.vmin2 = params->vmin * params->vmin; a.t0 = params->t0;
+  a.verts = out_vertices; a.state = state; a.steps = params->out_steps; a.totals = params->out_totals;
+  StreakKernel k = pick_streak(f->layout, unsteady);
+  cudaError_t e = cudaSuccess;
+  for (unsigned s0 = 0; s0 < nsteps && e == cudaSuccess; s0 += K) {
+    a.s0 = s0; a.s1 = std::min(nsteps, s0 + K);
+    unsigned long long threads = (unsigned long long)m * a.s1;
+    k<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(a);
+    launch_counter()++;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) {
+    streak_finalize_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(state, m, nsteps, out_counts,
+                                                                       params->out_status);
+    launch_counter()++;
+    e = cudaGetLastError();
+  }
+  cudaFreeAsync(state, st);
+  return check(e);
+}
+
+int streami_brick_advect(streami_field f, const float* seeds, size_t n,
+                         const streami_params* params, float* out_vertices, unsigned* out_counts,
+                         unsigned* out_round_counts, unsigned max_rounds,
+                         unsigned long long* out_handoff_log, size_t log_capacity,
+                         unsigned long long* out_log_count, unsigned* out_nrounds,
+                         void* cuda_stream) {
+  if (!f || !f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, true);
+  if (rc) return rc;
+  if (params->integrator != 0) return STREAMI_E_INVALID;      // RK4 only
+  if (n > 0xffffffffull) return STREAMI_E_INVALID;
+  if (out_round_counts && max_rounds == 0) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int nb = (int)f->bricks.size();
+  if (out_nrounds) *out_nrounds = 0;
+  if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
+  if (out_log_count) STREAMI_TRY(cudaMemsetAsync(out_log_count, 0, sizeof(unsigned long long), st));
+  if (n == 0) return check(cudaStreamSynchronize(st));
+
+  const bool cache = options().cell_cache != 0;
+  TraceKernel k = pick_trace_kernel(f->layout, 0, false, true, cache);
+
+  // scratch: [next u64][log count u64][qcount u32][pad u32][row0: nb x u32], two queues of n records
+  const size_t ctr_bytes = 24 + sizeof(unsigned) * (size_t)nb;
+  char* ctr = nullptr; QRec* q[2] = {nullptr, nullptr};
+  STREAMI_TRY(cudaMallocAsync((void**)&ctr, ctr_bytes, st));
+  cudaError_t e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
+  if (e == cudaSuccess) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
+  auto cleanup = [&]() { cudaFreeAsync(ctr, st); if (q[0]) cudaFreeAsync(q[0], st); if (q[1]) cudaFreeAsync(q[1], st); };
+  if (e != cudaSuccess) { if (e != cudaSuccess && !q[0]) q[0] = nullptr; cleanup(); return check(e); }
+  unsigned long long* d_next = (unsigned long long*)ctr;
+  unsigned long long* d_logc = out_log_count ? out_log_count : (unsigned long long*)(ctr + 8);
+  unsigned* d_qcount = (unsigned*)(ctr + 16);
+  unsigned* d_row0 = (unsigned*)(ctr + 24);
+  e = cudaMemsetAsync(ctr, 0, ctr_bytes, st);
+  if (e != cudaSuccess) { cleanup(); return check(e); }
+
+  TraceArgs a{};
+  a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
+  a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = nb;
+  a.seeds = seeds; a.perm = nullptr; a.next = d_next;
+  fill_integrator(a, params);
+  a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  a.qout_count = d_qcount;
+  a.log = out_handoff_log; a.log_cap = log_capacity; a.log_count = d_logc;
+
+  bool truncated = false;
+  unsigned round = 0;
+  unsigned long long nwork = n;
+  std::vector<unsigned> h_buf(1 + nb);
+  for (;;) {
+    a.round = (int)round; a.nwork = nwork;
+    a.qin = q[round & 1]; a.qout = q[(round + 1) & 1];
+    a.rc_this = nullptr; a.rc_next = nullptr;
+    if (round == 0) {
+      a.rc_this = out_round_counts ? out_round_counts : d_row0;
+      if (out_round_counts) e = cudaMemsetAsync(out_round_counts, 0, sizeof(unsigned) * nb, st);
+    }
+    if (out_round_counts && round + 1 < max_rounds) {
+      a.rc_next = out_round_counts + (size_t)(round + 1) * nb;
+      if (e == cudaSuccess) e = cudaMemsetAsync(a.rc_next, 0, sizeof(unsigned) * nb, st);
+    }
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_next, 0, sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_qcount, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) break;
+    int grid = 0;
+    rc = trace_grid(k, nwork, &grid);
+    if (rc) { cleanup(); return rc; }
+    k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+    launch_counter()++;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) break;
+    // the paper's fwdResult.numActiveAcrossAllRanks: read the live count
+    e = cudaMemcpyAsync(h_buf.data(), d_qcount, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && round == 0)
+      e = cudaMemcpyAsync(h_buf.data() + 1, a.rc_this, sizeof(unsigned) * nb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) break;
+    if (round == 0) {
+      unsigned long long inside = 0;
+      for (int b = 0; b < nb; ++b) inside += h_buf[1 + b];
+      if (inside == 0) break;                                  // nothing was ever queued
+    }
+    round++;
+    if (h_buf[0] == 0) break;
+    if (out_round_counts && round >= max_rounds) truncated = true;
+    nwork = h_buf[0];
+  }
+  if (e == cudaSuccess && out_handoff_log) {
+    unsigned long long h_logc = 0;
+    e = cudaMemcpyAsync(&h_logc, d_logc, sizeof(h_logc), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (h_logc > log_capacity) truncated = true;
+  }
+  cleanup();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return check(e);
+  if (out_nrounds) *out_nrounds = round;
+  return truncated ? STREAMI_E_TRUNCATED : STREAMI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,192 @@
+// csrc/api_trace.cu -- streami_trace_streamlines (+ host-buffer variant): argument checks,
+// scratch from the stream-ordered allocator, optional Morton presort, one persistent launch.
+// This is Tracer::trace() in Streamlines mode without the per-step host loop.
+#include <cmath>
+
+#include "internal.h"
+#include "presort.cuh"
+#include "trace_kernel.cuh"
+
+namespace streami {
+
+typedef void (*TraceKernel)(const TraceArgs);
+
+template <int L>
+static TraceKernel pick_l(int integ, bool unsteady, bool brick, bool cache) {
+  if (brick) return cache ? trace_kernel<L, 0, false, true, true> : trace_kernel<L, 0, false, true, false>;
+  if (unsteady) return integ ? trace_kernel<L, 1, true, false, false> : trace_kernel<L, 0, true, false, false>;
+  if (integ) return cache ? trace_kernel<L, 1, false, false, true> : trace_kernel<L, 1, false, false, false>;
+  return cache ? trace_kernel<L, 0, false, false, true> : trace_kernel<L, 0, false, false, false>;
+}
+
+TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache) {
+  switch (layout) {
+    case LAYOUT_PACKED3: return pick_l<LAYOUT_PACKED3>(integ, unsteady, brick, cache);
+    case LAYOUT_FLOAT4: return pick_l<LAYOUT_FLOAT4>(integ, unsteady, brick, cache);
+    default: return pick_l<LAYOUT_XPAIR>(integ, unsteady, brick, cache);
+  }
+}
+
+// Persistent grid: as many blocks as are resident at once (a multiple of the SM count).
+int trace_grid(TraceKernel k, unsigned long long nwork, int* grid) {
+  int per_sm = 0;
+  STREAMI_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, TRACE_BLOCK, 0));
+  int sms = num_sms();
+  if (per_sm < 1 || sms < 1) return STREAMI_E_CUDA;
+  unsigned long long want = (nwork + TRACE_BLOCK - 1) / TRACE_BLOCK;
+  unsigned long long full = (unsigned long long)per_sm * sms;
+  *grid = (int)std::max(1ull, std::min(want, full));
+  return STREAMI_OK;
+}
+
+int check_params(const streami_params* p, bool need_capacity) {
+  if (!p) return STREAMI_E_INVALID;
+  if (p->integrator != 0 && p->integrator != 1) return STREAMI_E_INVALID;
+  if (!(std::isfinite(p->h) && p->h > 0.0f)) return STREAMI_E_INVALID;
+  if (need_capacity && (p->capacity == 0 || p->stride == 0)) return STREAMI_E_INVALID;
+  if (!(p->vmin >= 0.0f) || !std::isfinite(p->t0)) return STREAMI_E_INVALID;
+  if (p->time_mode != 0 && p->time_mode != 1) return STREAMI_E_INVALID;
+  if (p->integrator == 1) {
+    if (!(p->h_min >= 0.0f) || !(p->h_max >= p->h_min) || !(p->atol >= 0.0f) || !(p->rtol >= 0.0f))
+      return STREAMI_E_INVALID;
+    if (!(p->atol > 0.0f || p->rtol > 0.0f)) return STREAMI_E_INVALID;
+  }
+  return STREAMI_OK;
+}
+
+void fill_integrator(TraceArgs& a, const streami_params* p) {
+  a.h = p->h; a.h2 = 0.5f * p->h; a.h6 = p->h / 6.0f;        // A4: computed once, fp32
+  a.hmin = p->h_min; a.hmax = p->h_max; a.atol = p->atol; a.rtol = p->rtol;
+  a.vmin2 = p->vmin * p->vmin; a.t0 = p->t0; a.max_steps = p->max_steps;
+  a.cap = p->capacity; a.stride = p->stride;
+  a.steps = p->out_steps; a.status = p->out_status; a.fin = p->out_final; a.totals = p->out_totals;
+}
+
+// Morton presort (a12): fills perm[n]; scratch is freed on the stream.
+int presort_seeds(const streami_field_s* f, const float* seeds, size_t n, unsigned* perm,
+                  cudaStream_t st) {
+  int maxdim = std::max(f->dims[0], std::max(f->dims[1], f->dims[2]));
+  int shift = 2;                                   // 4^3-cell blocks, at most 128 blocks per axis
+  while (((maxdim - 1) >> shift) >= 128) shift++;
+  unsigned bits = 0;
+  while ((1u << bits) <= (unsigned)((maxdim - 1) >> shift)) bits++;
+  unsigned nbins = 1u << (3 * bits);
+  unsigned* hist = nullptr; unsigned* keys = nullptr;
+  STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * nbins, st));
+  cudaError_t e = cudaMallocAsync((void**)&keys, sizeof(unsigned) * n, st);
+  if (e != cudaSuccess) { cudaFreeAsync(hist, st); return check(e); }
+  int rc = STREAMI_OK;
+  unsigned blocks = (unsigned)((n + 255) / 256);
+  e = cudaMemsetAsync(hist, 0, sizeof(unsigned) * nbins, st);
+  if (e == cudaSuccess) {
+    presort_hist_kernel<<<blocks, 256, 0, st>>>(f->g, shift, seeds, n, hist, keys);
+    presort_scan_kernel<<<1, 1024, 0, st>>>(hist, nbins);
+    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, perm);
+    launch_counter() += 3;
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess) rc = check(e);
+  cudaFreeAsync(hist, st); cudaFreeAsync(keys, st);
+  return rc;
+}
+
+}  // namespace streami
+
+using namespace streami;
+
+extern "C" {
+
+int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
+                              const streami_params* params, float* out_vertices,
+                              unsigned* out_counts, void* cuda_stream) {
+  if (!f || f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, true);
+  if (rc) return rc;
+  if (n > 0xffffffffull) return STREAMI_E_INVALID;           // particle ids are u32
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
+  if (n == 0) return STREAMI_OK;
+
+  const bool unsteady = f->g.nslices > 1;
+  const bool cache = options().cell_cache && !unsteady;
+  TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache);
+  int grid = 0;
+  rc = trace_grid(k, n, &grid);
+  if (rc) return rc;
+
+  unsigned long long* next = nullptr;
+  STREAMI_TRY(cudaMallocAsync((void**)&next, sizeof(unsigned long long), st));
+  unsigned* perm = nullptr;
+  auto cleanup = [&]() { cudaFreeAsync(next, st); if (perm) cudaFreeAsync(perm, st); };
+  cudaError_t e = cudaMemsetAsync(next, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess) { cleanup(); return check(e); }
+  if (options().presort && n >= 65536) {
+    e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+    if (e != cudaSuccess) { perm = nullptr; cleanup(); return check(e); }
+    rc = presort_seeds(f, seeds, n, perm, st);
+    if (rc) { cleanup(); return rc; }
+  }
+
+  TraceArgs a{};
+  a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
+  a.bricks = nullptr; a.nbricks = 0;
+  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.next = next; a.round = 0;
+  fill_integrator(a, params);
+  a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+  launch_counter()++;
+  e = cudaGetLastError();
+  cleanup();
+  return check(e);
+}
+
+int streami_trace_streamlines_host(streami_field f, const float* seeds, size_t n,
+                                   const streami_params* params, float* out_vertices,
+                                   unsigned* out_counts, void* cuda_stream) {
+  if (!f || f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, true);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n == 0) {
+    if (params->out_totals) for (int i = 0; i < 4; ++i) params->out_totals[i] = 0;
+    return STREAMI_OK;
+  }
+  const size_t nv = out_vertices ? 3 * n * (size_t)params->capacity : 0;
+  float *d_seeds = nullptr, *d_verts = nullptr, *d_final = nullptr;
+  unsigned *d_counts = nullptr, *d_steps = nullptr, *d_status = nullptr;
+  unsigned long long* d_totals = nullptr;
+  void* allocs[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  int na = 0;
+  auto alloc = [&](void** p, size_t bytes) {
+    cudaError_t e = cudaMallocAsync(p, bytes, st);
+    if (e == cudaSuccess) allocs[na++] = *p;
+    return e;
+  };
+  auto cleanup = [&]() { for (int i = 0; i < na; ++i) cudaFreeAsync(allocs[i], st); };
+  cudaError_t e = alloc((void**)&d_seeds, 3 * n * sizeof(float));
+  if (e == cudaSuccess) e = alloc((void**)&d_counts, n * sizeof(unsigned));
+  if (e == cudaSuccess && nv) e = alloc((void**)&d_verts, nv * sizeof(float));
+  if (e == cudaSuccess && params->out_steps) e = alloc((void**)&d_steps, n * sizeof(unsigned));
+  if (e == cudaSuccess && params->out_status) e = alloc((void**)&d_status, n * sizeof(unsigned));
+  if (e == cudaSuccess && params->out_final) e = alloc((void**)&d_final, 3 * n * sizeof(float));
+  if (e == cudaSuccess && params->out_totals) e = alloc((void**)&d_totals, 4 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_seeds, seeds, 3 * n * sizeof(float), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) { cleanup(); return check(e); }
+  streami_params dp = *params;
+  dp.out_steps = d_steps; dp.out_status = d_status; dp.out_final = d_final; dp.out_totals = d_totals;
+  rc = streami_trace_streamlines(f, d_seeds, n, &dp, d_verts, d_counts, cuda_stream);
+  if (rc) { cleanup(); return rc; }
+  // Slots beyond out_counts are "left untouched" on the device copy; the host array receives
+  // the device array as is (its untouched slots hold whatever the allocator returned).
+  e = cudaMemcpyAsync(out_counts, d_counts, n * sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && nv) e = cudaMemcpyAsync(out_vertices, d_verts, nv * sizeof(float), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d_steps) e = cudaMemcpyAsync(params->out_steps, d_steps, n * sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d_status) e = cudaMemcpyAsync(params->out_status, d_status, n * sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d_final) e = cudaMemcpyAsync(params->out_final, d_final, 3 * n * sizeof(float), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d_totals) e = cudaMemcpyAsync(params->out_totals, d_totals, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+  cleanup();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  return check(e);
+}
+
+}  // extern "C"

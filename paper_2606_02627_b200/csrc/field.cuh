@@ -1,0 +1,192 @@
+// csrc/field.cuh -- device-side field views and the field-sampling layer (a2, a3, a4 of
+// SURVEY.md 8(a)): cell location, trilinear gather + interpolation, linear interpolation in time.
+//
+// The paper's sample() is "computing offsets into [a CUDA global memory] array" of float3 voxels
+// (PAPER.md:63, 155); the filter itself is fixed by BASELINE.json (trilinear) and by the fp32
+// formula sheet A1-A3.  This file is written from that sheet; it shares
+// nothing with oracle/.  The translation unit is compiled with -fmad=false: every fused
+// multiply-add below is an explicit __fmaf_rn, everything else rounds once per operation.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace streami {
+
+enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3 };
+enum : unsigned { ST_ALIVE = 0, ST_OUT = 1, ST_MAXSTEPS = 2, ST_STAGNANT = 3, ST_HALO = 4 };
+
+// Global geometry (A1), uniform over the launch.
+struct Geom {
+  float ox, oy, oz;        // origin
+  float rx, ry, rz;        // 1/spacing, computed once on the host in fp32
+  float topx, topy, topz;  // (float)(N-1)
+  int nslices;
+  float q, top_s;          // 1/slice_dt, (float)(nslices-1)
+  int time_mode;           // 0 linear, 1 hold floor slice
+};
+
+// One stored array: the whole grid (lo = 0, hi = N-1) or one brick's stored box (A9).
+struct Store {
+  const void* data;        // layout-specific records, x fastest
+  int lox, loy, loz;       // stored box, global vertex indices, inclusive
+  int hix, hiy, hiz;
+  int topflagx, topflagy, topflagz;  // 1 where hi == N-1 (g == hi is then served too)
+  unsigned nx, nxy;        // row and plane strides in vertices
+  unsigned long long slice_stride;   // vertices per slice
+};
+
+// A brick grid (A9): owner of an in-domain position.
+struct BrickMap {
+  int nbx, nby, nbz;
+  int Bx, By, Bz;
+};
+
+__device__ __forceinline__ float lerp(float a, float b, float w) { return __fmaf_rn(w, b - a, a); }
+
+// ---- loads of the 8 cell vertices as 4 rows of {V[x].xyz, V[x+1].xyz} ----------------------
+// V[row*6 + dx*3 + c], row = dz*2 + dy.
+template <int LAYOUT> struct CellLoad;
+
+template <> struct CellLoad<LAYOUT_PACKED3> {
+  static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
+    const float* p = reinterpret_cast<const float*>(data) + 3ull * v;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) o[k] = __ldg(p + k);
+  }
+};
+template <> struct CellLoad<LAYOUT_FLOAT4> {
+  static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
+    const float4* p = reinterpret_cast<const float4*>(data) + v;
+    float4 a = __ldg(p), b = __ldg(p + 1);
+    o[0] = a.x; o[1] = a.y; o[2] = a.z; o[3] = b.x; o[4] = b.y; o[5] = b.z;
+  }
+};
+template <> struct CellLoad<LAYOUT_XPAIR> {
+  // one aligned 32-byte record per row: a single 256-bit read-only load (LDG.E.256 on sm_100a)
+  static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
+    const char* p = reinterpret_cast<const char*>(data) + 32ull * v;
+    float p6, p7;
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]),
+                   "=f"(p6), "=f"(p7)
+                 : "l"(p));
+    (void)p6; (void)p7;
+  }
+};
+
+template <int LAYOUT>
+__device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, float* V) {
+  CellLoad<LAYOUT>::row(s.data, v, V);
+  CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
+  CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
+  CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+}
+
+// A2.5: x first, then y, then z; 7 lerps per component.
+__device__ __forceinline__ void interp_cell(const float* V, float fx, float fy, float fz,
+                                            float& vx, float& vy, float& vz) {
+  float r[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    float c00 = lerp(V[0 + c], V[3 + c], fx);
+    float c01 = lerp(V[6 + c], V[9 + c], fx);
+    float c10 = lerp(V[12 + c], V[15 + c], fx);
+    float c11 = lerp(V[18 + c], V[21 + c], fx);
+    float c0 = lerp(c00, c01, fy);
+    float c1 = lerp(c10, c11, fy);
+    r[c] = lerp(c0, c1, fz);
+  }
+  vx = r[0]; vy = r[1]; vz = r[2];
+}
+
+// Register-resident copy of the current cell (build's choice: a sample that stays in the cell of
+// the previous one costs no loads; the arithmetic, hence the result, is unchanged).
+struct CellCache {
+  unsigned long long key;
+  float V[24];
+  __device__ __forceinline__ void invalidate() { key = ~0ull; }
+};
+
+// A2.1 + A2.2: index-space position and the closed-box test (NaN -> false).
+__device__ __forceinline__ bool to_index(const Geom& g, float px, float py, float pz, float& gx,
+                                         float& gy, float& gz) {
+  gx = (px - g.ox) * g.rx; gy = (py - g.oy) * g.ry; gz = (pz - g.oz) * g.rz;
+  return (gx >= 0.0f && gx <= g.topx) && (gy >= 0.0f && gy <= g.topy) &&
+         (gz >= 0.0f && gz <= g.topz);
+}
+
+// Cell location inside one store.  Returns false (HALO_MISS) if the store cannot serve g.
+// g >= 0 here, so float->int truncation equals floor.
+template <bool BRICK>
+__device__ __forceinline__ bool locate(const Store& s, float gx, float gy, float gz,
+                                       unsigned long long& v, float& fx, float& fy, float& fz) {
+  if (BRICK) {
+    bool in = (gx >= (float)s.lox) && (gx < (float)s.hix || (s.topflagx && gx <= (float)s.hix)) &&
+              (gy >= (float)s.loy) && (gy < (float)s.hiy || (s.topflagy && gy <= (float)s.hiy)) &&
+              (gz >= (float)s.loz) && (gz < (float)s.hiz || (s.topflagz && gz <= (float)s.hiz));
+    if (!in) return false;
+  }
+  int ix = min(__float2int_rz(gx), s.hix - 1);
+  int iy = min(__float2int_rz(gy), s.hiy - 1);
+  int iz = min(__float2int_rz(gz), s.hiz - 1);
+  fx = gx - (float)ix; fy = gy - (float)iy; fz = gz - (float)iz;
+  v = (unsigned long long)(unsigned)(iz - s.loz) * s.nxy + (unsigned)(iy - s.loy) * s.nx +
+      (unsigned)(ix - s.lox);
+  return true;
+}
+
+// A3: slice index and weight.  Returns the slice j to read first; two = read j+1 as well.
+__device__ __forceinline__ int time_slice(const Geom& g, float t, float& a, bool& two) {
+  float s = t * g.q;
+  s = fminf(fmaxf(s, 0.0f), g.top_s);
+  if (g.time_mode == 1) { two = false; a = 0.0f; return min(__float2int_rz(s), g.nslices - 1); }
+  int j = min(__float2int_rz(s), g.nslices - 2);
+  a = s - (float)j; two = true;
+  return j;
+}
+
+// Full sample S(p, t) (A2/A3, brick form A9).  Returns 0 ok, ST_OUT or ST_HALO.
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE>
+__device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCache& cc, float px,
+                                           float py, float pz, float t, float& vx, float& vy,
+                                           float& vz) {
+  float gx, gy, gz;
+  if (!to_index(g, px, py, pz, gx, gy, gz)) return ST_OUT;
+  unsigned long long v; float fx, fy, fz;
+  if (!locate<BRICK>(s, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
+  if (UNSTEADY) {
+    float a; bool two;
+    int j = time_slice(g, t, a, two);
+    unsigned long long vj = v + (unsigned long long)j * s.slice_stride;
+    float V[24];
+    load_cell<LAYOUT>(s, vj, V);
+    float ux, uy, uz;
+    interp_cell(V, fx, fy, fz, ux, uy, uz);
+    if (two) {
+      load_cell<LAYOUT>(s, vj + s.slice_stride, V);
+      float wx, wy, wz;
+      interp_cell(V, fx, fy, fz, wx, wy, wz);
+      vx = lerp(ux, wx, a); vy = lerp(uy, wy, a); vz = lerp(uz, wz, a);   // space first, time last
+    } else { vx = ux; vy = uy; vz = uz; }
+  } else if (CACHE) {
+    if (v != cc.key) { load_cell<LAYOUT>(s, v, cc.V); cc.key = v; }
+    interp_cell(cc.V, fx, fy, fz, vx, vy, vz);
+  } else {
+    float V[24];
+    load_cell<LAYOUT>(s, v, V);
+    interp_cell(V, fx, fy, fz, vx, vy, vz);
+  }
+  return 0;
+}
+
+// A9: owner brick of an in-domain position (destinationID).
+__device__ __forceinline__ int owner_of(const Geom& g, const BrickMap& m, float px, float py,
+                                        float pz) {
+  float gx = (px - g.ox) * g.rx, gy = (py - g.oy) * g.ry, gz = (pz - g.oz) * g.rz;
+  int bx = min(__float2int_rd(gx) / m.Bx, m.nbx - 1);
+  int by = min(__float2int_rd(gy) / m.By, m.nby - 1);
+  int bz = min(__float2int_rd(gz) / m.Bz, m.nbz - 1);
+  return (bz * m.nby + by) * m.nbx + bx;
+}
+
+}  // namespace streami

@@ -1,0 +1,50 @@
+// csrc/internal.h -- host-side state shared by the API translation units.
+#pragma once
+#include <atomic>
+#include <string>
+#include <vector>
+
+#include "../../include/streami.h"
+#include "field.cuh"
+
+struct streami_field_s {
+  streami::Geom g;
+  int dims[3];                       // global vertex counts
+  int layout;
+  bool bricked;
+  streami::Store store;              // monolithic
+  std::vector<streami::Store> bricks;  // host copies
+  streami::Store* d_bricks;          // device table
+  streami::BrickMap bm;
+  std::vector<void*> owned;          // device allocations owned by the handle
+  size_t owned_bytes;
+};
+
+namespace streami {
+
+struct Options { int cell_cache; int presort; int streak_window; };
+Options& options();
+std::atomic<unsigned long long>& launch_counter();
+void set_cuda_error(cudaError_t e);
+
+inline int check(cudaError_t e) {
+  if (e == cudaSuccess) return STREAMI_OK;
+  set_cuda_error(e);
+  return e == cudaErrorMemoryAllocation ? STREAMI_E_NOMEM : STREAMI_E_CUDA;
+}
+
+#define STREAMI_TRY(expr)                         \
+  do {                                            \
+    int rc__ = streami::check(expr);              \
+    if (rc__ != STREAMI_OK) return rc__;          \
+  } while (0)
+
+#define STREAMI_LAUNCHED()                        \
+  do {                                            \
+    streami::launch_counter()++;                  \
+    STREAMI_TRY(cudaGetLastError());              \
+  } while (0)
+
+int num_sms();
+
+}  // namespace streami

@@ -1,0 +1,128 @@
+// csrc/misc_kernels.cuh -- layout repack, the stand-alone sampler entry and the streakline kernel.
+#pragma once
+#include "trace.cuh"
+
+namespace streami {
+
+// ---- field repack: caller's packed float3 -> library-owned layout (D6 of SURVEY.md) ---------
+// One thread per vertex; reads are contiguous 12-byte triples, writes are 16/32-byte records.
+static __global__ void repack_float4_kernel(const float* __restrict__ src, float4* __restrict__ dst,
+                                     unsigned long long nvert) {
+  unsigned long long v = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; v < nvert; v += step)
+    dst[v] = make_float4(src[3 * v], src[3 * v + 1], src[3 * v + 2], 0.0f);
+}
+
+// XPAIR record v = {V[v].xyz, V[v+1].xyz, 0, 0}; the last vertex of a row repeats itself (its
+// upper half is never used: i_x <= nx-2).
+static __global__ void repack_xpair_kernel(const float* __restrict__ src, float4* __restrict__ dst,
+                                    unsigned long long nvert, unsigned nx) {
+  unsigned long long v = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; v < nvert; v += step) {
+    unsigned long long w = ((v % nx) == nx - 1) ? v : v + 1;
+    float a0 = src[3 * v], a1 = src[3 * v + 1], a2 = src[3 * v + 2];
+    float b0 = src[3 * w], b1 = src[3 * w + 1], b2 = src[3 * w + 2];
+    dst[2 * v] = make_float4(a0, a1, a2, b0);
+    dst[2 * v + 1] = make_float4(b1, b2, 0.0f, 0.0f);
+  }
+}
+
+// ---- a2-a4 alone ----------------------------------------------------------------------------
+template <int LAYOUT, bool UNSTEADY>
+__global__ void sample_kernel(Geom g, Store s, const float* __restrict__ pts, unsigned long long n,
+                              float t, float* __restrict__ out_v, unsigned* __restrict__ out_rc) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  CellCache cc; cc.invalidate();
+  float vx = 0.f, vy = 0.f, vz = 0.f;
+  unsigned rc = sample<LAYOUT, UNSTEADY, false, false>(g, s, cc, pts[3 * i], pts[3 * i + 1],
+                                                       pts[3 * i + 2], t, vx, vy, vz);
+  if (rc) { vx = 0.f; vy = 0.f; vz = 0.f; }
+  out_v[3 * i] = vx; out_v[3 * i + 1] = vy; out_v[3 * i + 2] = vz;
+  out_rc[i] = rc;
+}
+
+// ---- a11 + a10 for streaklines (A7; Listing 2) -----------------------------
+// One launch covers the global steps [s0, s1).  Particle id = j*m + i (release j, point i) is
+// born at point i at global step j.  Its state between launches is its output slot (the last
+// inside position is what the slot must hold anyway) plus one status byte.
+struct StreakArgs {
+  Geom g; Store s;
+  const float* points; unsigned long long m; unsigned nsteps, s0, s1;
+  float h, h2, h6, vmin2, t0;
+  float* verts;                  // [3][nsteps][m]
+  unsigned char* state;          // [nsteps*m] status, 0 = alive
+  unsigned* steps;               // optional [nsteps*m]
+  unsigned long long* totals;
+};
+
+template <int LAYOUT, bool UNSTEADY>
+__global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
+  __shared__ unsigned long long s_tot[3];
+  if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
+  __syncthreads();
+  const unsigned long long total = a.m * (unsigned long long)min(a.s1, a.nsteps);
+  unsigned long long id = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id < total) {
+    const unsigned j = (unsigned)(id / a.m);
+    const unsigned long long i = id - (unsigned long long)j * a.m;
+    const unsigned long long plane = a.m * (unsigned long long)a.nsteps;
+    float px, py, pz; unsigned st = ST_ALIVE; unsigned s = a.s0;
+    bool run = true;
+    if (j >= a.s0) {                                             // born in this window
+      px = a.points[3 * i]; py = a.points[3 * i + 1]; pz = a.points[3 * i + 2];
+      s = j;
+      float gx, gy, gz;
+      if (!to_index(a.g, px, py, pz, gx, gy, gz)) { st = ST_OUT; run = false; }
+    } else {
+      st = a.state[id];
+      if (st != ST_ALIVE) run = false;
+      else { px = a.verts[id]; py = a.verts[plane + id]; pz = a.verts[2 * plane + id]; }
+    }
+    if (run) {
+      TraceArgs ta;                                              // only the fields rk4_step reads
+      ta.g = a.g; ta.h = a.h; ta.h2 = a.h2; ta.h6 = a.h6; ta.vmin2 = a.vmin2;
+      ta.max_steps = 0xffffffffu; ta.verts = nullptr; ta.cap = 0; ta.stride = 0xffffffffu;
+      Lane L; L.px = px; L.py = py; L.pz = pz; L.id = 0; L.slot = 0; L.rec_cd = 0xffffffffu;
+      CellCache cc; cc.invalidate();
+      unsigned n_samples = 0, n_attempts = 0;
+      for (; s < a.s1; ++s) {
+        L.n = s;                                                 // t_s = t0 + (float)s*h, shared by all
+        ta.t0 = a.t0;
+        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false>(ta, a.s, cc, L, n_samples, n_attempts);
+        if (rc) { st = rc; break; }
+      }
+      if (st == ST_ALIVE && a.s1 >= a.nsteps) st = ST_MAXSTEPS;  // alive at the end
+      px = L.px; py = L.py; pz = L.pz;
+      atomicAdd(&s_tot[0], (unsigned long long)n_attempts);
+      atomicAdd(&s_tot[1], (unsigned long long)(s - max(j, a.s0)));
+      atomicAdd(&s_tot[2], (unsigned long long)n_samples);
+    }
+    if (run || j >= a.s0) {
+      a.verts[id] = px; a.verts[plane + id] = py; a.verts[2 * plane + id] = pz;
+      a.state[id] = (unsigned char)st;
+      if (a.steps && st != ST_ALIVE) a.steps[id] = s - j;
+    }
+  }
+  __syncthreads();
+  if (a.totals && threadIdx.x < 3 && s_tot[threadIdx.x]) atomicAdd(a.totals + threadIdx.x, s_tot[threadIdx.x]);
+}
+
+// out_counts[i] = number of particles of point i alive at the end; copy status to u32.
+static __global__ void streak_finalize_kernel(const unsigned char* __restrict__ state, unsigned long long m,
+                                       unsigned nsteps, unsigned* __restrict__ counts,
+                                       unsigned* __restrict__ status) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m) return;
+  unsigned c = 0;
+  for (unsigned j = 0; j < nsteps; ++j) {
+    unsigned st = state[(unsigned long long)j * m + i];
+    c += (st == ST_MAXSTEPS);
+    if (status) status[(unsigned long long)j * m + i] = st;
+  }
+  counts[i] = c;
+}
+
+}  // namespace streami

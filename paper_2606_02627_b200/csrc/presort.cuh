@@ -1,0 +1,67 @@
+// csrc/presort.cuh -- a12 of SURVEY.md 8(a): order the seeds by the Morton code of their coarse
+// cell block before tracing (the build's choice; not in the paper).  It is a permutation only:
+// every output is indexed by particle id, so results do not change.  Purpose: lanes that run at
+// the same time work in the same region of the field, so the gathers of concurrently resident
+// warps hit the same L2 lines / DRAM pages / TLB entries.  Counting sort: histogram over bins,
+// exclusive scan, scatter.  Order inside a bin is unspecified.
+#pragma once
+#include "field.cuh"
+
+namespace streami {
+
+__device__ __forceinline__ unsigned spread3(unsigned x) {   // 10 bits -> every third bit
+  x &= 0x3ffu;
+  x = (x | (x << 16)) & 0x030000ffu;
+  x = (x | (x << 8)) & 0x0300f00fu;
+  x = (x | (x << 4)) & 0x030c30c3u;
+  x = (x | (x << 2)) & 0x09249249u;
+  return x;
+}
+
+__device__ __forceinline__ unsigned seed_bin(const Geom& g, int shift, const float* seeds,
+                                             unsigned long long i) {
+  float gx, gy, gz;
+  if (!to_index(g, seeds[3 * i], seeds[3 * i + 1], seeds[3 * i + 2], gx, gy, gz)) return 0u;
+  unsigned bx = (unsigned)__float2int_rz(gx) >> shift, by = (unsigned)__float2int_rz(gy) >> shift,
+           bz = (unsigned)__float2int_rz(gz) >> shift;
+  return spread3(bx) | (spread3(by) << 1) | (spread3(bz) << 2);
+}
+
+static __global__ void presort_hist_kernel(Geom g, int shift, const float* __restrict__ seeds,
+                                    unsigned long long n, unsigned* __restrict__ hist,
+                                    unsigned* __restrict__ keys) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  unsigned k = seed_bin(g, shift, seeds, i);
+  keys[i] = k;
+  atomicAdd(hist + k, 1u);
+}
+
+// Exclusive scan of `hist` in place, one block of 1024 threads, nbins arbitrary.
+static __global__ void presort_scan_kernel(unsigned* __restrict__ hist, unsigned nbins) {
+  __shared__ unsigned s_part[1024];
+  const unsigned per = (nbins + 1023u) / 1024u;
+  const unsigned lo = threadIdx.x * per, hi = min(lo + per, nbins);
+  unsigned sum = 0;
+  for (unsigned k = lo; k < hi; ++k) sum += hist[k];
+  s_part[threadIdx.x] = sum;
+  __syncthreads();
+  for (unsigned d = 1; d < 1024; d <<= 1) {                 // Hillis-Steele inclusive scan
+    unsigned v = threadIdx.x >= d ? s_part[threadIdx.x - d] : 0u;
+    __syncthreads();
+    s_part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  unsigned run = s_part[threadIdx.x] - sum;
+  for (unsigned k = lo; k < hi; ++k) { unsigned c = hist[k]; hist[k] = run; run += c; }
+}
+
+static __global__ void presort_scatter_kernel(const unsigned* __restrict__ keys, unsigned long long n,
+                                       unsigned* __restrict__ offsets, unsigned* __restrict__ perm) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  unsigned pos = atomicAdd(offsets + keys[i], 1u);
+  perm[pos] = (unsigned)i;
+}
+
+}  // namespace streami

@@ -1,0 +1,109 @@
+// csrc/trace.cuh -- the advection kernel (a1, a5-a10 of SURVEY.md 8(a)).
+//
+// The paper's update() kernel (Listing 1) advances every particle by ONE RK4
+// step per launch and hands all of them to an all-to-all after each step.
+// This kernel is a B200 re-design of the same computation: a persistent grid sized to the
+// machine, one lane per particle, the particle kept in registers from seed to termination, and
+// a lane that loses its particle (terminated, or handed to another brick) immediately refills
+// from a global work counter (warp ballot + one atomic per warp).  No compaction pass and no
+// state round trip through memory is needed, and lanes stay busy although lifetimes differ by
+// orders of magnitude.  Results follow the formula sheet A4-A9 operation by operation.
+#pragma once
+#include "field.cuh"
+
+namespace streami {
+
+// hand-off record: what a particle carries to another brick (position + unique id, PAPER.md:69;
+// plus its step count).  32 bytes, read and written as two 16-byte accesses.
+struct __align__(16) QRec {
+  float px, py, pz; unsigned id;
+  unsigned n; unsigned brick; unsigned pad0, pad1;
+};
+
+struct TraceArgs {
+  Geom g;
+  Store s;                         // monolithic store
+  const Store* bricks; BrickMap bm; int nbricks;   // brick mode
+  // work
+  const float* seeds;              // [n][3]
+  const unsigned* perm;            // optional processing order of seeds (presort), or NULL
+  const QRec* qin;                 // brick rounds >= 1
+  unsigned long long nwork;
+  unsigned long long* next;        // global work counter
+  int round;
+  // integrator (host-computed fp32 constants, A4/A8)
+  float h, h2, h6, hmin, hmax, atol, rtol, vmin2, t0;
+  unsigned max_steps;
+  // outputs (A6)
+  float* verts; unsigned long long n; unsigned cap, stride;
+  unsigned* counts; unsigned* steps; unsigned* status; float* fin;
+  unsigned long long* totals;      // [4]
+  // brick outputs
+  QRec* qout; unsigned* qout_count;
+  unsigned* rc_this;               // round_counts row of this round (round 0 only), or NULL
+  unsigned* rc_next;               // round_counts row of the next round, or NULL
+  unsigned long long* log; unsigned long long log_cap; unsigned long long* log_count;
+};
+
+constexpr unsigned RC_HANDOFF = 100;
+
+struct Lane {
+  float px, py, pz;
+  unsigned id, n;
+  unsigned slot, rec_cd;           // next vertex slot, steps until the next recorded vertex
+  // DP5(4) only
+  float t, h, k1x, k1y, k1z; bool rejected;
+};
+
+__device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
+  if (--L.rec_cd == 0) {
+    L.rec_cd = a.stride;
+    if (L.slot < a.cap) {
+      if (a.verts) {
+        unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
+        unsigned long long plane = a.n * a.cap;
+        a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
+      }
+      L.slot++;
+    }
+  }
+}
+
+// ---- A4 + A5 steps 2-6: one RK4 step.  Returns 0 to continue, else the final status. -------
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE>
+__device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CellCache& cc,
+                                             Lane& L, unsigned& n_samples, unsigned& n_attempts) {
+  if (L.n == a.max_steps) return ST_MAXSTEPS;                                   // A5.2
+  float tn = 0.0f;
+  if (UNSTEADY) tn = a.t0 + (float)L.n * a.h;                                   // A4, not accumulated
+  float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z;
+  unsigned rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, L.px, L.py, L.pz, tn, k1x, k1y, k1z);
+  n_samples++;
+  if (rc) return rc;
+  float m = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));                // A5.3
+  if (m < a.vmin2) return ST_STAGNANT;
+  n_attempts++;
+  float qx = __fmaf_rn(a.h2, k1x, L.px), qy = __fmaf_rn(a.h2, k1y, L.py), qz = __fmaf_rn(a.h2, k1z, L.pz);
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h2, k2x, k2y, k2z);
+  n_samples++;
+  if (rc) return rc;
+  qx = __fmaf_rn(a.h2, k2x, L.px); qy = __fmaf_rn(a.h2, k2y, L.py); qz = __fmaf_rn(a.h2, k2z, L.pz);
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h2, k3x, k3y, k3z);
+  n_samples++;
+  if (rc) return rc;
+  qx = __fmaf_rn(a.h, k3x, L.px); qy = __fmaf_rn(a.h, k3y, L.py); qz = __fmaf_rn(a.h, k3z, L.pz);
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h, k4x, k4y, k4z);
+  n_samples++;
+  if (rc) return rc;
+  float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
+  float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
+  float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
+  float nx = __fmaf_rn(a.h6, sx, L.px), ny = __fmaf_rn(a.h6, sy, L.py), nz = __fmaf_rn(a.h6, sz, L.pz);
+  float gx, gy, gz;
+  if (!to_index(a.g, nx, ny, nz, gx, gy, gz)) return ST_OUT;                    // A5.5: not recorded
+  L.px = nx; L.py = ny; L.pz = nz; L.n++;                                       // A5.6
+  record_vertex(a, L);
+  return 0;
+}
+
+}  // namespace streami

@@ -1,0 +1,141 @@
+// csrc/trace_kernel.cuh -- the persistent advection kernel: refill, step, terminate / hand off.
+#pragma once
+#include "dp5.cuh"
+
+namespace streami {
+
+constexpr int TRACE_BLOCK = 256;
+
+__device__ __forceinline__ void finish_particle(const TraceArgs& a, const Lane& L, unsigned st) {
+  if (a.counts) a.counts[L.id] = L.slot;
+  if (a.steps) a.steps[L.id] = L.n;
+  if (a.status) a.status[L.id] = st;
+  if (a.fin) { a.fin[L.id] = L.px; a.fin[a.n + L.id] = L.py; a.fin[2 * a.n + L.id] = L.pz; }
+}
+
+// a9: append a brick leaver to the next round's queue (the device-side stand-in for
+// emitOutgoing + forward): one atomic per warp for the slot range.
+__device__ __forceinline__ void emit_outgoing(const TraceArgs& a, const Lane& L, int dest, bool emit) {
+  unsigned mask = __ballot_sync(__activemask(), emit);
+  if (!emit) return;
+  int lane = threadIdx.x & 31;
+  int leader = __ffs(mask) - 1;
+  unsigned base = 0;
+  if (lane == leader) base = atomicAdd(a.qout_count, (unsigned)__popc(mask));
+  base = __shfl_sync(mask, base, leader);
+  unsigned pos = base + __popc(mask & ((1u << lane) - 1u));
+  QRec r; r.px = L.px; r.py = L.py; r.pz = L.pz; r.id = L.id; r.n = L.n; r.brick = (unsigned)dest;
+  r.pad0 = 0; r.pad1 = 0;
+  a.qout[pos] = r;
+  if (a.rc_next) atomicAdd(a.rc_next + dest, 1u);
+  if (a.log_count) {
+    unsigned long long k = atomicAdd(a.log_count, 1ull);
+    if (a.log && k < a.log_cap)
+      a.log[k] = ((unsigned long long)(a.round + 1) << 48) | ((unsigned long long)dest << 32) | L.id;
+  }
+}
+
+template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE>
+__global__ void __launch_bounds__(TRACE_BLOCK)
+trace_kernel(const TraceArgs a) {
+  __shared__ unsigned long long s_tot[4];
+  if (threadIdx.x < 4) s_tot[threadIdx.x] = 0ull;
+  __syncthreads();
+
+  const int lane = threadIdx.x & 31;
+  const unsigned FULL = 0xffffffffu;
+  Lane L; L.rejected = false;
+  CellCache cc; cc.invalidate();
+  Store st = a.s;                 // brick mode: replaced per particle
+  int my_brick = 0;
+  bool active = false, exhausted = false;
+  unsigned n_samples = 0, n_attempts = 0, n_start = 0;
+
+  for (;;) {
+    // ---- a1: refill idle lanes from the global work counter --------------------------------
+    unsigned need = __ballot_sync(FULL, !active && !exhausted);
+    if (need) {
+      int leader = __ffs(need) - 1;
+      unsigned long long base = 0;
+      if (lane == leader) base = atomicAdd(a.next, (unsigned long long)__popc(need));
+      base = __shfl_sync(FULL, base, leader);
+      if (!active && !exhausted) {
+        unsigned long long w = base + __popc(need & ((1u << lane) - 1u));
+        if (w >= a.nwork) {
+          exhausted = true;
+        } else {
+          n_samples = 0; n_attempts = 0;
+          bool fresh = true;
+          if (BRICK && a.round > 0) {
+            const QRec r = a.qin[w];
+            L.px = r.px; L.py = r.py; L.pz = r.pz; L.id = r.id; L.n = r.n; my_brick = (int)r.brick;
+            L.slot = min(a.cap, L.n / a.stride + 1u);
+            L.rec_cd = a.stride - L.n % a.stride;
+            fresh = false;
+          } else {
+            L.id = a.perm ? a.perm[w] : (unsigned)w;
+            L.px = a.seeds[3ull * L.id]; L.py = a.seeds[3ull * L.id + 1]; L.pz = a.seeds[3ull * L.id + 2];
+            L.n = 0; L.slot = 0; L.rec_cd = 1;
+          }
+          n_start = L.n;
+          active = true;
+          if (fresh) {
+            float gx, gy, gz;
+            if (!to_index(a.g, L.px, L.py, L.pz, gx, gy, gz)) {                 // A5.1
+              finish_particle(a, L, ST_OUT);
+              active = false;
+            } else {
+              record_vertex(a, L);                                              // vertex 0 = seed
+              if (BRICK) {
+                my_brick = owner_of(a.g, a.bm, L.px, L.py, L.pz);
+                if (a.rc_this) atomicAdd(a.rc_this + my_brick, 1u);
+              }
+            }
+          }
+          if (active) {
+            if (BRICK) { st = a.bricks[my_brick]; }
+            cc.invalidate();
+            if (INTEG == 1) {
+              L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false;
+              unsigned rc = sample<LAYOUT, UNSTEADY, false, CACHE>(a.g, st, cc, L.px, L.py, L.pz, L.t,
+                                                                   L.k1x, L.k1y, L.k1z);
+              n_samples++;
+              if (rc) { finish_particle(a, L, rc); active = false; atomicAdd(&s_tot[2], 1ull); }
+            }
+          }
+        }
+      }
+    }
+    if (__all_sync(FULL, !active)) {
+      if (__all_sync(FULL, exhausted)) break;
+      continue;
+    }
+    // ---- a2-a8: one step (RK4) or one attempt (DP5(4)) --------------------------------------
+    bool emit = false; int dest = 0;
+    if (active) {
+      unsigned rc;
+      if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE>(a, st, cc, L, n_samples, n_attempts);
+      else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE>(a, st, cc, L, n_samples, n_attempts);
+      if (BRICK && rc == 0) {                                                   // a8: owner of p_new
+        dest = owner_of(a.g, a.bm, L.px, L.py, L.pz);
+        if (dest != my_brick) rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF;
+      }
+      if (rc) {
+        active = false;
+        if (rc == RC_HANDOFF) emit = true; else finish_particle(a, L, rc);
+        atomicAdd(&s_tot[0], (unsigned long long)n_attempts);
+        atomicAdd(&s_tot[1], (unsigned long long)(L.n - n_start));
+        atomicAdd(&s_tot[2], (unsigned long long)n_samples);
+        if (emit) atomicAdd(&s_tot[3], 1ull);
+      }
+    }
+    if (BRICK) {
+      unsigned any = __ballot_sync(FULL, emit);
+      if (any) emit_outgoing(a, L, dest, emit);
+    }
+  }
+  __syncthreads();
+  if (a.totals && threadIdx.x < 4 && s_tot[threadIdx.x]) atomicAdd(a.totals + threadIdx.x, s_tot[threadIdx.x]);
+}
+
+}  // namespace streami

@@ -1,0 +1,168 @@
+"""GPU parity for the two round loops: streaklines (A7) and brick advection with hand-off (A9)."""
+import numpy as np
+import pytest
+
+from helpers import gpu_field
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def S():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_2606_02627_b200 as S_
+    S_.lib()
+    return S_
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    return t
+
+
+def gpu_streaklines(S, torch, field, pts, nsteps, **kw):
+    m = pts.shape[0]
+    d_pts = torch.from_numpy(np.ascontiguousarray(pts, dtype=np.float32)).cuda()
+    verts = torch.full((3, nsteps, m), float("nan"), dtype=torch.float32, device="cuda")
+    counts = torch.full((m,), -1, dtype=torch.int32, device="cuda")
+    steps = torch.full((nsteps * m,), -1, dtype=torch.int32, device="cuda")
+    status = torch.full((nsteps * m,), -1, dtype=torch.int32, device="cuda")
+    totals = torch.zeros(4, dtype=torch.int64, device="cuda")
+    prm = S.params(out_steps=steps, out_status=status, out_totals=totals, **kw)
+    S.streami_trace_streaklines(field, d_pts, nsteps, prm, verts, counts)
+    torch.cuda.synchronize()
+    return (verts.cpu().numpy(), counts.cpu().numpy().astype(np.uint32),
+            steps.cpu().numpy().astype(np.uint32), status.cpu().numpy().astype(np.uint32),
+            totals.cpu().numpy().astype(np.uint64))
+
+
+@pytest.mark.parametrize("layout", [1, 2, 3])
+@pytest.mark.parametrize("window", [0, 1, 7])
+def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window):
+    """A scaled-down config 4: double gyre slices, rake + a few points that leave or start outside."""
+    fld = wl.double_gyre_field(dims=(64, 32, 16), nslices=10, dt=0.25)
+    pts = wl.rake_c4(16, 8)
+    pts = np.concatenate([pts, np.array([[2.5, 0.5, 0.5], [1.999, 0.5, 0.999], [0.001, 0.999, 0.001]],
+                                        dtype=np.float32)])
+    nsteps = 90                               # t up to 4.5 > last slice time 2.25: frozen field (Q10)
+    kw = dict(integrator=0, h=0.05, vmin=0.0, t0=0.0)
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+    ref = oracle.streaklines(g, pts, nsteps, oracle.params(**kw), "f32")
+    S.streami_set_option("streak_window", window)
+    try:
+        v, counts, steps, status, totals = gpu_streaklines(S, torch, gpu_field(S, torch, fld, layout),
+                                                           pts, nsteps, **kw)
+    finally:
+        S.streami_set_option("streak_window", 0)
+    assert np.array_equal(status, ref.status) and np.array_equal(steps, ref.steps)
+    assert np.array_equal(counts, ref.counts)
+    assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(totals[:3], ref.totals[:3])
+    assert np.count_nonzero(ref.status == 1) >= nsteps       # the outside point, every release
+
+
+def test_streaklines_steady_field_with_deaths(S, torch, oracle, wl):
+    fld = wl.turb_field_cpu(32, 48, 1, 6)
+    pts = wl.seeds_uniform(3, 300, [31.0] * 3)
+    nsteps = 120
+    kw = dict(integrator=0, h=0.25, vmin=1e-6, t0=0.0)
+    ref = oracle.streaklines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), pts, nsteps,
+                             oracle.params(**kw), "f32")
+    for window in (0, 16):
+        S.streami_set_option("streak_window", window)
+        try:
+            v, counts, steps, status, totals = gpu_streaklines(S, torch, gpu_field(S, torch, fld), pts,
+                                                               nsteps, **kw)
+        finally:
+            S.streami_set_option("streak_window", 0)
+        assert np.array_equal(status, ref.status) and np.array_equal(steps, ref.steps)
+        assert np.array_equal(counts, ref.counts)
+        assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32))
+        assert np.array_equal(totals[:3], ref.totals[:3])
+    assert np.count_nonzero(ref.status == 1) > 100 and np.count_nonzero(ref.status == 2) > 100
+
+
+def gpu_bricks(S, torch, wl, fld, nb, seeds, ghost=1, layout=0, max_rounds=64, log_cap=None, **kw):
+    arrays = [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nb, ghost)]
+    f = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, ghost, arrays, layout)
+    n = seeds.shape[0]
+    cap = kw.get("capacity", 1)
+    nbricks = nb[0] * nb[1] * nb[2]
+    d_seeds = torch.from_numpy(np.ascontiguousarray(seeds, dtype=np.float32)).cuda()
+    verts = torch.full((3, n, cap), float("nan"), dtype=torch.float32, device="cuda")
+    counts = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    steps = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    status = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    final = torch.zeros((3, n), dtype=torch.float32, device="cuda")
+    totals = torch.zeros(4, dtype=torch.int64, device="cuda")
+    rcounts = torch.full((max_rounds, nbricks), -1, dtype=torch.int32, device="cuda")
+    log = torch.zeros(64 * n + 16 if log_cap is None else log_cap, dtype=torch.int64, device="cuda")
+    logc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    prm = S.params(out_steps=steps, out_status=status, out_final=final, out_totals=totals, **kw)
+    nrounds, truncated = S.streami_brick_advect(f, d_seeds, prm, verts, counts, rcounts, log, logc)
+    torch.cuda.synchronize()
+    nlog = int(logc.item())
+    return dict(vertices=verts.cpu().numpy(), counts=counts.cpu().numpy().astype(np.uint32),
+                steps=steps.cpu().numpy().astype(np.uint32),
+                status=status.cpu().numpy().astype(np.uint32), final=final.cpu().numpy(),
+                totals=totals.cpu().numpy().astype(np.uint64), nrounds=nrounds, truncated=truncated,
+                round_counts=rcounts.cpu().numpy(), nlog=nlog,
+                log=np.sort(log.cpu().numpy().view(np.uint64)[:min(nlog, log.numel())]))
+
+
+@pytest.mark.parametrize("nb,N,layout", [((2, 2, 2), 32, 3), ((2, 2, 2), 32, 1), ((3, 2, 1), 31, 2),
+                                         ((1, 1, 1), 24, 3)])
+def test_bricks_vs_oracle_and_monolithic(S, torch, oracle, wl, nb, N, layout):
+    fld = wl.turb_field_cpu(N, 48, 1, 6)
+    n = 30011
+    seeds = wl.seeds_uniform(42, n, [N - 1.0] * 3)
+    seeds[3] = [-1, 2, 2]; seeds[4] = [N - 1.0] * 3
+    kw = dict(integrator=0, h=0.25, max_steps=400, vmin=1e-6, capacity=101, stride=4)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    out = gpu_bricks(S, torch, wl, fld, nb, seeds, layout=layout, **kw)
+    assert not out["truncated"]
+    for key in ("status", "steps", "counts"):
+        assert np.array_equal(out[key], getattr(ref, key)), key
+    assert np.array_equal(out["final"].view(np.uint32), ref.final.view(np.uint32))
+    assert np.array_equal(out["vertices"].view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(out["totals"], ref.totals)
+    # queue membership: rounds, per-round per-brick counts, sorted hand-off log -- bit exact
+    assert out["nrounds"] == ref.nrounds and out["nlog"] == ref.nlog
+    assert np.array_equal(out["round_counts"][:ref.nrounds].astype(np.uint32),
+                          ref.round_counts[:ref.nrounds])
+    assert np.array_equal(out["log"], ref.log)
+    assert np.count_nonzero(ref.status == 4) == 0
+    if nb != (1, 1, 1):
+        assert ref.nrounds >= 3 and ref.nlog > n // 10
+    # P9 on the GPU: the brick-wise trace equals the monolithic GPU trace bit for bit
+    from helpers import gpu_streamlines
+    mono = gpu_streamlines(S, torch, gpu_field(S, torch, fld, layout), seeds, **kw)
+    for key in ("status", "steps", "counts"):
+        assert np.array_equal(out[key], mono[key]), key
+    assert np.array_equal(out["vertices"].view(np.uint32), mono["vertices"].view(np.uint32))
+
+
+def test_bricks_halo_miss_and_truncation(S, torch, oracle, wl):
+    N, nb = 9, (2, 1, 1)
+    fast = np.zeros((1, N, N, N, 3), dtype=np.float32); fast[..., 0] = 3.0
+    fld = wl.Field((N, N, N), (0, 0, 0), (1, 1, 1), fast)
+    seeds = np.array([[3.5, 4, 4], [4.0, 4, 4], [2.0, 4, 4]], dtype=np.float32)
+    kw = dict(integrator=0, h=1.0, max_steps=50, vmin=0.0, capacity=51)
+    out = gpu_bricks(S, torch, wl, fld, nb, seeds, **kw)
+    assert list(out["status"]) == [4, 1, 4]
+    # slow field: ping-pong free straight lines; tiny log and round table overflow -> TRUNCATED
+    slow = fast.copy(); slow[..., 0] = 1.0
+    fld = wl.Field((N, N, N), (0, 0, 0), (1, 1, 1), slow)
+    out = gpu_bricks(S, torch, wl, fld, nb, seeds, max_rounds=1, log_cap=1, **kw)
+    assert out["truncated"] and out["nlog"] == 2 and out["nrounds"] == 2
+    assert list(out["steps"]) == [4, 4, 6] and list(out["status"]) == [1, 1, 1]
+    assert list(out["round_counts"][0]) == [2, 1]
+    # nothing inside: zero rounds
+    out = gpu_bricks(S, torch, wl, fld, nb, np.full((5, 3), 99.0, dtype=np.float32), **kw)
+    assert out["nrounds"] == 0 and list(out["status"]) == [1] * 5 and out["nlog"] == 0
