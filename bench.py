@@ -1,0 +1,521 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the particle-update hot path on B200 (contract: task prompt, section 4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of
+synthetic input: one C-ABI trace call over all seeds of the workload -- Morton presort, the
+persistent advection kernel (fetch, cell location, trilinear gather, RK stages, termination,
+vertex record, refill) until every particle has terminated.  Default workload = BASELINE.json
+configs[1] (C2): 256^3 turbulence, 1,048,576 seeds, RK4 h = 0.25, max 2,000 steps, throughput
+recording (capacity 256, stride 8).
+
+metric  = RK particle-steps per second (step ATTEMPTS), whole job over all ranks.
+value   = device-resident inputs, CUDA events on the launching stream around each step.
+e2e     = the same through streami_trace_streamlines_host with pinned HOST buffers
+          (H2D of the seeds and D2H of every output inside the timed region).
+roofline= the advection kernel alone (event pair recorded by the library around its launch):
+          algorithmic bytes / its duration, against MEASURED_PEAKS.json.
+cpu_baseline = the fp32 oracle, as it stands, on the host cores, on a bounded strided sample.
+
+Multi-GPU (torchrun): the field is replicated, every rank traces its own 1,048,576 seeds
+(engine seed 42 + rank), no data-path collective -> "scaling": "weak".
+`--impl reference` times the CPU oracle instead (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "rk_particle_steps_per_sec"
+UNIT = "particle-steps/s"
+
+# name -> recipe (throughput-run recording parameters)
+WORKLOADS = {
+    "c1": dict(kind="abc", N=32, n=1024, ext=None, prm=dict(integrator=0, h=0.01, max_steps=1000,
+               vmin=1e-6, capacity=1001, stride=1)),
+    "c2": dict(kind="turb", N=256, M=512, kmax=64, n=1 << 20, prm=dict(integrator=0, h=0.25,
+               max_steps=2000, vmin=1e-6, capacity=256, stride=8)),
+    "c3": dict(kind="bricks", N=512, M=512, kmax=64, n=1 << 22, nb=(2, 2, 2), prm=dict(integrator=0,
+               h=0.25, max_steps=4000, vmin=1e-6, capacity=256, stride=16)),
+    "c4": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6)),
+    "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
+               h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
+               stride=128)),
+    # reduced sizes for quick checks of this script itself (never a reported number)
+    "tiny": dict(kind="turb", N=48, M=32, kmax=8, n=4096, prm=dict(integrator=0, h=0.25,
+                 max_steps=500, vmin=1e-6, capacity=64, stride=8)),
+}
+DESCR = {
+    "c1": "C1 ABC 32^3, 1,024 seeds, RK4 h=0.01, max 1,000",
+    "c2": "C2 turbulence 256^3 (512 modes), 1,048,576 seeds, RK4 h=0.25, max 2,000 steps",
+    "c3": "C3 turbulence 512^3 in 2x2x2 bricks (ghost 1), 4,194,304 seeds, RK4 h=0.25, max 4,000",
+    "c4": "C4 double gyre 256x128x64 x 64 slices, 4,096-point rake, 1,000 steps, streaklines",
+    "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
+    "tiny": "tiny turbulence 48^3 (script self-check only)",
+}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.thr = [], None, None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], None, [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                smax = float(f[1])
+                if t0 <= ts <= t1 + 0.2:
+                    sm.append(float(f[0])); power.append(float(f[2]))
+                    for k, nm in enumerate(names):
+                        if f[3 + k].lower().startswith("active"):
+                            reasons.add(nm)
+            except ValueError:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax,
+                "power_w_max": max(power) if power else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
+    ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 packed3, 2 float4, 3 xpair")
+    ap.add_argument("--opt", action="append", default=[], help="library option name=value")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+# workloads: device-resident inputs for our arm, host arrays for the oracle legs
+# ------------------------------------------------------------------------------------------------
+def host_inputs(name, rank, need_field=True):
+    """Host-side (numpy) field + seeds of a workload, for the oracle legs.  Large turbulence
+    fields are filled on the GPU when one is present (workloads/fill.cu, input generation only)
+    and copied back: the oracle then sees the same bytes as the CUDA path."""
+    import numpy as np
+    import workloads as wl
+    w = WORKLOADS[name]
+    if w["kind"] == "abc":
+        return wl.abc_field(w["N"]), wl.seeds_uniform(42 + rank, w["n"], [2 * np.pi] * 3)
+    if w["kind"] == "gyre":
+        return wl.double_gyre_field(), wl.rake_c4()
+    seeds = wl.seeds_uniform(42 + rank, w["n"], [w["N"] - 1.0] * 3)
+    fld = None
+    if need_field:
+        import torch
+        if torch.cuda.is_available():
+            fld, _ = wl.turb_field_cuda(w["N"], w["M"], 1.0, w["kmax"])
+        else:
+            if w["N"] > 64:
+                raise SystemExit("no GPU: the %d^3 field cannot be generated on the CPU in time" % w["N"])
+            fld = wl.turb_field_cpu(w["N"], w["M"], 1.0, w["kmax"])
+    return fld, seeds
+
+
+class Job:
+    """One workload on one GPU through the Python binding of the C ABI."""
+
+    def __init__(self, name, rank, layout):
+        import numpy as np
+        import torch
+        import workloads as wl
+        import paper_2606_02627_b200 as S
+        self.S, self.torch, self.np, self.name = S, torch, np, name
+        w = self.w = WORKLOADS[name]
+        self.kind = w["kind"]
+        self.host_field = None
+        if self.kind == "abc":
+            fld = self.host_field = wl.abc_field(w["N"])
+            self.data = torch.from_numpy(fld.data).cuda()
+            self.field = S.streami_field_create(fld.dims, fld.origin, fld.spacing, 1, 1.0, self.data, layout)
+            self.seeds_h = wl.seeds_uniform(42 + rank, w["n"], [2 * np.pi] * 3)
+        elif self.kind == "gyre":
+            fld = self.host_field = wl.double_gyre_field()
+            self.data = torch.from_numpy(fld.data).cuda()
+            self.field = S.streami_field_create(fld.dims, fld.origin, fld.spacing, fld.nslices,
+                                                fld.slice_dt, self.data, layout)
+            self.seeds_h = wl.rake_c4()
+        else:
+            N = w["N"]
+            want_host = N <= 512
+            fld, dev = wl.turb_field_cuda(N, w["M"], 1.0, w["kmax"], host=want_host)
+            self.host_field = fld
+            if self.kind == "bricks":
+                self.data = wl.cut_bricks_cuda(dev, (N, N, N), w["nb"], 1)
+                del dev
+                self.field = S.streami_field_create_bricked((N, N, N), (0, 0, 0), (1, 1, 1), w["nb"], 1,
+                                                            self.data, layout)
+            else:
+                self.data = dev
+                self.field = S.streami_field_create((N, N, N), (0, 0, 0), (1, 1, 1), 1, 1.0, dev, layout)
+            self.seeds_h = wl.seeds_uniform(42 + rank, w["n"], [N - 1.0] * 3)
+        self.layout, self.owned_bytes = self.field.info()
+        self.n = self.seeds_h.shape[0]
+        self.seeds = torch.from_numpy(self.seeds_h).cuda()
+        dev = "cuda"
+        if self.kind == "gyre":
+            self.nsteps = w["nsteps"]
+            npart = self.n * self.nsteps
+            self.verts = torch.empty((3, self.nsteps, self.n), dtype=torch.float32, device=dev)
+            self.counts = torch.empty(self.n, dtype=torch.int32, device=dev)
+        else:
+            npart = self.n
+            cap = w["prm"]["capacity"]
+            self.verts = torch.empty((3, self.n, cap), dtype=torch.float32, device=dev)
+            self.counts = torch.empty(self.n, dtype=torch.int32, device=dev)
+        self.npart = npart
+        self.steps_o = torch.empty(npart, dtype=torch.int32, device=dev)
+        self.status_o = torch.empty(npart, dtype=torch.int32, device=dev)
+        self.final_o = None if self.kind == "gyre" else torch.empty((3, self.n), dtype=torch.float32, device=dev)
+        self.totals_o = torch.zeros(4, dtype=torch.int64, device=dev)
+        self.prm = S.params(out_steps=self.steps_o, out_status=self.status_o, out_final=self.final_o,
+                            out_totals=self.totals_o, **w["prm"])
+        self.nrounds = 0
+        # pinned host buffers for the e2e leg
+        self.h = None
+
+    # -- one step, inputs and outputs resident in HBM ------------------------------------------
+    def step_device(self):
+        S = self.S
+        if self.kind == "gyre":
+            S.streami_trace_streaklines(self.field, self.seeds, self.nsteps, self.prm, self.verts, self.counts)
+        elif self.kind == "bricks":
+            self.nrounds, _ = S.streami_brick_advect(self.field, self.seeds, self.prm, self.verts, self.counts)
+        else:
+            S.streami_trace_streamlines(self.field, self.seeds, self.prm, self.verts, self.counts)
+
+    # -- one step through host buffers -----------------------------------------------------------
+    def _pinned(self):
+        t = self.torch
+        if self.h is None:
+            pin = lambda x: t.empty(x.shape, dtype=x.dtype).pin_memory()
+            self.h = dict(seeds=t.from_numpy(self.seeds_h).pin_memory(), verts=pin(self.verts),
+                          counts=pin(self.counts), steps=pin(self.steps_o), status=pin(self.status_o),
+                          final=None if self.final_o is None else pin(self.final_o),
+                          totals=t.zeros(4, dtype=t.int64).pin_memory())
+            if self.kind not in ("gyre", "bricks"):
+                self.prm_h = self.S.params(out_steps=None, out_status=None, out_final=None,
+                                           out_totals=None, **self.w["prm"])
+                self.prm_h.out_steps = self.h["steps"].data_ptr()
+                self.prm_h.out_status = self.h["status"].data_ptr()
+                self.prm_h.out_final = self.h["final"].data_ptr()
+                self.prm_h.out_totals = self.h["totals"].data_ptr()
+        return self.h
+
+    def e2e_bytes(self):
+        h = self._pinned()
+        nb = lambda x: 0 if x is None else x.numel() * x.element_size()
+        bi = nb(h["seeds"])
+        bo = sum(nb(h[k]) for k in ("verts", "counts", "steps", "status", "final", "totals"))
+        return bi, bo
+
+    def step_host(self):
+        """Streamlines: the C-ABI host-buffer call does the copies itself.  Streaklines and
+        bricks have no host-buffer entry point yet: the same copies are issued here around the
+        device call (pinned host -> device, device -> pinned host, then a stream sync)."""
+        h = self._pinned()
+        if self.kind not in ("gyre", "bricks"):
+            self.S.streami_trace_streamlines_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
+            return
+        self.seeds.copy_(h["seeds"], non_blocking=True)
+        self.step_device()
+        for k, d in (("verts", self.verts), ("counts", self.counts), ("steps", self.steps_o),
+                     ("status", self.status_o), ("final", self.final_o), ("totals", self.totals_o)):
+            if d is not None:
+                h[k].copy_(d, non_blocking=True)
+        self.torch.cuda.current_stream().synchronize()
+
+    def work(self):
+        """(attempted steps, accepted steps, field samples, hand-offs, stored vertices) of the
+        last device step."""
+        tot = [int(x) for x in self.totals_o.cpu().tolist()]
+        stored = self.npart if self.kind == "gyre" else int(self.counts.to(self.torch.int64).sum().item())
+        return tot[0], tot[1], tot[2], tot[3], stored
+
+    def algorithmic_bytes(self, samples, stored):
+        """useful gather bytes (8 vertices x 12 B per sample and slice) +
+        12 B per stored vertex + per-particle fetch (12 B) and results (24 B)."""
+        per_sample = 192 if self.kind == "gyre" else 96
+        return samples * per_sample + stored * 12 + self.npart * 36
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): the only places that execute oracle/
+# ------------------------------------------------------------------------------------------------
+class OracleRun:
+    """The fp32 CPU oracle, as it stands, on a strided sample of the workload's particles."""
+
+    def __init__(self, name, fld, seeds):
+        import oracle
+        import workloads as wl
+        self.o, self.name, self.w = oracle, name, WORKLOADS[name]
+        self.kind = self.w["kind"]
+        self.seeds = seeds
+        oracle.build()
+        prm = dict(self.w["prm"])
+        if self.kind == "gyre":
+            prm.update(capacity=1, stride=1, max_steps=self.w["nsteps"])
+        self.prm = oracle.params(**prm)
+        if self.kind == "bricks":
+            N = self.w["N"]
+            boxes = wl.brick_boxes(fld.dims, self.w["nb"], 1)
+            cut = wl.cut_bricks(fld, self.w["nb"], 1)
+            self.field = [oracle.grid(c, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+                          for c, (lo, hi) in zip(cut, boxes)]
+        else:
+            self.field = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+        self.cores = oracle.num_threads()
+
+    def run(self, stride):
+        """Trace every stride-th particle; returns (attempted steps, seconds, particles)."""
+        o = self.o
+        sub = self.seeds[::stride]
+        t0 = time.perf_counter()
+        if self.kind == "gyre":
+            r = o.streaklines(self.field, sub, self.w["nsteps"], self.prm, "f32")
+        elif self.kind == "bricks":
+            r = o.brick_advect(self.field, self.w["nb"], sub, self.prm, "f32", record=False)
+        else:
+            r = o.streamlines(self.field, sub, self.prm, "f32", record=False)
+        dt = time.perf_counter() - t0
+        npart = sub.shape[0] * (self.w["nsteps"] if self.kind == "gyre" else 1)
+        return int(r.totals[0]), dt, npart
+
+    def bounded(self, seconds):
+        """Pick the stride so that one run takes about `seconds` (probe first), then run it."""
+        n = self.seeds.shape[0]
+        probe = max(1, n // max(64, 16 * self.cores))
+        a, dt, _ = self.run(probe)
+        rate = a / max(dt, 1e-6)
+        per_particle = max(a, 1) / max(1, len(range(0, n, probe)))
+        want = max(1.0, rate * seconds / per_particle)
+        stride = max(1, int(n / want))
+        a, dt, npart = self.run(stride)
+        return a, dt, npart, stride
+
+
+def reference_arm(args, rank):
+    """--impl reference: the oracle on the host cores; each step = one bounded sample."""
+    if rank != 0:
+        return
+    fld, seeds = host_inputs(args.workload, 0)
+    orc = OracleRun(args.workload, fld, seeds)
+    per_step = max(2.0, min(30.0, 150.0 / max(1, args.steps + args.warmup)))
+    a, dt, npart, stride = orc.bounded(per_step)
+    for _ in range(max(0, args.warmup - 1)):
+        orc.run(stride)
+    tot_a, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        a, dt, npart = orc.run(stride)
+        tot_a += a; tot_t += dt
+    value = tot_a / tot_t
+    sample = "every %d-th particle (%d particles, %d step attempts per step)" % (stride, npart, tot_a // max(1, args.steps))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": {"workload": DESCR[args.workload], "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        reference_arm(args, rank)
+        return
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def allmax(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def allsum(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    import paper_2606_02627_b200 as S
+    for kv in args.opt:
+        k, v = kv.split("=")
+        S.streami_set_option(k, int(v))
+    job = Job(args.workload, rank, args.layout)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    for _ in range(args.warmup):
+        job.step_device()
+    torch.cuda.synchronize()
+    attempts, accepted, samples, handoffs, stored = job.work()
+
+    # ---- timed region: exactly K steps, device-resident ---------------------------------------
+    S.streami_set_option("kernel_timing", 1)
+    S.streami_kernel_time()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    l0 = S.streami_launch_count()
+    t0 = time.time()
+    for a, b in ev:
+        flush.zero_()                       # L2 flush between timed iterations (outside the events)
+        a.record()
+        job.step_device()
+        b.record()
+    barrier()
+    t1 = time.time()
+    launches = S.streami_launch_count() - l0
+    clocks = sampler.stop(t0, t1) if sampler else None
+    kern_ms, kern_n = S.streami_kernel_time()
+    S.streami_set_option("kernel_timing", 0)
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    total_ms = allmax(total_ms)
+    job_attempts = allsum(float(attempts))
+    value = job_attempts * args.steps / (total_ms * 1e-3)
+
+    # ---- e2e: host buffers, copies inside the timed region --------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        bi, bo = job.e2e_bytes()
+        job.step_host()
+        barrier()
+        w0 = time.perf_counter()
+        for _ in range(args.steps):
+            job.step_host()
+        torch.cuda.synchronize()
+        w1 = time.perf_counter()
+        e_ms = allmax((w1 - w0) * 1e3)
+        e2e = {"value": job_attempts * args.steps / (e_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "ms_per_step": e_ms / args.steps}
+        barrier()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the advection kernel (rank 0) ----------------------------------------------
+    peak, peak_src = peaks()
+    alg = job.algorithmic_bytes(samples, stored)
+    launches_per_step = max(1, kern_n // max(1, args.steps))
+    kms = kern_ms / max(1, kern_n)
+    achieved = (alg / launches_per_step) / (kms * 1e-3) / 1e9 if kms > 0 else None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": None if achieved is None else achieved / peak, "traffic": None,
+                "kernel": "trace_kernel" if job.kind != "gyre" else "streak_kernel",
+                "kernel_ms_per_launch": kms, "kernel_launches_per_step": launches_per_step,
+                "algorithmic_bytes_per_launch": alg / launches_per_step, "peak_source": peak_src,
+                "kernel_share_of_step": kern_ms / total_ms if world == 1 else None}
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            tr = json.load(f).get(args.workload)
+        if tr:
+            roofline["traffic"] = tr["dram_bytes_per_launch"]
+            roofline["traffic_source"] = tr["source"]
+
+    cpu = None
+    if world == 1 and not args.no_cpu and job.host_field is not None:
+        orc = OracleRun(args.workload, job.host_field, job.seeds_h)
+        a, dt, npart, stride = orc.bounded(args.cpu_seconds)
+        cpu = {"value": a / dt, "unit": UNIT, "cores": orc.cores, "kind": "oracle",
+               "sample": "every %d-th particle of the same workload (%d particles, %d step attempts, %.1f s)"
+                         % (stride, npart, a, dt)}
+
+    lay = {1: "packed3", 2: "float4", 3: "xpair"}.get(job.layout, str(job.layout))
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": DESCR[args.workload], "seeds_per_gpu": job.n,
+                   "recording": {k: job.w["prm"][k] for k in ("capacity", "stride") if k in job.w["prm"]},
+                   "field_layout": lay, "field_bytes_owned": job.owned_bytes,
+                   "l2": "flushed between timed steps (256 MiB memset) and the field is larger than L2",
+                   "parallelism": "seeds sharded over %d GPU(s), field replicated" % world,
+                   "options": {k: S.streami_get_option(k) for k in ("cell_cache", "presort")}},
+        "work_per_step_per_gpu": {"step_attempts": attempts, "accepted_steps": accepted,
+                                  "field_samples": samples, "handoffs": handoffs,
+                                  "stored_vertices": stored, "rounds": job.nrounds},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -168,12 +168,18 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
 /* Tuning knobs for measurement (process-wide, not part of the method): name is one of
  * "cell_cache" (0/1, reuse the 8 cell vertices in registers while a sample stays in the cell),
  * "presort" (0/1, order seeds by coarse Morton bin before tracing), "streak_window" (global
- * steps per launch, 0 = automatic).  Returns INVALID for unknown names. */
+ * steps per launch, 0 = automatic), "kernel_timing" (0/1, record a CUDA event pair on the
+ * launching stream around every advection-kernel launch).  Returns INVALID for unknown names. */
 int streami_set_option(const char* name, int value);
 int streami_get_option(const char* name, int* value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */
 unsigned long long streami_launch_count(void);
+
+/* With option "kernel_timing" = 1: device time (ms) of the advection-kernel launches recorded
+ * since the previous call of this function, and how many there were; waits for those launches
+ * to finish (event synchronise), then forgets them.  launches may be NULL. */
+int streami_kernel_time(float* total_ms, unsigned* launches);
 
 const char* streami_error_string(int code);
 

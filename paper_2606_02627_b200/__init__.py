@@ -57,6 +57,7 @@ def lib():
         L.streami_set_option.argtypes = [ctypes.c_char_p, I]
         L.streami_get_option.argtypes = [ctypes.c_char_p, P]
         L.streami_launch_count.restype = ctypes.c_ulonglong
+        L.streami_kernel_time.argtypes = [P, P]
         L.streami_error_string.restype = ctypes.c_char_p
         L.streami_error_string.argtypes = [I]
         _lib = L
@@ -221,3 +222,11 @@ def streami_get_option(name):
 
 def streami_launch_count():
     return lib().streami_launch_count()
+
+
+def streami_kernel_time():
+    """(total_ms, launches) of the advection-kernel launches since the last call (option
+    "kernel_timing" must be 1)."""
+    ms, cnt = ctypes.c_float(0.0), ctypes.c_uint(0)
+    _check(lib().streami_kernel_time(ctypes.byref(ms), ctypes.byref(cnt)))
+    return ms.value, cnt.value

@@ -3,13 +3,15 @@
 #include <cmath>
 #include <cstring>
 #include <mutex>
+#include <utility>
+#include <vector>
 
 #include "internal.h"
 #include "misc_kernels.cuh"
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0}; return o; }
+Options& options() { static Options o{1, 1, 0, 0}; return o; }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -28,6 +30,35 @@ int num_sms() {
     if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
   }
   return n;
+}
+
+static std::mutex g_time_mutex;
+static std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_time_pairs;   // recorded, not yet read
+static std::vector<cudaEvent_t> g_time_free;
+static cudaEvent_t g_time_open = nullptr;
+
+static cudaEvent_t take_event() {
+  if (!g_time_free.empty()) { cudaEvent_t e = g_time_free.back(); g_time_free.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+  return e;
+}
+
+void timing_begin(cudaStream_t st) {
+  if (!options().kernel_timing) return;
+  std::lock_guard<std::mutex> lk(g_time_mutex);
+  g_time_open = take_event();
+  if (g_time_open) cudaEventRecord(g_time_open, st);
+}
+
+void timing_end(cudaStream_t st) {
+  if (!options().kernel_timing) return;
+  std::lock_guard<std::mutex> lk(g_time_mutex);
+  if (!g_time_open) return;
+  cudaEvent_t e = take_event();
+  if (e) { cudaEventRecord(e, st); g_time_pairs.emplace_back(g_time_open, e); }
+  else g_time_free.push_back(g_time_open);
+  g_time_open = nullptr;
 }
 
 static bool finite_pos(float x) { return std::isfinite(x) && x > 0.0f; }
@@ -220,6 +251,7 @@ int streami_set_option(const char* name, int value) {
   if (!strcmp(name, "cell_cache")) o.cell_cache = value != 0;
   else if (!strcmp(name, "presort")) o.presort = value != 0;
   else if (!strcmp(name, "streak_window")) o.streak_window = value < 0 ? 0 : value;
+  else if (!strcmp(name, "kernel_timing")) o.kernel_timing = value != 0;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }
@@ -230,11 +262,30 @@ int streami_get_option(const char* name, int* value) {
   if (!strcmp(name, "cell_cache")) *value = o.cell_cache;
   else if (!strcmp(name, "presort")) *value = o.presort;
   else if (!strcmp(name, "streak_window")) *value = o.streak_window;
+  else if (!strcmp(name, "kernel_timing")) *value = o.kernel_timing;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }
 
 unsigned long long streami_launch_count(void) { return launch_counter().load(); }
+
+int streami_kernel_time(float* total_ms, unsigned* launches) {
+  if (!total_ms) return STREAMI_E_INVALID;
+  std::lock_guard<std::mutex> lk(g_time_mutex);
+  float sum = 0.0f; unsigned cnt = 0;
+  cudaError_t err = cudaSuccess;
+  for (auto& pr : g_time_pairs) {
+    float ms = 0.0f;
+    cudaError_t e = cudaEventSynchronize(pr.second);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, pr.first, pr.second);
+    if (e == cudaSuccess) { sum += ms; cnt++; } else err = e;
+    g_time_free.push_back(pr.first); g_time_free.push_back(pr.second);
+  }
+  g_time_pairs.clear();
+  *total_ms = sum;
+  if (launches) *launches = cnt;
+  return check(err);
+}
 
 const char* streami_error_string(int code) {
   switch (code) {

@@ -66,7 +66,9 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
   for (unsigned s0 = 0; s0 < nsteps && e == cudaSuccess; s0 += K) {
     a.s0 = s0; a.s1 = std::min(nsteps, s0 + K);
     unsigned long long threads = (unsigned long long)m * a.s1;
+    timing_begin(st);
     k<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(a);
+    timing_end(st);
     launch_counter()++;
     e = cudaGetLastError();
   }
@@ -148,7 +150,9 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
     int grid = 0;
     rc = trace_grid(k, nwork, &grid);
     if (rc) { cleanup(); return rc; }
+    timing_begin(st);
     k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+    timing_end(st);
     launch_counter()++;
     e = cudaGetLastError();
     if (e != cudaSuccess) break;

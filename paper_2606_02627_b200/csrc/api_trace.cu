@@ -133,7 +133,9 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.next = next; a.round = 0;
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  timing_begin(st);
   k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+  timing_end(st);
   launch_counter()++;
   e = cudaGetLastError();
   cleanup();

@@ -22,7 +22,7 @@ struct streami_field_s {
 
 namespace streami {
 
-struct Options { int cell_cache; int presort; int streak_window; };
+struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; };
 Options& options();
 std::atomic<unsigned long long>& launch_counter();
 void set_cuda_error(cudaError_t e);
@@ -46,5 +46,11 @@ inline int check(cudaError_t e) {
   } while (0)
 
 int num_sms();
+
+// Optional device timing of the advection kernel alone (option "kernel_timing"): a pair of CUDA
+// events recorded on the launching stream around each advection launch, summed by
+// streami_kernel_time().  Off by default; bench.py's roofline leg turns it on.
+void timing_begin(cudaStream_t st);
+void timing_end(cudaStream_t st);
 
 }  // namespace streami

@@ -150,3 +150,89 @@ def cut_bricks(fld, brick_grid, ghost=1):
         out.append(np.ascontiguousarray(
             vol[lo[2]:hi[2] + 1, lo[1]:hi[1] + 1, lo[0]:hi[0] + 1, :]))
     return out
+
+
+# ---- CUDA generators for the large fields (input generation only; see workloads/fill.cu) ------
+_cuda = None
+
+
+def _cuda_lib():
+    global _cuda
+    if _cuda is None:
+        L = ctypes.CDLL(_build.build_cuda())
+        P, i32, f64, Z = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        L.wl_cuda_turb_partials.argtypes = [Z]
+        L.wl_cuda_turb_partials.restype = Z
+        L.wl_cuda_turb_fill.argtypes = [P, P, i32, P, P, P, P]
+        L.wl_cuda_scale_round.argtypes = [Z, P, f64, P, P]
+        L.wl_cuda_cut_box.argtypes = [P, P, P, P, P, P]
+        _cuda = L
+    return _cuda
+
+
+def turb_field_cuda(N, M, kmin, kmax, seed=2606, host=True, zchunk=64):
+    """Turbulence generator on the GPU (C2/C3/C5 sizes), same recipe and mode table as
+    turb_field_cpu: fp64 evaluation, one normalisation over the whole grid, one rounding to
+    fp32.  Returns (Field or None, cuda tensor [1,N,N,N,3]); Field.data is the host copy of the
+    SAME bytes (host=False skips it).  The fp64 intermediate is produced in z-chunks; per-block
+    sums of squares are added on the host in block order, so the result is deterministic."""
+    import torch
+    L = _cuda_lib()
+    table = turb_modes(seed, M, kmin, kmax, N)
+    d_table = torch.from_numpy(table).cuda()
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    out = torch.empty((1, N, N, N, 3), dtype=torch.float32, device="cuda")
+    # pass 1: sum of squares (fp64 values kept per chunk only when everything fits one chunk)
+    zchunk = min(zchunk, N)
+    tmp = torch.empty((zchunk, N, N, 3), dtype=torch.float64, device="cuda")
+    part = torch.empty(L.wl_cuda_turb_partials(zchunk * N * N), dtype=torch.float64, device="cuda")
+    sumsq = 0.0
+
+    def fill(z0, nz):
+        dims = (ctypes.c_int * 3)(N, N, nz)
+        lo = (ctypes.c_int * 3)(0, 0, z0)
+        rc = L.wl_cuda_turb_fill(dims, lo, M, d_table.data_ptr(), tmp.data_ptr(), part.data_ptr(), st)
+        if rc:
+            raise RuntimeError("wl_cuda_turb_fill: cudaError %d" % rc)
+        return L.wl_cuda_turb_partials(nz * N * N)
+
+    for z0 in range(0, N, zchunk):
+        nz = min(zchunk, N - z0)
+        nb = fill(z0, nz)
+        sumsq += float(np.sum(part[:nb].cpu().numpy(), dtype=np.float64))
+    scale = 1.0 / math.sqrt(sumsq / float(N) ** 3)
+    # pass 2: (re)compute each chunk, scale in fp64, round once to fp32
+    for z0 in range(0, N, zchunk):
+        nz = min(zchunk, N - z0)
+        if N > zchunk:
+            fill(z0, nz)
+        dst = out[0, z0:z0 + nz]
+        rc = L.wl_cuda_scale_round(nz * N * N * 3, tmp.data_ptr(), scale, dst.data_ptr(), st)
+        if rc:
+            raise RuntimeError("wl_cuda_scale_round: cudaError %d" % rc)
+    torch.cuda.synchronize()
+    del tmp, part
+    fld = None
+    if host:
+        fld = Field((N, N, N), (0.0, 0.0, 0.0), (1.0, 1.0, 1.0), out.cpu().numpy())
+    return fld, out
+
+
+def cut_bricks_cuda(vol, global_dims, brick_grid, ghost=1):
+    """Brick cut on the device: vol is a cuda tensor [1,Nz,Ny,Nx,3]; returns one cuda tensor per
+    brick (each its own allocation), same boxes as cut_bricks."""
+    import torch
+    L = _cuda_lib()
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    N = (ctypes.c_int * 3)(*global_dims)
+    out = []
+    for lo, hi in brick_boxes(global_dims, brick_grid, ghost):
+        shp = (hi[2] - lo[2] + 1, hi[1] - lo[1] + 1, hi[0] - lo[0] + 1, 3)
+        t = torch.empty(shp, dtype=torch.float32, device="cuda")
+        rc = L.wl_cuda_cut_box(vol.data_ptr(), N, (ctypes.c_int * 3)(*lo), (ctypes.c_int * 3)(*hi),
+                               t.data_ptr(), st)
+        if rc:
+            raise RuntimeError("wl_cuda_cut_box: cudaError %d" % rc)
+        out.append(t)
+    torch.cuda.synchronize()
+    return out
