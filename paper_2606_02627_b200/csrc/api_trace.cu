@@ -71,8 +71,9 @@ int presort_seeds(const streami_field_s* f, const float* seeds, size_t n, unsign
   unsigned bits = 0;
   while ((1u << bits) <= (unsigned)((maxdim - 1) >> shift)) bits++;
   unsigned nbins = 1u << (3 * bits);
-  unsigned* hist = nullptr; unsigned* keys = nullptr;
-  STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * nbins, st));
+  const unsigned nseg = (nbins + PRESORT_SEG - 1) / PRESORT_SEG;
+  unsigned* hist = nullptr; unsigned* keys = nullptr;   // hist: [nbins] counts + [nseg] totals
+  STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * ((size_t)nbins + nseg), st));
   cudaError_t e = cudaMallocAsync((void**)&keys, sizeof(unsigned) * n, st);
   if (e != cudaSuccess) { cudaFreeAsync(hist, st); return check(e); }
   int rc = STREAMI_OK;
@@ -80,9 +81,10 @@ int presort_seeds(const streami_field_s* f, const float* seeds, size_t n, unsign
   e = cudaMemsetAsync(hist, 0, sizeof(unsigned) * nbins, st);
   if (e == cudaSuccess) {
     presort_hist_kernel<<<blocks, 256, 0, st>>>(f->g, shift, seeds, n, hist, keys);
-    presort_scan_kernel<<<1, 1024, 0, st>>>(hist, nbins);
-    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, perm);
-    launch_counter() += 3;
+    presort_scan_seg_kernel<<<nseg, 256, 0, st>>>(hist, nbins, hist + nbins);
+    presort_scan_top_kernel<<<1, 1024, 0, st>>>(hist + nbins, nseg);
+    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, hist + nbins, perm);
+    launch_counter() += 4;
     e = cudaGetLastError();
   }
   if (e != cudaSuccess) rc = check(e);

@@ -37,13 +37,46 @@ static __global__ void presort_hist_kernel(Geom g, int shift, const float* __res
   atomicAdd(hist + k, 1u);
 }
 
-// Exclusive scan of `hist` in place, one block of 1024 threads, nbins arbitrary.
-static __global__ void presort_scan_kernel(unsigned* __restrict__ hist, unsigned nbins) {
+// Exclusive scan of `hist` in two levels.  Level 1: each block scans one segment of 1024 bins in
+// place (4 consecutive bins per thread, warp shuffles, one shared-memory hop) and writes the
+// segment total.  Level 2: one block scans the <= 2048 segment totals.  The scatter adds both.
+constexpr unsigned PRESORT_SEG = 1024;
+
+static __global__ void __launch_bounds__(256)
+presort_scan_seg_kernel(unsigned* __restrict__ hist, unsigned nbins, unsigned* __restrict__ seg_total) {
+  __shared__ unsigned s_warp[8];
+  const unsigned base = blockIdx.x * PRESORT_SEG + threadIdx.x * 4u;
+  unsigned c[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) c[k] = (base + k < nbins) ? hist[base + k] : 0u;
+  const unsigned mine = c[0] + c[1] + c[2] + c[3];
+  unsigned incl = mine;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    unsigned v = __shfl_up_sync(0xffffffffu, incl, d);
+    if (lane >= d) incl += v;
+  }
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  unsigned woff = 0;
+  for (int w = 0; w < warp; ++w) woff += s_warp[w];
+  unsigned run = woff + incl - mine;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    if (base + k < nbins) hist[base + k] = run;
+    run += c[k];
+  }
+  if (threadIdx.x == 255) seg_total[blockIdx.x] = run;
+}
+
+static __global__ void __launch_bounds__(1024)
+presort_scan_top_kernel(unsigned* __restrict__ seg_total, unsigned nseg) {
   __shared__ unsigned s_part[1024];
-  const unsigned per = (nbins + 1023u) / 1024u;
-  const unsigned lo = threadIdx.x * per, hi = min(lo + per, nbins);
+  const unsigned per = (nseg + 1023u) / 1024u;
+  const unsigned lo = threadIdx.x * per, hi = min(lo + per, nseg);
   unsigned sum = 0;
-  for (unsigned k = lo; k < hi; ++k) sum += hist[k];
+  for (unsigned k = lo; k < hi; ++k) sum += seg_total[k];
   s_part[threadIdx.x] = sum;
   __syncthreads();
   for (unsigned d = 1; d < 1024; d <<= 1) {                 // Hillis-Steele inclusive scan
@@ -53,14 +86,17 @@ static __global__ void presort_scan_kernel(unsigned* __restrict__ hist, unsigned
     __syncthreads();
   }
   unsigned run = s_part[threadIdx.x] - sum;
-  for (unsigned k = lo; k < hi; ++k) { unsigned c = hist[k]; hist[k] = run; run += c; }
+  for (unsigned k = lo; k < hi; ++k) { unsigned c = seg_total[k]; seg_total[k] = run; run += c; }
 }
 
 static __global__ void presort_scatter_kernel(const unsigned* __restrict__ keys, unsigned long long n,
-                                       unsigned* __restrict__ offsets, unsigned* __restrict__ perm) {
+                                       unsigned* __restrict__ offsets,
+                                       const unsigned* __restrict__ seg_base,
+                                       unsigned* __restrict__ perm) {
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  unsigned pos = atomicAdd(offsets + keys[i], 1u);
+  const unsigned k = keys[i];
+  unsigned pos = atomicAdd(offsets + k, 1u) + seg_base[k / PRESORT_SEG];
   perm[pos] = (unsigned)i;
 }
 

@@ -1,0 +1,190 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The CUDA path runs the whole workload (bench.Job: same field generator, seeds, parameters, layout
+and options as the timed run); the oracle runs a strided sample of the particles one by one on
+the SAME field bytes (copied from the device) and every per-particle output of those ids is
+compared bit for bit.  Properties that hold at any size (P10 invariants) are checked on all ids.
+Tolerance: the formula sheet makes both sides execute the same IEEE operations, so the bar here is
+bit-exact (stricter than north_star's 99.9 % / 1e-4 cell, which tests/test_gpu_parity.py
+::test_gpu_tolerance_form also evaluates).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return t
+
+
+@pytest.fixture(scope="module")
+def bench():
+    import bench as b
+    return b
+
+
+def _gpu_outputs(job, torch, ids):
+    job.step_device()
+    torch.cuda.synchronize()
+    idx = torch.from_numpy(ids.astype(np.int64)).cuda()
+    out = dict(counts=job.counts[idx].cpu().numpy().astype(np.uint32),
+               steps=job.steps_o[idx].cpu().numpy().astype(np.uint32),
+               status=job.status_o[idx].cpu().numpy().astype(np.uint32),
+               final=job.final_o[:, idx].cpu().numpy(),
+               vertices=job.verts[:, idx, :].cpu().numpy())
+    return out
+
+
+def _invariants(job, torch, max_steps, cap, N):
+    """P10 on ALL particles: status in 1..4, steps <= max_steps, counts <= capacity, final inside."""
+    st = job.status_o
+    assert int(st.min()) >= 1 and int(st.max()) <= 4
+    assert int(job.steps_o.max()) <= max_steps
+    assert int(job.counts.max()) <= cap and int(job.counts.min()) >= 0
+    f = job.final_o
+    assert bool(((f >= 0) & (f <= N - 1)).all())
+    tot = job.totals_o.cpu().numpy()
+    assert int(tot[1]) == int(job.steps_o.to(torch.int64).sum().item())      # accepted steps
+    assert tot[0] >= tot[1]
+
+
+def _compare(gpu, ref, what):
+    k = gpu["counts"].shape[0]
+    assert np.array_equal(gpu["status"], ref.status), what + " status"
+    assert np.array_equal(gpu["steps"], ref.steps), what + " steps"
+    assert np.array_equal(gpu["counts"], ref.counts), what + " counts"
+    assert np.array_equal(gpu["final"].view(np.uint32), ref.final.view(np.uint32)), what + " final"
+    cap = gpu["vertices"].shape[2]
+    mask = np.arange(cap)[None, :] < ref.counts[:, None]                      # stored slots only
+    for c in range(3):
+        a = gpu["vertices"][c].view(np.uint32)[mask]
+        b = ref.vertices[c].view(np.uint32)[mask]
+        assert np.array_equal(a, b), what + " vertices plane %d" % c
+    assert k == ref.status.shape[0]
+
+
+def test_c2_full_size_sampled(torch, bench, oracle):
+    """C2 (the bench default): 256^3 turbulence, 1,048,576 seeds, RK4 h = 0.25, max 2,000 steps,
+    capacity 256 stride 8; oracle on every 64th seed (16,384 particles)."""
+    job = bench.Job("c2", 0, 0)
+    fld = job.host_field
+    ids = np.arange(0, job.n, 64)
+    gpu = _gpu_outputs(job, torch, ids)
+    _invariants(job, torch, 2000, 256, 256)
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing)
+    ref = oracle.streamlines(g, job.seeds_h[ids], oracle.params(**job.w["prm"]), "f32")
+    _compare(gpu, ref, "c2")
+    # workload shape, recorded in DESIGN.md section 4
+    st = job.steps_o.float()
+    print("C2 steps/particle mean %.1f median %.1f at cap %.3f" %
+          (st.mean().item(), st.median().item(), (job.steps_o == 2000).float().mean().item()))
+
+
+def test_c2_parity_recording_first_200_vertices(torch, bench, oracle, wl):
+    """C2 with the parity-run recording (capacity 201, stride 1): every one of the first 200
+    vertices of every 256th particle, bit for bit, plus north_star's tolerance form."""
+    import paper_2606_02627_b200 as S
+    job = bench.Job("c2", 0, 0)
+    fld = job.host_field
+    prm = dict(job.w["prm"]); prm.update(capacity=201, stride=1)
+    n = job.n
+    verts = torch.empty((3, n, 201), dtype=torch.float32, device="cuda")
+    job.verts = verts
+    job.prm = S.params(out_steps=job.steps_o, out_status=job.status_o, out_final=job.final_o,
+                       out_totals=job.totals_o, **prm)
+    ids = np.arange(0, n, 256)
+    gpu = _gpu_outputs(job, torch, ids)
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing)
+    ref = oracle.streamlines(g, job.seeds_h[ids], oracle.params(**prm), "f32")
+    _compare(gpu, ref, "c2 parity run")
+    mask = np.arange(201)[None, :] < ref.counts[:, None]
+    d = np.abs(gpu["vertices"].astype(np.float64) - ref.vertices.astype(np.float64))
+    assert float(d[:, mask].max()) <= 1e-4            # cell widths (spacing 1), first 200 steps
+    assert np.mean(gpu["status"] == ref.status) >= 0.999
+
+
+def test_c3_full_size_sampled(torch, bench, oracle, wl):
+    """C3: 512^3 turbulence in 2x2x2 bricks, 4,194,304 seeds, rounds until all terminate; oracle
+    (brick rounds, A9) on every 256th seed.  Also: no HALO_MISS anywhere (Q14) and the hand-off
+    log restricted to the sampled ids equals the oracle's."""
+    job = bench.Job("c3", 0, 0)
+    fld = job.host_field
+    n = job.n
+    log = torch.zeros(16 * n, dtype=torch.int64, device="cuda")
+    logc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    rcounts = torch.zeros((256, 8), dtype=torch.int32, device="cuda")
+    import paper_2606_02627_b200 as S
+    nrounds, trunc = S.streami_brick_advect(job.field, job.seeds, job.prm, job.verts, job.counts,
+                                            rcounts, log, logc)
+    torch.cuda.synchronize()
+    assert not trunc
+    ids = np.arange(0, n, 256)
+    idx = torch.from_numpy(ids.astype(np.int64)).cuda()
+    gpu = dict(counts=job.counts[idx].cpu().numpy().astype(np.uint32),
+               steps=job.steps_o[idx].cpu().numpy().astype(np.uint32),
+               status=job.status_o[idx].cpu().numpy().astype(np.uint32),
+               final=job.final_o[:, idx].cpu().numpy(), vertices=job.verts[:, idx, :].cpu().numpy())
+    _invariants(job, torch, 4000, 256, 512)
+    assert int((job.status_o == 4).sum().item()) == 0, "HALO_MISS must not occur in C3 (Q14)"
+    boxes = wl.brick_boxes(fld.dims, (2, 2, 2), 1)
+    cut = wl.cut_bricks(fld, (2, 2, 2), 1)
+    bricks = [oracle.grid(c, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for c, (lo, hi) in zip(cut, boxes)]
+    ref = oracle.brick_advect(bricks, (2, 2, 2), job.seeds_h[ids], oracle.params(**job.w["prm"]), "f32")
+    _compare(gpu, ref, "c3")
+    # hand-off log: entries (round+1)<<48 | dest<<32 | id; restrict to sampled ids, renumber, sort
+    nlog = int(logc.item())
+    assert nlog <= log.numel()
+    L = log[:nlog].cpu().numpy().astype(np.uint64)
+    lid = (L & np.uint64(0xffffffff)).astype(np.int64)
+    sel = (lid % 256) == 0
+    mine = np.sort((L[sel] & ~np.uint64(0xffffffff)) | (lid[sel] // 256).astype(np.uint64))
+    assert np.array_equal(mine, ref.log), "hand-off log membership"
+    # P10: round table sums
+    rc = rcounts.cpu().numpy().astype(np.int64)
+    assert rc[0].sum() == n, "Q_0 holds every (inside) seed once"
+    assert rc[1:nrounds + 1].sum() == nlog, "total hand-offs = sum of later queue sizes"
+    assert int(job.totals_o[3].item()) == nlog
+
+
+def test_c4_full_size_sampled(torch, bench, oracle):
+    """C4: double gyre 256x128x64 x 64 slices, 4,096-point rake, 1,000 global steps; oracle on
+    every 64th rake point (64 points x 1,000 releases)."""
+    job = bench.Job("c4", 0, 0)
+    fld = job.host_field
+    job.step_device()
+    torch.cuda.synchronize()
+    m, ns = job.n, job.nsteps
+    pts = np.arange(0, m, 64)
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+    prm = oracle.params(integrator=0, h=0.05, vmin=1e-6, max_steps=ns, capacity=1, stride=1)
+    ref = oracle.streaklines(g, job.seeds_h[pts], ns, prm, "f32")
+    v = job.verts.cpu().numpy()[:, :, pts]                                   # [3][ns][k]
+    assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32)), "c4 slots"
+    st = job.status_o.cpu().numpy().astype(np.uint32).reshape(ns, m)[:, pts].reshape(-1)
+    sp = job.steps_o.cpu().numpy().astype(np.uint32).reshape(ns, m)[:, pts].reshape(-1)
+    assert np.array_equal(st, ref.status), "c4 status"
+    dead = ref.status != 2
+    assert np.array_equal(sp[dead], ref.steps[dead]), "c4 steps of the dead"
+    assert np.array_equal(job.counts.cpu().numpy().astype(np.uint32)[pts], ref.counts), "c4 counts"
+
+
+def test_c5_full_size_sampled(torch, bench, oracle):
+    """C5: 1024^3 turbulence (12.9 GB), 16,777,216 seeds, DP5(4) tol 1e-5, h in [0.01, 1], max
+    8,000 accepted steps, capacity 64 stride 128; oracle on every 2048th seed (8,192 particles)
+    on a host copy of the same field bytes."""
+    job = bench.Job("c5", 0, 0)
+    ids = np.arange(0, job.n, 2048)
+    gpu = _gpu_outputs(job, torch, ids)
+    _invariants(job, torch, 8000, 64, 1024)
+    data = job.data.cpu().numpy()                                            # the same bytes
+    g = oracle.grid(data, (1024, 1024, 1024), (0, 0, 0), (1, 1, 1))
+    ref = oracle.streamlines(g, job.seeds_h[ids], oracle.params(**job.w["prm"]), "f32")
+    _compare(gpu, ref, "c5")
+    tot = job.totals_o.cpu().numpy()
+    print("C5 attempts %d accepted %d samples %d" % (tot[0], tot[1], tot[2]))
