@@ -63,26 +63,45 @@ void timing_end(cudaStream_t st) {
 
 static bool finite_pos(float x) { return std::isfinite(x) && x > 0.0f; }
 
-// Build the library-owned copy of one packed float3 array with `nvert` vertices.
-static int repack(const float* src, unsigned long long nvert, unsigned nx, int layout, void** out,
-                  size_t* bytes) {
+// Records of the library-owned copy of a stored box of nx*ny*nz vertices x nslices.
+static unsigned long long layout_records(int layout, unsigned nx, unsigned ny, unsigned nz, unsigned nslices) {
+  if (layout == LAYOUT_CELL) return (unsigned long long)(nx - 1) * (ny - 1) * (nz - 1) * nslices;
+  return (unsigned long long)nx * ny * nz * nslices;
+}
+static size_t layout_record_bytes(int layout) {
+  return layout == LAYOUT_FLOAT4 ? 16 : (layout == LAYOUT_XPAIR ? 32 : (layout == LAYOUT_CELL ? 128 : 12));
+}
+
+// Build the library-owned copy of one packed float3 array (stored box nx*ny*nz, nslices slices).
+static int repack(const float* src, unsigned nx, unsigned ny, unsigned nz, unsigned nslices, int layout,
+                  void** out, size_t* bytes) {
   *out = nullptr; *bytes = 0;
   if (layout == LAYOUT_PACKED3) { *out = const_cast<float*>(src); return STREAMI_OK; }
-  size_t rec = layout == LAYOUT_FLOAT4 ? 16 : 32;
+  const unsigned long long nvert = (unsigned long long)nx * ny * nz * nslices;
+  const unsigned long long nrec = layout_records(layout, nx, ny, nz, nslices);
+  const size_t rec = layout_record_bytes(layout);
   void* dst = nullptr;
-  STREAMI_TRY(cudaMalloc(&dst, rec * nvert + 32));   // +32: FLOAT4 reads p[1] of the last vertex
+  STREAMI_TRY(cudaMalloc(&dst, rec * nrec + 32));   // +32: FLOAT4 reads p[1] of the last vertex
   int blocks = 148 * 8;
   if (layout == LAYOUT_FLOAT4)
     repack_float4_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert);
-  else
+  else if (layout == LAYOUT_XPAIR)
     repack_xpair_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert, nx);
+  else
+    repack_cell_kernel<<<blocks, 256>>>(src, (float4*)dst, nx, ny, nz, nslices);
   launch_counter()++;
   cudaError_t e = cudaGetLastError();
-  if (e == cudaSuccess) e = cudaMemset((char*)dst + rec * nvert, 0, 32);
+  if (e == cudaSuccess) e = cudaMemset((char*)dst + rec * nrec, 0, 32);
   if (e == cudaSuccess) e = cudaStreamSynchronize(0);
   if (e != cudaSuccess) { cudaFree(dst); return check(e); }
-  *out = dst; *bytes = rec * nvert + 32;
+  *out = dst; *bytes = rec * nrec + 32;
   return STREAMI_OK;
+}
+
+// LAYOUT_CELL addresses cells, not vertices: the strides of the store become those of the cell grid.
+static void cell_strides(Store& s, unsigned nx, unsigned ny, unsigned nz) {
+  s.nx = nx - 1; s.nxy = (nx - 1) * (ny - 1);
+  s.slice_stride = (unsigned long long)(nx - 1) * (ny - 1) * (nz - 1);
 }
 
 static int fill_geom(Geom& g, const int dims[3], const float origin[3], const float spacing[3],
@@ -105,7 +124,8 @@ static int fill_geom(Geom& g, const int dims[3], const float origin[3], const fl
 
 static int pick_layout(int hint) {
   if (hint == STREAMI_LAYOUT_AUTO) return LAYOUT_XPAIR;   // measured fastest
-  if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR)
+  if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR ||
+      hint == STREAMI_LAYOUT_CELL)
     return hint;
   return -1;
 }
@@ -135,8 +155,9 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
-  rc = repack(dev_ptr, s.slice_stride * (unsigned long long)nslices, s.nx, layout, &data, &bytes);
+  rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
   if (rc) { delete f; return rc; }
+  if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
   s.data = data;
   if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
   *out = f;
@@ -192,8 +213,11 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
         s.nxy = s.nx * (unsigned)(hi[1] - lo[1] + 1);
         s.slice_stride = (unsigned long long)s.nxy * (unsigned)(hi[2] - lo[2] + 1);
         void* data = nullptr; size_t bytes = 0;
-        rc = repack(src, s.slice_stride, s.nx, layout, &data, &bytes);
+        const unsigned bnx = (unsigned)(hi[0] - lo[0] + 1), bny = (unsigned)(hi[1] - lo[1] + 1),
+                       bnz = (unsigned)(hi[2] - lo[2] + 1);
+        rc = repack(src, bnx, bny, bnz, 1u, layout, &data, &bytes);
         if (rc) return fail(rc);
+        if (layout == LAYOUT_CELL) cell_strides(s, bnx, bny, bnz);
         s.data = data;
         if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
         f->bricks.push_back(s);
@@ -238,7 +262,9 @@ int streami_sample(streami_field f, const float* points, size_t n, float t, int 
     case LAYOUT_FLOAT4 * 2: GO(LAYOUT_FLOAT4, false); break;
     case LAYOUT_FLOAT4 * 2 + 1: GO(LAYOUT_FLOAT4, true); break;
     case LAYOUT_XPAIR * 2: GO(LAYOUT_XPAIR, false); break;
-    default: GO(LAYOUT_XPAIR, true); break;
+    case LAYOUT_XPAIR * 2 + 1: GO(LAYOUT_XPAIR, true); break;
+    case LAYOUT_CELL * 2: GO(LAYOUT_CELL, false); break;
+    default: GO(LAYOUT_CELL, true); break;
   }
 #undef GO
   STREAMI_LAUNCHED();

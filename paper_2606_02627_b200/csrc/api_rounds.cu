@@ -10,7 +10,8 @@
 
 namespace streami {
 typedef void (*TraceKernel)(const TraceArgs);
-TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache);
+TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache, bool unit);
+bool unit_geometry(const Geom& g);
 int trace_grid(TraceKernel k, unsigned long long nwork, int* grid);
 int check_params(const streami_params* p, bool need_capacity);
 void fill_integrator(TraceArgs& a, const streami_params* p);
@@ -20,6 +21,7 @@ static StreakKernel pick_streak(int layout, bool unsteady) {
   switch (layout) {
     case LAYOUT_PACKED3: return unsteady ? streak_kernel<LAYOUT_PACKED3, true> : streak_kernel<LAYOUT_PACKED3, false>;
     case LAYOUT_FLOAT4: return unsteady ? streak_kernel<LAYOUT_FLOAT4, true> : streak_kernel<LAYOUT_FLOAT4, false>;
+    case LAYOUT_CELL: return unsteady ? streak_kernel<LAYOUT_CELL, true> : streak_kernel<LAYOUT_CELL, false>;
     default: return unsteady ? streak_kernel<LAYOUT_XPAIR, true> : streak_kernel<LAYOUT_XPAIR, false>;
   }
 }
@@ -102,7 +104,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   if (n == 0) return check(cudaStreamSynchronize(st));
 
   const bool cache = options().cell_cache != 0;
-  TraceKernel k = pick_trace_kernel(f->layout, 0, false, true, cache);
+  TraceKernel k = pick_trace_kernel(f->layout, 0, false, true, cache, unit_geometry(f->g));
 
   // scratch: [next u64][log count u64][qcount u32][pad u32][row0: nb x u32], two queues of n records
   const size_t ctr_bytes = 24 + sizeof(unsigned) * (size_t)nb;

@@ -11,20 +11,31 @@ namespace streami {
 
 typedef void (*TraceKernel)(const TraceArgs);
 
-template <int L>
-static TraceKernel pick_l(int integ, bool unsteady, bool brick, bool cache) {
-  if (brick) return cache ? trace_kernel<L, 0, false, true, true> : trace_kernel<L, 0, false, true, false>;
-  if (unsteady) return integ ? trace_kernel<L, 1, true, false, false> : trace_kernel<L, 0, true, false, false>;
-  if (integ) return cache ? trace_kernel<L, 1, false, false, true> : trace_kernel<L, 1, false, false, false>;
-  return cache ? trace_kernel<L, 0, false, false, true> : trace_kernel<L, 0, false, false, false>;
+template <int L, bool U>
+static TraceKernel pick_lu(int integ, bool brick, bool cache) {      // steady
+  if (brick) return cache ? trace_kernel<L, 0, false, true, true, U> : trace_kernel<L, 0, false, true, false, U>;
+  if (integ) return cache ? trace_kernel<L, 1, false, false, true, U> : trace_kernel<L, 1, false, false, false, U>;
+  return cache ? trace_kernel<L, 0, false, false, true, U> : trace_kernel<L, 0, false, false, false, U>;
 }
 
-TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache) {
+template <int L>
+static TraceKernel pick_l(int integ, bool unsteady, bool brick, bool cache, bool unit) {
+  if (unsteady) return integ ? trace_kernel<L, 1, true, false, false, false> : trace_kernel<L, 0, true, false, false, false>;
+  return unit ? pick_lu<L, true>(integ, brick, cache) : pick_lu<L, false>(integ, brick, cache);
+}
+
+// unit = the grid is its own index space (origin 0, spacing 1): see index_pos in field.cuh.
+TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache, bool unit) {
   switch (layout) {
-    case LAYOUT_PACKED3: return pick_l<LAYOUT_PACKED3>(integ, unsteady, brick, cache);
-    case LAYOUT_FLOAT4: return pick_l<LAYOUT_FLOAT4>(integ, unsteady, brick, cache);
-    default: return pick_l<LAYOUT_XPAIR>(integ, unsteady, brick, cache);
+    case LAYOUT_PACKED3: return pick_l<LAYOUT_PACKED3>(integ, unsteady, brick, cache, unit);
+    case LAYOUT_FLOAT4: return pick_l<LAYOUT_FLOAT4>(integ, unsteady, brick, cache, unit);
+    case LAYOUT_CELL: return pick_l<LAYOUT_CELL>(integ, unsteady, brick, cache, unit);
+    default: return pick_l<LAYOUT_XPAIR>(integ, unsteady, brick, cache, unit);
   }
+}
+
+bool unit_geometry(const Geom& g) {
+  return g.ox == 0.0f && g.oy == 0.0f && g.oz == 0.0f && g.rx == 1.0f && g.ry == 1.0f && g.rz == 1.0f;
 }
 
 // Persistent grid: as many blocks as are resident at once (a multiple of the SM count).
@@ -111,7 +122,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
 
   const bool unsteady = f->g.nslices > 1;
   const bool cache = options().cell_cache && !unsteady;
-  TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache);
+  TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache, unit_geometry(f->g));
   int grid = 0;
   rc = trace_grid(k, n, &grid);
   if (rc) return rc;

@@ -53,12 +53,12 @@ __device__ __forceinline__ float rp10(float x) {
 }
 
 #define STREAMI_S(PX, PY, PZ, T, KX, KY, KZ)                                                   \
-  rc = sample<LAYOUT, UNSTEADY, false, CACHE>(a.g, s, cc, PX, PY, PZ, T, KX, KY, KZ);          \
+  rc = sample<LAYOUT, UNSTEADY, false, CACHE, UNIT>(a.g, s, cc, PX, PY, PZ, T, KX, KY, KZ);    \
   n_samples++;                                                                                 \
   if (rc) return rc;
 
 // One DP5(4) attempt.  L.k1 holds k1 (FSAL).  Returns 0 to continue, else the final status.
-template <int LAYOUT, bool UNSTEADY, bool CACHE>
+template <int LAYOUT, bool UNSTEADY, bool CACHE, bool UNIT>
 __device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store& s, CellCache& cc,
                                                 Lane& L, unsigned& n_samples, unsigned& n_attempts) {
   if (L.n == a.max_steps) return ST_MAXSTEPS;
@@ -93,7 +93,7 @@ __device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store&
   const float nx = __fmaf_rn(h, ax, px), ny = __fmaf_rn(h, ay, py), nz = __fmaf_rn(h, az, pz);
   {
     float gx, gy, gz;
-    if (!to_index(a.g, nx, ny, nz, gx, gy, gz)) return ST_OUT;
+    if (!to_index<UNIT>(a.g, nx, ny, nz, gx, gy, gz)) return ST_OUT;
   }
   STREAMI_S(nx, ny, nz, t + h, k7x, k7y, k7z)
   // error vector, scale, RMS norm (squared)

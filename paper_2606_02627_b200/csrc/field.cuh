@@ -12,7 +12,7 @@
 
 namespace streami {
 
-enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3 };
+enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3, LAYOUT_CELL = 4 };
 enum : unsigned { ST_ALIVE = 0, ST_OUT = 1, ST_MAXSTEPS = 2, ST_STAGNANT = 3, ST_HALO = 4 };
 
 // Global geometry (A1), uniform over the launch.
@@ -31,8 +31,8 @@ struct Store {
   int lox, loy, loz;       // stored box, global vertex indices, inclusive
   int hix, hiy, hiz;
   int topflagx, topflagy, topflagz;  // 1 where hi == N-1 (g == hi is then served too)
-  unsigned nx, nxy;        // row and plane strides in vertices
-  unsigned long long slice_stride;   // vertices per slice
+  unsigned nx, nxy;        // row and plane strides in records (vertices; LAYOUT_CELL: cells)
+  unsigned long long slice_stride;   // records per slice
 };
 
 // A brick grid (A9): owner of an in-domain position.
@@ -74,12 +74,49 @@ template <> struct CellLoad<LAYOUT_XPAIR> {
   }
 };
 
+// LAYOUT_CELL: one aligned 128-byte record per CELL = the four XPAIR rows of that cell back to
+// back, i.e. all 8 corner vertices in ONE L2 line / one contiguous DRAM access.  Random 32-byte
+// sector gathers top out near 1.7 TB/s on B200 and contiguous 128-byte ones near 5.4 TB/s
+// (DESIGN.md section 6), which is what this layout buys with 8x the memory.
+template <> struct CellLoad<LAYOUT_CELL> {
+  static __device__ __forceinline__ void cell(const void* data, unsigned long long c, float* V) {
+    const char* p = reinterpret_cast<const char*>(data) + 128ull * c;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      float p6, p7;
+      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=f"(V[6 * r]), "=f"(V[6 * r + 1]), "=f"(V[6 * r + 2]), "=f"(V[6 * r + 3]),
+                     "=f"(V[6 * r + 4]), "=f"(V[6 * r + 5]), "=f"(p6), "=f"(p7)
+                   : "l"(p + 32 * r));
+      (void)p6; (void)p7;
+    }
+  }
+};
+
 template <int LAYOUT>
 __device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, float* V) {
-  CellLoad<LAYOUT>::row(s.data, v, V);
-  CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
-  CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
-  CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+  if constexpr (LAYOUT == LAYOUT_CELL) {
+    CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+  } else {
+    CellLoad<LAYOUT>::row(s.data, v, V);
+    CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
+    CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+  }
+}
+
+// A steady store holds fewer than 2^32 vertices (checked at create time), so the four row
+// indices fit 32 bits (v + nxy + nx <= nvert - 1) and each address is one 32x32->64 multiply-add.
+template <int LAYOUT>
+__device__ __forceinline__ void load_cell32(const Store& s, unsigned v, float* V) {
+  if constexpr (LAYOUT == LAYOUT_CELL) {
+    CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+  } else {
+    CellLoad<LAYOUT>::row(s.data, v, V);
+    CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
+    CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+  }
 }
 
 // A2.5: x first, then y, then z; 7 lerps per component.
@@ -102,17 +139,29 @@ __device__ __forceinline__ void interp_cell(const float* V, float fx, float fy, 
 // Register-resident copy of the current cell (build's choice: a sample that stays in the cell of
 // the previous one costs no loads; the arithmetic, hence the result, is unchanged).
 struct CellCache {
-  unsigned long long key;
+  unsigned key;                  // vertex index of the cell's low corner inside the current store
   float V[24];
-  __device__ __forceinline__ void invalidate() { key = ~0ull; }
+  __device__ __forceinline__ void invalidate() { key = 0xffffffffu; }   // never a low corner
 };
 
 // A2.1 + A2.2: index-space position and the closed-box test (NaN -> false).
-__device__ __forceinline__ bool to_index(const Geom& g, float px, float py, float pz, float& gx,
-                                         float& gy, float& gz) {
-  gx = (px - g.ox) * g.rx; gy = (py - g.oy) * g.ry; gz = (pz - g.oz) * g.rz;
+// UNIT = the grid is its own index space (origin 0, spacing 1, hence r = 1): (p - 0.0f) * 1.0f
+// returns p bit for bit, so the two operations are skipped.  C2, C3 and C5 are such grids.
+template <bool UNIT>
+__device__ __forceinline__ void index_pos(const Geom& g, float px, float py, float pz, float& gx,
+                                          float& gy, float& gz) {
+  if (UNIT) { gx = px; gy = py; gz = pz; }
+  else { gx = (px - g.ox) * g.rx; gy = (py - g.oy) * g.ry; gz = (pz - g.oz) * g.rz; }
+}
+__device__ __forceinline__ bool in_domain(const Geom& g, float gx, float gy, float gz) {
   return (gx >= 0.0f && gx <= g.topx) && (gy >= 0.0f && gy <= g.topy) &&
          (gz >= 0.0f && gz <= g.topz);
+}
+template <bool UNIT = false>
+__device__ __forceinline__ bool to_index(const Geom& g, float px, float py, float pz, float& gx,
+                                         float& gy, float& gz) {
+  index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
+  return in_domain(g, gx, gy, gz);
 }
 
 // Cell location inside one store.  Returns false (HALO_MISS) if the store cannot serve g.
@@ -146,12 +195,15 @@ __device__ __forceinline__ int time_slice(const Geom& g, float t, float& a, bool
 }
 
 // Full sample S(p, t) (A2/A3, brick form A9).  Returns 0 ok, ST_OUT or ST_HALO.
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE>
+// KNOWN: the caller has already established that p is inside the domain (it passed the A5.5 test
+// at the end of the previous step, or the A5.1 test at the seed), so the test is not repeated.
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT = false, bool KNOWN = false>
 __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCache& cc, float px,
                                            float py, float pz, float t, float& vx, float& vy,
                                            float& vz) {
   float gx, gy, gz;
-  if (!to_index(g, px, py, pz, gx, gy, gz)) return ST_OUT;
+  index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
+  if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
   unsigned long long v; float fx, fy, fz;
   if (!locate<BRICK>(s, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
   if (UNSTEADY) {
@@ -169,20 +221,23 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
       vx = lerp(ux, wx, a); vy = lerp(uy, wy, a); vz = lerp(uz, wz, a);   // space first, time last
     } else { vx = ux; vy = uy; vz = uz; }
   } else if (CACHE) {
-    if (v != cc.key) { load_cell<LAYOUT>(s, v, cc.V); cc.key = v; }
+    const unsigned v32 = (unsigned)v;
+    if (v32 != cc.key) { load_cell32<LAYOUT>(s, v32, cc.V); cc.key = v32; }
     interp_cell(cc.V, fx, fy, fz, vx, vy, vz);
   } else {
     float V[24];
-    load_cell<LAYOUT>(s, v, V);
+    load_cell32<LAYOUT>(s, (unsigned)v, V);
     interp_cell(V, fx, fy, fz, vx, vy, vz);
   }
   return 0;
 }
 
 // A9: owner brick of an in-domain position (destinationID).
+template <bool UNIT = false>
 __device__ __forceinline__ int owner_of(const Geom& g, const BrickMap& m, float px, float py,
                                         float pz) {
-  float gx = (px - g.ox) * g.rx, gy = (py - g.oy) * g.ry, gz = (pz - g.oz) * g.rz;
+  float gx, gy, gz;
+  index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
   int bx = min(__float2int_rd(gx) / m.Bx, m.nbx - 1);
   int by = min(__float2int_rd(gy) / m.By, m.nby - 1);
   int bz = min(__float2int_rd(gz) / m.Bz, m.nbz - 1);

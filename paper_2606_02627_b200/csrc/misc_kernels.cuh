@@ -29,6 +29,29 @@ static __global__ void repack_xpair_kernel(const float* __restrict__ src, float4
   }
 }
 
+// CELL record c = the four XPAIR rows (dz*2+dy) of cell c back to back: 128 bytes, 8 corners.
+// One thread per (cell, row): 6 source floats in, 32 bytes out; consecutive threads write
+// consecutive 32-byte pieces.
+static __global__ void repack_cell_kernel(const float* __restrict__ src, float4* __restrict__ dst,
+                                          unsigned nx, unsigned ny, unsigned nz, unsigned nslices) {
+  const unsigned cx = nx - 1, cy = ny - 1, cz = nz - 1;
+  const unsigned long long per_slice = (unsigned long long)cx * cy * cz;
+  const unsigned long long total = 4ull * per_slice * nslices;
+  unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; t < total; t += step) {
+    const unsigned r = (unsigned)(t & 3ull);
+    unsigned long long c = t >> 2;
+    const unsigned sl = (unsigned)(c / per_slice);
+    c -= (unsigned long long)sl * per_slice;
+    const unsigned ix = (unsigned)(c % cx), iy = (unsigned)((c / cx) % cy), iz = (unsigned)(c / ((unsigned long long)cx * cy));
+    const unsigned long long v = (((unsigned long long)sl * nz + iz + (r >> 1)) * ny + iy + (r & 1u)) * nx + ix;
+    const float* p = src + 3ull * v;
+    dst[2 * t] = make_float4(p[0], p[1], p[2], p[3]);
+    dst[2 * t + 1] = make_float4(p[4], p[5], 0.0f, 0.0f);
+  }
+}
+
 // ---- a2-a4 alone ----------------------------------------------------------------------------
 template <int LAYOUT, bool UNSTEADY>
 __global__ void sample_kernel(Geom g, Store s, const float* __restrict__ pts, unsigned long long n,
@@ -88,12 +111,15 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
       Lane L; L.px = px; L.py = py; L.pz = pz; L.id = 0; L.slot = 0; L.rec_cd = 0xffffffffu;
       CellCache cc; cc.invalidate();
       unsigned n_samples = 0, n_attempts = 0;
+      const unsigned s_first = s;
       for (; s < a.s1; ++s) {
         L.n = s;                                                 // t_s = t0 + (float)s*h, shared by all
         ta.t0 = a.t0;
-        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false>(ta, a.s, cc, L, n_samples, n_attempts);
-        if (rc) { st = rc; break; }
+        unsigned done;
+        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false, false>(ta, a.s, cc, L, done);
+        if (rc) { st = rc; n_attempts = done >= 2u ? 1u : 0u; n_samples = min(done, 4u); break; }
       }
+      n_attempts += s - s_first; n_samples += 4u * (s - s_first);
       if (st == ST_ALIVE && a.s1 >= a.nsteps) st = ST_MAXSTEPS;  // alive at the end
       px = L.px; py = L.py; pz = L.pz;
       atomicAdd(&s_tot[0], (unsigned long long)n_attempts);

@@ -70,37 +70,42 @@ __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
 }
 
 // ---- A4 + A5 steps 2-6: one RK4 step.  Returns 0 to continue, else the final status. -------
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE>
+// `done` = field samples taken in this call (0..4); the caller derives its counters from it:
+// a call that returns 0 took 4 samples and is one attempt; a call that ends the particle took
+// `done` samples and is an attempt iff done >= 2 or the new position left the domain (A5.3
+// comes before the attempt is counted).  The stage-1 sample does not repeat the domain test:
+// p passed it at the end of the previous step (A5.5) or at the seed (A5.1).
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
 __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CellCache& cc,
-                                             Lane& L, unsigned& n_samples, unsigned& n_attempts) {
+                                             Lane& L, unsigned& done) {
+  done = 0;
   if (L.n == a.max_steps) return ST_MAXSTEPS;                                   // A5.2
   float tn = 0.0f;
   if (UNSTEADY) tn = a.t0 + (float)L.n * a.h;                                   // A4, not accumulated
   float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z;
-  unsigned rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, L.px, L.py, L.pz, tn, k1x, k1y, k1z);
-  n_samples++;
-  if (rc) return rc;
+  unsigned rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT, true>(a.g, s, cc, L.px, L.py, L.pz, tn, k1x, k1y, k1z);
+  done = 1;
+  if (BRICK) { if (rc) return rc; }
   float m = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));                // A5.3
   if (m < a.vmin2) return ST_STAGNANT;
-  n_attempts++;
   float qx = __fmaf_rn(a.h2, k1x, L.px), qy = __fmaf_rn(a.h2, k1y, L.py), qz = __fmaf_rn(a.h2, k1z, L.pz);
-  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h2, k2x, k2y, k2z);
-  n_samples++;
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a.g, s, cc, qx, qy, qz, tn + a.h2, k2x, k2y, k2z);
+  done = 2;
   if (rc) return rc;
   qx = __fmaf_rn(a.h2, k2x, L.px); qy = __fmaf_rn(a.h2, k2y, L.py); qz = __fmaf_rn(a.h2, k2z, L.pz);
-  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h2, k3x, k3y, k3z);
-  n_samples++;
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a.g, s, cc, qx, qy, qz, tn + a.h2, k3x, k3y, k3z);
+  done = 3;
   if (rc) return rc;
   qx = __fmaf_rn(a.h, k3x, L.px); qy = __fmaf_rn(a.h, k3y, L.py); qz = __fmaf_rn(a.h, k3z, L.pz);
-  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE>(a.g, s, cc, qx, qy, qz, tn + a.h, k4x, k4y, k4z);
-  n_samples++;
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a.g, s, cc, qx, qy, qz, tn + a.h, k4x, k4y, k4z);
+  done = 4;
   if (rc) return rc;
   float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
   float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
   float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
   float nx = __fmaf_rn(a.h6, sx, L.px), ny = __fmaf_rn(a.h6, sy, L.py), nz = __fmaf_rn(a.h6, sz, L.pz);
   float gx, gy, gz;
-  if (!to_index(a.g, nx, ny, nz, gx, gy, gz)) return ST_OUT;                    // A5.5: not recorded
+  if (!to_index<UNIT>(a.g, nx, ny, nz, gx, gy, gz)) { done = 5; return ST_OUT; }  // A5.5: not recorded
   L.px = nx; L.py = ny; L.pz = nz; L.n++;                                       // A5.6
   record_vertex(a, L);
   return 0;

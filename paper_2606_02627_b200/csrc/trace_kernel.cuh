@@ -35,7 +35,7 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, const Lane& L,
   }
 }
 
-template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE>
+template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
 __global__ void __launch_bounds__(TRACE_BLOCK)
 trace_kernel(const TraceArgs a) {
   __shared__ unsigned long long s_tot[4];
@@ -81,13 +81,13 @@ trace_kernel(const TraceArgs a) {
           active = true;
           if (fresh) {
             float gx, gy, gz;
-            if (!to_index(a.g, L.px, L.py, L.pz, gx, gy, gz)) {                 // A5.1
+            if (!to_index<UNIT>(a.g, L.px, L.py, L.pz, gx, gy, gz)) {                 // A5.1
               finish_particle(a, L, ST_OUT);
               active = false;
             } else {
               record_vertex(a, L);                                              // vertex 0 = seed
               if (BRICK) {
-                my_brick = owner_of(a.g, a.bm, L.px, L.py, L.pz);
+                my_brick = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
                 if (a.rc_this) atomicAdd(a.rc_this + my_brick, 1u);
               }
             }
@@ -97,7 +97,7 @@ trace_kernel(const TraceArgs a) {
             cc.invalidate();
             if (INTEG == 1) {
               L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false;
-              unsigned rc = sample<LAYOUT, UNSTEADY, false, CACHE>(a.g, st, cc, L.px, L.py, L.pz, L.t,
+              unsigned rc = sample<LAYOUT, UNSTEADY, false, CACHE, UNIT, true>(a.g, st, cc, L.px, L.py, L.pz, L.t,
                                                                    L.k1x, L.k1y, L.k1z);
               n_samples++;
               if (rc) { finish_particle(a, L, rc); active = false; atomicAdd(&s_tot[2], 1ull); }
@@ -113,16 +113,20 @@ trace_kernel(const TraceArgs a) {
     // ---- a2-a8: one step (RK4) or one attempt (DP5(4)) --------------------------------------
     bool emit = false; int dest = 0;
     if (active) {
-      unsigned rc;
-      if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE>(a, st, cc, L, n_samples, n_attempts);
-      else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE>(a, st, cc, L, n_samples, n_attempts);
+      unsigned rc, done = 0;
+      if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, done);
+      else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE, UNIT>(a, st, cc, L, n_samples, n_attempts);
       if (BRICK && rc == 0) {                                                   // a8: owner of p_new
-        dest = owner_of(a.g, a.bm, L.px, L.py, L.pz);
-        if (dest != my_brick) rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF;
+        dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
+        if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; }
       }
       if (rc) {
         active = false;
         if (rc == RC_HANDOFF) emit = true; else finish_particle(a, L, rc);
+        if (INTEG == 0) {                       // RK4 counters are derived (see rk4_step)
+          n_attempts = (L.n - n_start) + (done >= 2u ? 1u : 0u);
+          n_samples = 4u * (L.n - n_start) + min(done, 4u);
+        }
         atomicAdd(&s_tot[0], (unsigned long long)n_attempts);
         atomicAdd(&s_tot[1], (unsigned long long)(L.n - n_start));
         atomicAdd(&s_tot[2], (unsigned long long)n_samples);

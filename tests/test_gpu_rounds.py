@@ -39,7 +39,7 @@ def gpu_streaklines(S, torch, field, pts, nsteps, **kw):
             totals.cpu().numpy().astype(np.uint64))
 
 
-@pytest.mark.parametrize("layout", [1, 2, 3])
+@pytest.mark.parametrize("layout", [1, 2, 3, 4])
 @pytest.mark.parametrize("window", [0, 1, 7])
 def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window):
     """A scaled-down config 4: double gyre slices, rake + a few points that leave or start outside."""
@@ -114,7 +114,7 @@ def gpu_bricks(S, torch, wl, fld, nb, seeds, ghost=1, layout=0, max_rounds=64, l
 
 
 @pytest.mark.parametrize("nb,N,layout", [((2, 2, 2), 32, 3), ((2, 2, 2), 32, 1), ((3, 2, 1), 31, 2),
-                                         ((1, 1, 1), 24, 3)])
+                                         ((1, 1, 1), 24, 3), ((2, 2, 2), 32, 4), ((3, 2, 1), 31, 4)])
 def test_bricks_vs_oracle_and_monolithic(S, torch, oracle, wl, nb, N, layout):
     fld = wl.turb_field_cpu(N, 48, 1, 6)
     n = 30011
