@@ -11,7 +11,7 @@
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0, 0}; return o; }
+Options& options() { static Options o{1, 1, 0, 0, 0, 1}; return o; }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -278,6 +278,8 @@ int streami_set_option(const char* name, int value) {
   else if (!strcmp(name, "presort")) o.presort = value != 0;
   else if (!strcmp(name, "streak_window")) o.streak_window = value < 0 ? 0 : value;
   else if (!strcmp(name, "kernel_timing")) o.kernel_timing = value != 0;
+  else if (!strcmp(name, "segment_steps")) o.segment_steps = value < 0 ? 0 : value;
+  else if (!strcmp(name, "vertex_staging")) o.vertex_staging = value != 0;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }
@@ -289,6 +291,8 @@ int streami_get_option(const char* name, int* value) {
   else if (!strcmp(name, "presort")) *value = o.presort;
   else if (!strcmp(name, "streak_window")) *value = o.streak_window;
   else if (!strcmp(name, "kernel_timing")) *value = o.kernel_timing;
+  else if (!strcmp(name, "segment_steps")) *value = o.segment_steps;
+  else if (!strcmp(name, "vertex_staging")) *value = o.vertex_staging;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }

@@ -124,9 +124,10 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
   a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = nb;
-  a.seeds = seeds; a.perm = nullptr; a.next = d_next;
+  a.seeds = seeds; a.perm = nullptr; a.next = d_next; a.nwork_dev = nullptr; a.seg_budget = 0;
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
   a.qout_count = d_qcount;
   a.log = out_handoff_log; a.log_cap = log_capacity; a.log_count = d_logc;
 
@@ -136,7 +137,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   std::vector<unsigned> h_buf(1 + nb);
   for (;;) {
     a.round = (int)round; a.nwork = nwork;
-    a.qin = q[round & 1]; a.qout = q[(round + 1) & 1];
+    a.qin = round ? q[round & 1] : nullptr; a.qout = q[(round + 1) & 1];
     a.rc_this = nullptr; a.rc_next = nullptr;
     if (round == 0) {
       a.rc_this = out_round_counts ? out_round_counts : d_row0;

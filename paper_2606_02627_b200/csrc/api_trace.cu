@@ -69,39 +69,48 @@ void fill_integrator(TraceArgs& a, const streami_params* p) {
   a.h = p->h; a.h2 = 0.5f * p->h; a.h6 = p->h / 6.0f;        // A4: computed once, fp32
   a.hmin = p->h_min; a.hmax = p->h_max; a.atol = p->atol; a.rtol = p->rtol;
   a.vmin2 = p->vmin * p->vmin; a.t0 = p->t0; a.max_steps = p->max_steps;
-  a.cap = p->capacity; a.stride = p->stride;
+  a.cap = p->capacity; a.stride = p->stride; a.vec_ok = 0; a.staging = options().vertex_staging;
   a.steps = p->out_steps; a.status = p->out_status; a.fin = p->out_final; a.totals = p->out_totals;
 }
 
-// Morton presort (a12): fills perm[n]; scratch is freed on the stream.
-int presort_seeds(const streami_field_s* f, const float* seeds, size_t n, unsigned* perm,
-                  cudaStream_t st) {
-  int maxdim = std::max(f->dims[0], std::max(f->dims[1], f->dims[2]));
-  int shift = 2;                                   // 4^3-cell blocks, at most 128 blocks per axis
-  while (((maxdim - 1) >> shift) >= 128) shift++;
-  unsigned bits = 0;
-  while ((1u << bits) <= (unsigned)((maxdim - 1) >> shift)) bits++;
-  unsigned nbins = 1u << (3 * bits);
-  const unsigned nseg = (nbins + PRESORT_SEG - 1) / PRESORT_SEG;
-  unsigned* hist = nullptr; unsigned* keys = nullptr;   // hist: [nbins] counts + [nseg] totals
-  STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * ((size_t)nbins + nseg), st));
-  cudaError_t e = cudaMallocAsync((void**)&keys, sizeof(unsigned) * n, st);
-  if (e != cudaSuccess) { cudaFreeAsync(hist, st); return check(e); }
-  int rc = STREAMI_OK;
-  unsigned blocks = (unsigned)((n + 255) / 256);
-  e = cudaMemsetAsync(hist, 0, sizeof(unsigned) * nbins, st);
-  if (e == cudaSuccess) {
-    presort_hist_kernel<<<blocks, 256, 0, st>>>(f->g, shift, seeds, n, hist, keys);
+// Morton sort of work items (a12): a counting sort by the Morton code of the item's coarse cell
+// block.  Scratch is allocated once per trace call and reused by every segment.
+struct MortonSorter {
+  int shift; unsigned nbins, nseg;
+  unsigned* hist; unsigned* keys; size_t cap;
+  cudaStream_t st;
+
+  int init(const streami_field_s* f, size_t n, cudaStream_t stream) {
+    st = stream; cap = n; hist = nullptr; keys = nullptr;
+    int maxdim = std::max(f->dims[0], std::max(f->dims[1], f->dims[2]));
+    shift = 2;                                     // 4^3-cell blocks, at most 128 blocks per axis
+    while (((maxdim - 1) >> shift) >= 128) shift++;
+    unsigned bits = 0;
+    while ((1u << bits) <= (unsigned)((maxdim - 1) >> shift)) bits++;
+    nbins = 1u << (3 * bits);
+    nseg = (nbins + PRESORT_SEG - 1) / PRESORT_SEG;
+    STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * ((size_t)nbins + nseg), st));   // counts + totals
+    cudaError_t e = cudaMallocAsync((void**)&keys, sizeof(unsigned) * n, st);
+    if (e != cudaSuccess) { cudaFreeAsync(hist, st); hist = nullptr; return check(e); }
+    return STREAMI_OK;
+  }
+  void release() { if (hist) cudaFreeAsync(hist, st); if (keys) cudaFreeAsync(keys, st); hist = keys = nullptr; }
+
+  // perm[0..count) = the items ordered by bin; count = n, or *n_dev (<= cap) when n_dev is set.
+  int sort(const Geom& g, const float* pos, unsigned stride_floats, size_t n, const unsigned* n_dev,
+           unsigned* perm) {
+    STREAMI_TRY(cudaMemsetAsync(hist, 0, sizeof(unsigned) * nbins, st));
+    size_t items = n_dev ? cap : n;
+    unsigned blocks = (unsigned)std::min<size_t>((items + 255) / 256, (size_t)num_sms() * 16);
+    if (blocks == 0) blocks = 1;
+    presort_hist_kernel<<<blocks, 256, 0, st>>>(g, shift, pos, stride_floats, n, n_dev, hist, keys);
     presort_scan_seg_kernel<<<nseg, 256, 0, st>>>(hist, nbins, hist + nbins);
     presort_scan_top_kernel<<<1, 1024, 0, st>>>(hist + nbins, nseg);
-    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, hist + nbins, perm);
+    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, n_dev, hist, hist + nbins, perm);
     launch_counter() += 4;
-    e = cudaGetLastError();
+    return check(cudaGetLastError());
   }
-  if (e != cudaSuccess) rc = check(e);
-  cudaFreeAsync(hist, st); cudaFreeAsync(keys, st);
-  return rc;
-}
+};
 
 }  // namespace streami
 
@@ -127,30 +136,84 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   rc = trace_grid(k, n, &grid);
   if (rc) return rc;
 
-  unsigned long long* next = nullptr;
-  STREAMI_TRY(cudaMallocAsync((void**)&next, sizeof(unsigned long long), st));
-  unsigned* perm = nullptr;
-  auto cleanup = [&]() { cudaFreeAsync(next, st); if (perm) cudaFreeAsync(perm, st); };
-  cudaError_t e = cudaMemsetAsync(next, 0, sizeof(unsigned long long), st);
+  // Segments: K step attempts per particle per launch, Morton re-sort of the survivors between
+  // launches (trace_kernel.cuh).  K = 0, or a trace too short or too small to need it: one launch.
+  const bool sorting = options().presort && n >= 65536;
+  unsigned K = (unsigned)options().segment_steps;
+  if (!sorting || K >= params->max_steps) K = 0;
+  const bool dp5 = params->integrator == 1;
+
+  // scratch: [0] work counter u64, [8] queue counts u32 x 2
+  char* ctr = nullptr;
+  STREAMI_TRY(cudaMallocAsync((void**)&ctr, 16, st));
+  unsigned long long* next = (unsigned long long*)ctr;
+  unsigned* qcount = (unsigned*)(ctr + 8);
+  unsigned* perm = nullptr; QRec* q[2] = {nullptr, nullptr};
+  MortonSorter sorter{}; bool have_sorter = false;
+  auto cleanup = [&]() {
+    cudaFreeAsync(ctr, st);
+    if (perm) cudaFreeAsync(perm, st);
+    if (q[0]) cudaFreeAsync(q[0], st);
+    if (q[1]) cudaFreeAsync(q[1], st);
+    if (have_sorter) sorter.release();
+  };
+  cudaError_t e = cudaMemsetAsync(ctr, 0, 16, st);
+  if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+  if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
+  if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
   if (e != cudaSuccess) { cleanup(); return check(e); }
-  if (options().presort && n >= 65536) {
-    e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
-    if (e != cudaSuccess) { perm = nullptr; cleanup(); return check(e); }
-    rc = presort_seeds(f, seeds, n, perm, st);
+  if (sorting) {
+    rc = sorter.init(f, n, st);
+    if (rc) { cleanup(); return rc; }
+    have_sorter = true;
+    rc = sorter.sort(f->g, seeds, 3, n, nullptr, perm);
     if (rc) { cleanup(); return rc; }
   }
 
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
   a.bricks = nullptr; a.nbricks = 0;
-  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.next = next; a.round = 0;
+  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr; a.next = next; a.round = 0;
+  a.seg_budget = K;
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
+  a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
   timing_begin(st);
   k<<<grid, TRACE_BLOCK, 0, st>>>(a);
   timing_end(st);
   launch_counter()++;
   e = cudaGetLastError();
+
+  if (K && e == cudaSuccess) {
+    // RK4: a particle takes exactly K steps per segment, so ceil(max_steps / K) launches finish
+    // everything and no count has to come back to the host (the call stays asynchronous; a launch
+    // whose queue is empty exits at once).  DP5(4): rejected attempts spend budget too, so the live
+    // count is read back every few segments (this synchronises the stream).
+    const unsigned planned = (params->max_steps + K - 1) / K;
+    for (unsigned r = 1; e == cudaSuccess; ++r) {
+      if (!dp5 && r >= planned) break;
+      const unsigned in = (r - 1) & 1u, out = r & 1u;
+      if (dp5 && (r % 4u) == 0u) {
+        unsigned live = 0;
+        e = cudaMemcpyAsync(&live, qcount + in, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess || live == 0) break;
+      }
+      e = cudaMemsetAsync(qcount + out, 0, sizeof(unsigned), st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(next, 0, sizeof(unsigned long long), st);
+      if (e != cudaSuccess) break;
+      rc = sorter.sort(f->g, (const float*)q[in], 8, 0, qcount + in, perm);
+      if (rc) { cleanup(); return rc; }
+      a.seeds = nullptr; a.qin = q[in]; a.nwork_dev = qcount + in; a.qout = q[out]; a.qout_count = qcount + out;
+      a.round = (int)r;
+      timing_begin(st);
+      k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+      timing_end(st);
+      launch_counter()++;
+      e = cudaGetLastError();
+    }
+  }
   cleanup();
   return check(e);
 }

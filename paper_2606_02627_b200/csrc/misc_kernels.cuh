@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
         L.n = s;                                                 // t_s = t0 + (float)s*h, shared by all
         ta.t0 = a.t0;
         unsigned done;
-        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false, false>(ta, a.s, cc, L, done);
+        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false, false, false>(ta, a.s, cc, L, done);
         if (rc) { st = rc; n_attempts = done >= 2u ? 1u : 0u; n_samples = min(done, 4u); break; }
       }
       n_attempts += s - s_first; n_samples += 4u * (s - s_first);

@@ -18,23 +18,29 @@ __device__ __forceinline__ unsigned spread3(unsigned x) {   // 10 bits -> every 
   return x;
 }
 
-__device__ __forceinline__ unsigned seed_bin(const Geom& g, int shift, const float* seeds,
+// Positions are read with a stride in floats: 3 for the seed array, 8 for queue records.
+__device__ __forceinline__ unsigned seed_bin(const Geom& g, int shift, const float* pos, unsigned stride,
                                              unsigned long long i) {
   float gx, gy, gz;
-  if (!to_index(g, seeds[3 * i], seeds[3 * i + 1], seeds[3 * i + 2], gx, gy, gz)) return 0u;
+  const float* p = pos + (unsigned long long)stride * i;
+  if (!to_index(g, p[0], p[1], p[2], gx, gy, gz)) return 0u;
   unsigned bx = (unsigned)__float2int_rz(gx) >> shift, by = (unsigned)__float2int_rz(gy) >> shift,
            bz = (unsigned)__float2int_rz(gz) >> shift;
   return spread3(bx) | (spread3(by) << 1) | (spread3(bz) << 2);
 }
 
-static __global__ void presort_hist_kernel(Geom g, int shift, const float* __restrict__ seeds,
-                                    unsigned long long n, unsigned* __restrict__ hist,
-                                    unsigned* __restrict__ keys) {
+// The item count is `n`, or *n_dev when n_dev is set (a queue whose size only the device knows).
+static __global__ void presort_hist_kernel(Geom g, int shift, const float* __restrict__ pos, unsigned stride,
+                                    unsigned long long n, const unsigned* __restrict__ n_dev,
+                                    unsigned* __restrict__ hist, unsigned* __restrict__ keys) {
+  if (n_dev) n = *n_dev;
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  unsigned k = seed_bin(g, shift, seeds, i);
-  keys[i] = k;
-  atomicAdd(hist + k, 1u);
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; i < n; i += step) {
+    unsigned k = seed_bin(g, shift, pos, stride, i);
+    keys[i] = k;
+    atomicAdd(hist + k, 1u);
+  }
 }
 
 // Exclusive scan of `hist` in two levels.  Level 1: each block scans one segment of 1024 bins in
@@ -90,14 +96,18 @@ presort_scan_top_kernel(unsigned* __restrict__ seg_total, unsigned nseg) {
 }
 
 static __global__ void presort_scatter_kernel(const unsigned* __restrict__ keys, unsigned long long n,
+                                       const unsigned* __restrict__ n_dev,
                                        unsigned* __restrict__ offsets,
                                        const unsigned* __restrict__ seg_base,
                                        unsigned* __restrict__ perm) {
+  if (n_dev) n = *n_dev;
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const unsigned k = keys[i];
-  unsigned pos = atomicAdd(offsets + k, 1u) + seg_base[k / PRESORT_SEG];
-  perm[pos] = (unsigned)i;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; i < n; i += step) {
+    const unsigned k = keys[i];
+    unsigned pos = atomicAdd(offsets + k, 1u) + seg_base[k / PRESORT_SEG];
+    perm[pos] = (unsigned)i;
+  }
 }
 
 }  // namespace streami

@@ -13,8 +13,9 @@
 
 namespace streami {
 
-// hand-off record: what a particle carries to another brick (position + unique id, PAPER.md:69;
-// plus its step count).  32 bytes, read and written as two 16-byte accesses.
+// hand-off record: what a particle carries to another brick or into the next segment (position +
+// unique id; plus its step count; DP5(4): t and h as bits in pad0/pad1).  32 bytes,
+// read and written as two 16-byte accesses.
 struct __align__(16) QRec {
   float px, py, pz; unsigned id;
   unsigned n; unsigned brick; unsigned pad0, pad1;
@@ -26,9 +27,11 @@ struct TraceArgs {
   const Store* bricks; BrickMap bm; int nbricks;   // brick mode
   // work
   const float* seeds;              // [n][3]
-  const unsigned* perm;            // optional processing order of seeds (presort), or NULL
-  const QRec* qin;                 // brick rounds >= 1
+  const unsigned* perm;            // optional processing order of the work items (Morton sort), or NULL
+  const QRec* qin;                 // work = queue records (brick rounds >= 1, segments >= 1), else seeds
   unsigned long long nwork;
+  const unsigned* nwork_dev;       // if set, the work count is read from device memory instead
+  unsigned seg_budget;             // step attempts per particle per launch, 0 = unlimited
   unsigned long long* next;        // global work counter
   int round;
   // integrator (host-computed fp32 constants, A4/A8)
@@ -36,6 +39,8 @@ struct TraceArgs {
   unsigned max_steps;
   // outputs (A6)
   float* verts; unsigned long long n; unsigned cap, stride;
+  int vec_ok;                      // capacity % 8 == 0 and verts 32-byte aligned: full-sector vertex stores
+  int staging;                     // 1 = stage vertices in shared memory (default), 0 = store each directly
   unsigned* counts; unsigned* steps; unsigned* status; float* fin;
   unsigned long long* totals;      // [4]
   // brick outputs
@@ -51,20 +56,73 @@ struct Lane {
   float px, py, pz;
   unsigned id, n;
   unsigned slot, rec_cd;           // next vertex slot, steps until the next recorded vertex
+  unsigned stage0;                 // first slot held in the shared-memory staging group (<= slot)
   // DP5(4) only
   float t, h, k1x, k1y, k1z; bool rejected;
 };
 
+// a7, the output writer.  A vertex is 3 x 4 bytes into three planes; written one at a time each
+// store dirties 4 bytes of a 32-byte sector that is evicted long before the particle's next vertex
+// arrives (measured on C2: 6.6 GB of DRAM writes plus read-modify-write reads for 1.3 GB of
+// vertices, 13-24 % of the kernel).  So vertices are staged per lane in shared memory, 8 slots per
+// plane, and written as ONE full 32-byte sector per plane when the group of 8 is complete; a
+// partial group (at termination, at a hand-off, or for a capacity that is not a multiple of 8)
+// goes out with scalar stores.  Slots beyond the count stay untouched (A6).
+constexpr int REC_GROUP = 8;
+constexpr int REC_THREADS = 256;
+__device__ __forceinline__ float* rec_stage() {
+  __shared__ float s_rec[3 * REC_GROUP * REC_THREADS];        // [plane][slot & 7][thread]
+  return s_rec + threadIdx.x;
+}
+
+__device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
+  const unsigned cnt = L.slot - L.stage0;
+  if (cnt != 0u && a.verts) {
+    const float* s = rec_stage();
+    const unsigned long long plane = a.n * a.cap;
+    float* dst = a.verts + (unsigned long long)L.id * a.cap + L.stage0;
+    if (cnt == (unsigned)REC_GROUP && a.vec_ok) {               // stage0 is then a multiple of 8
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float* sc = s + c * REC_GROUP * REC_THREADS;
+        asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst + c * plane),
+                     "f"(sc[0]), "f"(sc[REC_THREADS]), "f"(sc[2 * REC_THREADS]), "f"(sc[3 * REC_THREADS]),
+                     "f"(sc[4 * REC_THREADS]), "f"(sc[5 * REC_THREADS]), "f"(sc[6 * REC_THREADS]),
+                     "f"(sc[7 * REC_THREADS])
+                     : "memory");
+      }
+    } else {
+      const unsigned j0 = L.stage0 & (REC_GROUP - 1);
+      for (unsigned j = 0; j < cnt; ++j) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) dst[c * plane + j] = s[(c * REC_GROUP + j0 + j) * REC_THREADS];
+      }
+    }
+  }
+  L.stage0 = L.slot;
+}
+
+template <bool REC = true>
 __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
+  if (!REC) return;
   if (--L.rec_cd == 0) {
     L.rec_cd = a.stride;
     if (L.slot < a.cap) {
-      if (a.verts) {
-        unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
-        unsigned long long plane = a.n * a.cap;
-        a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
+      if (!a.staging) {                          // option "vertex_staging" = 0 (for A/B measurement)
+        if (a.verts) {
+          unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
+          unsigned long long plane = a.n * a.cap;
+          a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
+        }
+        L.slot++; L.stage0 = L.slot;
+      } else {
+        if (a.verts) {
+          float* s = rec_stage() + (L.slot & (REC_GROUP - 1)) * REC_THREADS;
+          s[0] = L.px; s[REC_GROUP * REC_THREADS] = L.py; s[2 * REC_GROUP * REC_THREADS] = L.pz;
+        }
+        L.slot++;
+        if ((L.slot & (REC_GROUP - 1)) == 0u) flush_vertices(a, L);
       }
-      L.slot++;
     }
   }
 }
@@ -75,7 +133,7 @@ __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
 // `done` samples and is an attempt iff done >= 2 or the new position left the domain (A5.3
 // comes before the attempt is counted).  The stage-1 sample does not repeat the domain test:
 // p passed it at the end of the previous step (A5.5) or at the seed (A5.1).
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool REC = true>
 __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CellCache& cc,
                                              Lane& L, unsigned& done) {
   done = 0;
@@ -107,7 +165,7 @@ __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s,
   float gx, gy, gz;
   if (!to_index<UNIT>(a.g, nx, ny, nz, gx, gy, gz)) { done = 5; return ST_OUT; }  // A5.5: not recorded
   L.px = nx; L.py = ny; L.pz = nz; L.n++;                                       // A5.6
-  record_vertex(a, L);
+  record_vertex<REC>(a, L);
   return 0;
 }
 

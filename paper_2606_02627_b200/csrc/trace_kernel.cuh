@@ -1,4 +1,12 @@
 // csrc/trace_kernel.cuh -- the persistent advection kernel: refill, step, terminate / hand off.
+//
+// Segments (the build's choice, a12 of SURVEY.md 8(a); not in the paper).  A launch may give every
+// particle a budget of `seg_budget` step attempts; a particle that is still alive when its budget
+// is spent is appended to the out queue exactly like a brick leaver, the host re-sorts the queue
+// by Morton cell block and launches the next segment.  The lanes that run at the same time then
+// work in the same region of the field at ALL times of the trace, not only at the seeds: their
+// gathers share TLB entries, DRAM pages and L2 lines.  It is a schedule only: a particle's
+// arithmetic does not depend on where its trajectory is cut, and every output is indexed by id.
 #pragma once
 #include "dp5.cuh"
 
@@ -6,18 +14,23 @@ namespace streami {
 
 constexpr int TRACE_BLOCK = 256;
 
-__device__ __forceinline__ void finish_particle(const TraceArgs& a, const Lane& L, unsigned st) {
+__device__ __forceinline__ void finish_particle(const TraceArgs& a, Lane& L, unsigned st) {
+  flush_vertices(a, L);
   if (a.counts) a.counts[L.id] = L.slot;
   if (a.steps) a.steps[L.id] = L.n;
   if (a.status) a.status[L.id] = st;
   if (a.fin) { a.fin[L.id] = L.px; a.fin[a.n + L.id] = L.py; a.fin[2 * a.n + L.id] = L.pz; }
 }
 
-// a9: append a brick leaver to the next round's queue (the device-side stand-in for
-// emitOutgoing + forward): one atomic per warp for the slot range.
-__device__ __forceinline__ void emit_outgoing(const TraceArgs& a, const Lane& L, int dest, bool emit) {
+// a9: append a particle to the next launch's queue: a brick leaver (the device-side stand-in for
+// emitOutgoing + forward) or a particle whose segment budget is spent.
+// One atomic per warp for the slot range.  `handoff` = it changes brick (counted and logged, A9).
+template <int INTEG>
+__device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int dest, bool emit,
+                                              bool handoff) {
   unsigned mask = __ballot_sync(__activemask(), emit);
   if (!emit) return;
+  flush_vertices(a, L);
   int lane = threadIdx.x & 31;
   int leader = __ffs(mask) - 1;
   unsigned base = 0;
@@ -26,17 +39,24 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, const Lane& L,
   unsigned pos = base + __popc(mask & ((1u << lane) - 1u));
   QRec r; r.px = L.px; r.py = L.py; r.pz = L.pz; r.id = L.id; r.n = L.n; r.brick = (unsigned)dest;
   r.pad0 = 0; r.pad1 = 0;
+  if (INTEG == 1) { r.pad0 = __float_as_uint(L.t); r.pad1 = __float_as_uint(L.h); }
   a.qout[pos] = r;
-  if (a.rc_next) atomicAdd(a.rc_next + dest, 1u);
-  if (a.log_count) {
-    unsigned long long k = atomicAdd(a.log_count, 1ull);
-    if (a.log && k < a.log_cap)
-      a.log[k] = ((unsigned long long)(a.round + 1) << 48) | ((unsigned long long)dest << 32) | L.id;
+  if (handoff) {
+    if (a.rc_next) atomicAdd(a.rc_next + dest, 1u);
+    if (a.log_count) {
+      unsigned long long k = atomicAdd(a.log_count, 1ull);
+      if (a.log && k < a.log_cap)
+        a.log[k] = ((unsigned long long)(a.round + 1) << 48) | ((unsigned long long)dest << 32) | L.id;
+    }
   }
 }
 
+// Resident blocks per SM the compiler must allow for.  3 blocks of 256 (<= 80 registers): capping
+// the steady RK4 kernel at 64 registers for a 4th block was measured on C2 and lost to its spills.
+constexpr int trace_min_blocks(int integ, bool unsteady, bool brick) { return 3; }
+
 template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
-__global__ void __launch_bounds__(TRACE_BLOCK)
+__global__ void __launch_bounds__(TRACE_BLOCK, trace_min_blocks(INTEG, UNSTEADY, BRICK))
 trace_kernel(const TraceArgs a) {
   __shared__ unsigned long long s_tot[4];
   if (threadIdx.x < 4) s_tot[threadIdx.x] = 0ull;
@@ -44,12 +64,13 @@ trace_kernel(const TraceArgs a) {
 
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xffffffffu;
+  const unsigned long long nwork = a.nwork_dev ? (unsigned long long)*a.nwork_dev : a.nwork;
   Lane L; L.rejected = false;
   CellCache cc; cc.invalidate();
   Store st = a.s;                 // brick mode: replaced per particle
   int my_brick = 0;
   bool active = false, exhausted = false;
-  unsigned n_samples = 0, n_attempts = 0, n_start = 0;
+  unsigned n_samples = 0, n_attempts = 0, n_start = 0, budget = 0;
 
   for (;;) {
     // ---- a1: refill idle lanes from the global work counter --------------------------------
@@ -61,27 +82,32 @@ trace_kernel(const TraceArgs a) {
       base = __shfl_sync(FULL, base, leader);
       if (!active && !exhausted) {
         unsigned long long w = base + __popc(need & ((1u << lane) - 1u));
-        if (w >= a.nwork) {
+        if (w >= nwork) {
           exhausted = true;
         } else {
           n_samples = 0; n_attempts = 0;
+          budget = a.seg_budget;
+          const unsigned src = a.perm ? a.perm[w] : (unsigned)w;
           bool fresh = true;
-          if (BRICK && a.round > 0) {
-            const QRec r = a.qin[w];
+          if (a.qin) {                                        // a continued or handed-over particle
+            const QRec r = a.qin[src];
             L.px = r.px; L.py = r.py; L.pz = r.pz; L.id = r.id; L.n = r.n; my_brick = (int)r.brick;
+            if (INTEG == 1) { L.t = __uint_as_float(r.pad0); L.h = __uint_as_float(r.pad1); L.rejected = false; }
             L.slot = min(a.cap, L.n / a.stride + 1u);
             L.rec_cd = a.stride - L.n % a.stride;
+            L.stage0 = L.slot;
             fresh = false;
           } else {
-            L.id = a.perm ? a.perm[w] : (unsigned)w;
+            L.id = src;
             L.px = a.seeds[3ull * L.id]; L.py = a.seeds[3ull * L.id + 1]; L.pz = a.seeds[3ull * L.id + 2];
-            L.n = 0; L.slot = 0; L.rec_cd = 1;
+            L.n = 0; L.slot = 0; L.rec_cd = 1; L.stage0 = 0;
+            if (INTEG == 1) { L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false; }
           }
           n_start = L.n;
           active = true;
           if (fresh) {
             float gx, gy, gz;
-            if (!to_index<UNIT>(a.g, L.px, L.py, L.pz, gx, gy, gz)) {                 // A5.1
+            if (!to_index<UNIT>(a.g, L.px, L.py, L.pz, gx, gy, gz)) {           // A5.1
               finish_particle(a, L, ST_OUT);
               active = false;
             } else {
@@ -96,10 +122,11 @@ trace_kernel(const TraceArgs a) {
             if (BRICK) { st = a.bricks[my_brick]; }
             cc.invalidate();
             if (INTEG == 1) {
-              L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false;
+              // k1 of the first attempt.  For a continued particle this recomputes the FSAL value
+              // S(p, t) it carried (same operands, same operations), so it is not counted again.
               unsigned rc = sample<LAYOUT, UNSTEADY, false, CACHE, UNIT, true>(a.g, st, cc, L.px, L.py, L.pz, L.t,
-                                                                   L.k1x, L.k1y, L.k1z);
-              n_samples++;
+                                                                               L.k1x, L.k1y, L.k1z);
+              if (fresh) n_samples++;
               if (rc) { finish_particle(a, L, rc); active = false; atomicAdd(&s_tot[2], 1ull); }
             }
           }
@@ -111,14 +138,19 @@ trace_kernel(const TraceArgs a) {
       continue;
     }
     // ---- a2-a8: one step (RK4) or one attempt (DP5(4)) --------------------------------------
-    bool emit = false; int dest = 0;
+    bool emit = false, handoff = false; int dest = my_brick;
     if (active) {
       unsigned rc, done = 0;
       if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, done);
       else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE, UNIT>(a, st, cc, L, n_samples, n_attempts);
       if (BRICK && rc == 0) {                                                   // a8: owner of p_new
         dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
-        if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; }
+        if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; handoff = rc == RC_HANDOFF; }
+      }
+      if (rc == 0 && --budget == 0u) {                                          // segment budget spent
+        // (seg_budget == 0 wraps to 2^32-1: no segments.)  A rejected DP5(4) attempt must retry
+        // with the flag it carries, so the cut waits for the next accepted step.
+        if (INTEG == 1 && L.rejected) budget = 1u; else { rc = RC_HANDOFF; done = 0; }
       }
       if (rc) {
         active = false;
@@ -130,12 +162,12 @@ trace_kernel(const TraceArgs a) {
         atomicAdd(&s_tot[0], (unsigned long long)n_attempts);
         atomicAdd(&s_tot[1], (unsigned long long)(L.n - n_start));
         atomicAdd(&s_tot[2], (unsigned long long)n_samples);
-        if (emit) atomicAdd(&s_tot[3], 1ull);
+        if (handoff) atomicAdd(&s_tot[3], 1ull);
       }
     }
-    if (BRICK) {
+    if (a.qout) {
       unsigned any = __ballot_sync(FULL, emit);
-      if (any) emit_outgoing(a, L, dest, emit);
+      if (any) emit_outgoing<INTEG>(a, L, dest, emit, handoff);
     }
   }
   __syncthreads();
