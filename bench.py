@@ -49,6 +49,10 @@ WORKLOADS = {
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
                stride=128)),
+    # L2-resident variant of C2 (same step size and seed count, 64^3 field): isolates the instruction
+    # stream from the DRAM gathers when reading profiles (never a reported number)
+    "c2s": dict(kind="turb", N=64, M=64, kmax=16, n=1 << 20, prm=dict(integrator=0, h=0.25,
+                max_steps=2000, vmin=1e-6, capacity=256, stride=8)),
     # reduced sizes for quick checks of this script itself (never a reported number)
     "tiny": dict(kind="turb", N=48, M=32, kmax=8, n=4096, prm=dict(integrator=0, h=0.25,
                  max_steps=500, vmin=1e-6, capacity=64, stride=8)),
@@ -59,6 +63,7 @@ DESCR = {
     "c3": "C3 turbulence 512^3 in 2x2x2 bricks (ghost 1), 4,194,304 seeds, RK4 h=0.25, max 4,000",
     "c4": "C4 double gyre 256x128x64 x 64 slices, 4,096-point rake, 1,000 steps, streaklines",
     "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
+    "c2s": "C2 with an L2-resident 64^3 field (profiling aid only)",
     "tiny": "tiny turbulence 48^3 (script self-check only)",
 }
 
