@@ -6,6 +6,7 @@
 
 #include "internal.h"
 #include "misc_kernels.cuh"
+#include "sorter.cuh"
 #include "trace_kernel.cuh"
 
 namespace streami {
@@ -112,7 +113,14 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   STREAMI_TRY(cudaMallocAsync((void**)&ctr, ctr_bytes, st));
   cudaError_t e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
   if (e == cudaSuccess) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
-  auto cleanup = [&]() { cudaFreeAsync(ctr, st); if (q[0]) cudaFreeAsync(q[0], st); if (q[1]) cudaFreeAsync(q[1], st); };
+  unsigned* perm = nullptr; MortonSorter sorter{}; bool have_sorter = false;
+  const bool sorting = options().presort && n >= 65536;
+  auto cleanup = [&]() {
+    cudaFreeAsync(ctr, st); if (q[0]) cudaFreeAsync(q[0], st); if (q[1]) cudaFreeAsync(q[1], st);
+    if (perm) cudaFreeAsync(perm, st);
+    if (have_sorter) sorter.release();
+  };
+  if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
   if (e != cudaSuccess) { if (e != cudaSuccess && !q[0]) q[0] = nullptr; cleanup(); return check(e); }
   unsigned long long* d_next = (unsigned long long*)ctr;
   unsigned long long* d_logc = out_log_count ? out_log_count : (unsigned long long*)(ctr + 8);
@@ -131,6 +139,11 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   a.qout_count = d_qcount;
   a.log = out_handoff_log; a.log_cap = log_capacity; a.log_count = d_logc;
 
+  if (sorting) {            // a12: each round's work is processed in Morton order of its positions
+    rc = sorter.init(f, n, st);
+    if (rc) { cleanup(); return rc; }
+    have_sorter = true;
+  }
   bool truncated = false;
   unsigned round = 0;
   unsigned long long nwork = n;
@@ -138,6 +151,13 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   for (;;) {
     a.round = (int)round; a.nwork = nwork;
     a.qin = round ? q[round & 1] : nullptr; a.qout = q[(round + 1) & 1];
+    a.perm = nullptr;
+    if (sorting && nwork >= 65536) {
+      rc = round ? sorter.sort(f->g, (const float*)q[round & 1], 8, nwork, nullptr, perm)
+                 : sorter.sort(f->g, seeds, 3, nwork, nullptr, perm);
+      if (rc) { cleanup(); return rc; }
+      a.perm = perm;
+    }
     a.rc_this = nullptr; a.rc_next = nullptr;
     if (round == 0) {
       a.rc_this = out_round_counts ? out_round_counts : d_row0;

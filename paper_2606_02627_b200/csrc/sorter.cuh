@@ -1,0 +1,50 @@
+// csrc/sorter.cuh -- host driver of the Morton counting sort (a12), shared by the streamline and
+// the brick round loops.
+#pragma once
+#include <algorithm>
+
+#include "internal.h"
+#include "presort.cuh"
+
+namespace streami {
+
+// Morton sort of work items (a12): a counting sort by the Morton code of the item's coarse cell
+// block.  Scratch is allocated once per trace call and reused by every segment.
+struct MortonSorter {
+  int shift; unsigned nbins, nseg;
+  unsigned* hist; unsigned* keys; size_t cap;
+  cudaStream_t st;
+
+  int init(const streami_field_s* f, size_t n, cudaStream_t stream) {
+    st = stream; cap = n; hist = nullptr; keys = nullptr;
+    int maxdim = std::max(f->dims[0], std::max(f->dims[1], f->dims[2]));
+    shift = 2;                                     // 4^3-cell blocks, at most 128 blocks per axis
+    while (((maxdim - 1) >> shift) >= 128) shift++;
+    unsigned bits = 0;
+    while ((1u << bits) <= (unsigned)((maxdim - 1) >> shift)) bits++;
+    nbins = 1u << (3 * bits);
+    nseg = (nbins + PRESORT_SEG - 1) / PRESORT_SEG;
+    STREAMI_TRY(cudaMallocAsync((void**)&hist, sizeof(unsigned) * ((size_t)nbins + nseg), st));   // counts + totals
+    cudaError_t e = cudaMallocAsync((void**)&keys, sizeof(unsigned) * n, st);
+    if (e != cudaSuccess) { cudaFreeAsync(hist, st); hist = nullptr; return check(e); }
+    return STREAMI_OK;
+  }
+  void release() { if (hist) cudaFreeAsync(hist, st); if (keys) cudaFreeAsync(keys, st); hist = keys = nullptr; }
+
+  // perm[0..count) = the items ordered by bin; count = n, or *n_dev (<= cap) when n_dev is set.
+  int sort(const Geom& g, const float* pos, unsigned stride_floats, size_t n, const unsigned* n_dev,
+           unsigned* perm) {
+    STREAMI_TRY(cudaMemsetAsync(hist, 0, sizeof(unsigned) * nbins, st));
+    size_t items = n_dev ? cap : n;
+    unsigned blocks = (unsigned)std::min<size_t>((items + 255) / 256, (size_t)num_sms() * 16);
+    if (blocks == 0) blocks = 1;
+    presort_hist_kernel<<<blocks, 256, 0, st>>>(g, shift, pos, stride_floats, n, n_dev, hist, keys);
+    presort_scan_seg_kernel<<<nseg, 256, 0, st>>>(hist, nbins, hist + nbins);
+    presort_scan_top_kernel<<<1, 1024, 0, st>>>(hist + nbins, nseg);
+    presort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, n_dev, hist, hist + nbins, perm);
+    launch_counter() += 4;
+    return check(cudaGetLastError());
+  }
+};
+
+}  // namespace streami
