@@ -2,6 +2,7 @@
 // responsible for data handling"), layout repack, options, streami_sample.
 #include <cmath>
 #include <cstring>
+#include <limits>
 #include <mutex>
 #include <utility>
 #include <vector>
@@ -209,6 +210,18 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
         s.hix = hi[0]; s.hiy = hi[1]; s.hiz = hi[2];
         s.topflagx = hi[0] == global_dims[0] - 1; s.topflagy = hi[1] == global_dims[1] - 1;
         s.topflagz = hi[2] == global_dims[2] - 1;
+        {
+          const float inf = std::numeric_limits<float>::infinity();
+          s.flox = (float)lo[0]; s.floy = (float)lo[1]; s.floz = (float)lo[2];
+          s.fhix = s.topflagx ? inf : (float)hi[0]; s.fhiy = s.topflagy ? inf : (float)hi[1];
+          s.fhiz = s.topflagz ? inf : (float)hi[2];
+          int ol[3], oh[3];
+          for (int a = 0; a < 3; ++a) {
+            ol[a] = B[a] * b[a];
+            oh[a] = (b[a] == brick_grid[a] - 1) ? std::numeric_limits<int>::max() : B[a] * (b[a] + 1);
+          }
+          s.olox = ol[0]; s.oloy = ol[1]; s.oloz = ol[2]; s.ohix = oh[0]; s.ohiy = oh[1]; s.ohiz = oh[2];
+        }
         s.nx = (unsigned)(hi[0] - lo[0] + 1);
         s.nxy = s.nx * (unsigned)(hi[1] - lo[1] + 1);
         s.slice_stride = (unsigned long long)s.nxy * (unsigned)(hi[2] - lo[2] + 1);

@@ -31,6 +31,12 @@ struct Store {
   int lox, loy, loz;       // stored box, global vertex indices, inclusive
   int hix, hiy, hiz;
   int topflagx, topflagy, topflagz;  // 1 where hi == N-1 (g == hi is then served too)
+  // A9 serve test lo <= g < hi as floats, computed once: fhi = +inf where hi == N-1, because there
+  // g <= hi is what the domain test has already established.
+  float flox, floy, floz, fhix, fhiy, fhiz;
+  // owned cell box of the brick [olo, ohi) in global cell indices (ohi = INT_MAX on the top brick of
+  // an axis): floor(g) inside it <=> owner(g) == this brick, without the integer divisions of A9.
+  int olox, oloy, oloz, ohix, ohiy, ohiz;
   unsigned nx, nxy;        // row and plane strides in records (vertices; LAYOUT_CELL: cells)
   unsigned long long slice_stride;   // records per slice
 };
@@ -169,10 +175,9 @@ __device__ __forceinline__ bool to_index(const Geom& g, float px, float py, floa
 template <bool BRICK>
 __device__ __forceinline__ bool locate(const Store& s, float gx, float gy, float gz,
                                        unsigned long long& v, float& fx, float& fy, float& fz) {
-  if (BRICK) {
-    bool in = (gx >= (float)s.lox) && (gx < (float)s.hix || (s.topflagx && gx <= (float)s.hix)) &&
-              (gy >= (float)s.loy) && (gy < (float)s.hiy || (s.topflagy && gy <= (float)s.hiy)) &&
-              (gz >= (float)s.loz) && (gz < (float)s.hiz || (s.topflagz && gz <= (float)s.hiz));
+  if (BRICK) {           // the caller has passed the domain test, so g <= N-1 already holds
+    bool in = (gx >= s.flox) && (gx < s.fhix) && (gy >= s.floy) && (gy < s.fhiy) &&
+              (gz >= s.floz) && (gz < s.fhiz);
     if (!in) return false;
   }
   int ix = min(__float2int_rz(gx), s.hix - 1);
@@ -233,6 +238,15 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
 }
 
 // A9: owner brick of an in-domain position (destinationID).
+// Same brick as before?  floor(g) per axis inside the owned box (g >= 0 here: truncation = floor).
+template <bool UNIT = false>
+__device__ __forceinline__ bool still_owned(const Geom& g, const Store& s, float px, float py, float pz) {
+  float gx, gy, gz;
+  index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
+  const int ix = __float2int_rz(gx), iy = __float2int_rz(gy), iz = __float2int_rz(gz);
+  return ix >= s.olox && ix < s.ohix && iy >= s.oloy && iy < s.ohiy && iz >= s.oloz && iz < s.ohiz;
+}
+
 template <bool UNIT = false>
 __device__ __forceinline__ int owner_of(const Geom& g, const BrickMap& m, float px, float py,
                                         float pz) {

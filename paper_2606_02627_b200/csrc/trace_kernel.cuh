@@ -144,7 +144,7 @@ trace_kernel(const TraceArgs a) {
       if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, done);
       else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE, UNIT>(a, st, cc, L, n_samples, n_attempts);
       if (BRICK && rc == 0) {                                                   // a8: owner of p_new
-        dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
+        if (!still_owned<UNIT>(a.g, st, L.px, L.py, L.pz)) dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
         if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; handoff = rc == RC_HANDOFF; }
       }
       if (rc == 0 && --budget == 0u) {                                          // segment budget spent
