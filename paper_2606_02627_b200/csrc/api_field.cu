@@ -153,6 +153,7 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.lox = s.loy = s.loz = 0;
   s.hix = dims[0] - 1; s.hiy = dims[1] - 1; s.hiz = dims[2] - 1;
   s.topflagx = s.topflagy = s.topflagz = 1;
+  s.cmx = s.hix - 1; s.cmy = s.hiy - 1; s.cmz = s.hiz - 1;
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
@@ -208,6 +209,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
         Store s;
         s.lox = lo[0]; s.loy = lo[1]; s.loz = lo[2];
         s.hix = hi[0]; s.hiy = hi[1]; s.hiz = hi[2];
+        s.cmx = hi[0] - 1; s.cmy = hi[1] - 1; s.cmz = hi[2] - 1;
         s.topflagx = hi[0] == global_dims[0] - 1; s.topflagy = hi[1] == global_dims[1] - 1;
         s.topflagz = hi[2] == global_dims[2] - 1;
         {

@@ -30,6 +30,7 @@ struct Store {
   const void* data;        // layout-specific records, x fastest
   int lox, loy, loz;       // stored box, global vertex indices, inclusive
   int hix, hiy, hiz;
+  int cmx, cmy, cmz;       // hi - 1: the last cell per axis (A2.3 clamp), precomputed
   int topflagx, topflagy, topflagz;  // 1 where hi == N-1 (g == hi is then served too)
   // A9 serve test lo <= g < hi as floats, computed once: fhi = +inf where hi == N-1, because there
   // g <= hi is what the domain test has already established.
@@ -191,12 +192,13 @@ __device__ __forceinline__ bool locate(const Store& s, float gx, float gy, float
               (gz >= s.floz) && (gz < s.fhiz);
     if (!in) return false;
   }
-  int ix = min(__float2int_rz(gx), s.hix - 1);
-  int iy = min(__float2int_rz(gy), s.hiy - 1);
-  int iz = min(__float2int_rz(gz), s.hiz - 1);
+  int ix = min(__float2int_rz(gx), s.cmx);
+  int iy = min(__float2int_rz(gy), s.cmy);
+  int iz = min(__float2int_rz(gz), s.cmz);
   fx = gx - (float)ix; fy = gy - (float)iy; fz = gz - (float)iz;
-  v = (unsigned long long)(unsigned)(iz - s.loz) * s.nxy + (unsigned)(iy - s.loy) * s.nx +
-      (unsigned)(ix - s.lox);
+  if (BRICK) { ix -= s.lox; iy -= s.loy; iz -= s.loz; }   // a monolithic store starts at 0
+  // fewer than 2^32 records per slice (checked at create time): 32-bit arithmetic is exact
+  v = (unsigned long long)((unsigned)iz * s.nxy + (unsigned)iy * s.nx + (unsigned)ix);
   return true;
 }
 
