@@ -70,6 +70,7 @@ void fill_integrator(TraceArgs& a, const streami_params* p) {
   a.hmin = p->h_min; a.hmax = p->h_max; a.atol = p->atol; a.rtol = p->rtol;
   a.vmin2 = p->vmin * p->vmin; a.t0 = p->t0; a.max_steps = p->max_steps;
   a.cap = p->capacity; a.stride = p->stride; a.vec_ok = 0; a.staging = options().vertex_staging;
+  a.prefetch = options().prefetch;
   a.steps = p->out_steps; a.status = p->out_status; a.fin = p->out_final; a.totals = p->out_totals;
 }
 

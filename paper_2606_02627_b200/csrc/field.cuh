@@ -250,6 +250,50 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
   return 0;
 }
 
+// ---- one-step-ahead cell prefetch (build's choice; results unchanged) ------------------------
+// The first touch of a new cell stalls the whole warp for an L2/DRAM round trip, and it happens
+// mid-step (stage 2 or 4), where the lane has nothing else to do.  At the END of a step the next
+// step's stage points are known to ~1 % of a cell (p_new + 0.5 d and p_new + d with
+// d = p_new - p), so the cells they fall in are requested then, a whole warp-iteration early.
+// The request is a 4-byte cp.async (LDGSTS, .ca: allocates in L1) per 32-byte sector into a
+// scratch word of shared memory that is never read: no destination registers, nothing to wait on.
+__device__ __forceinline__ void prefetch_sector(const void* gptr, unsigned smem_addr) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+
+template <int LAYOUT>
+__device__ __forceinline__ void prefetch_cell32(const Store& s, unsigned v, unsigned smem_addr) {
+  if constexpr (LAYOUT == LAYOUT_CELL) {
+    const char* p = reinterpret_cast<const char*>(s.data) + 128ull * v;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) prefetch_sector(p + 32 * r, smem_addr);
+  } else {
+    constexpr unsigned long long REC = LAYOUT == LAYOUT_XPAIR ? 32ull : (LAYOUT == LAYOUT_FLOAT4 ? 16ull : 12ull);
+    const char* p = reinterpret_cast<const char*>(s.data);
+    prefetch_sector(p + REC * v, smem_addr);
+    prefetch_sector(p + REC * (v + s.nx), smem_addr);
+    prefetch_sector(p + REC * (v + s.nxy), smem_addr);
+    prefetch_sector(p + REC * (v + s.nxy + s.nx), smem_addr);
+  }
+}
+
+// Cell (record index inside the store) that holds index-space position g, clamped into the store
+// so that the address is always valid (a prediction may point anywhere; NaN converts to 0).
+template <bool BRICK>
+__device__ __forceinline__ unsigned clamped_cell(const Store& s, float gx, float gy, float gz) {
+  int ix, iy, iz;
+  if (BRICK) {
+    ix = max(min(__float2int_rz(gx), s.cmx), s.lox) - s.lox;
+    iy = max(min(__float2int_rz(gy), s.cmy), s.loy) - s.loy;
+    iz = max(min(__float2int_rz(gz), s.cmz), s.loz) - s.loz;
+  } else {
+    ix = max(min(__float2int_rz(gx), s.cmx), 0);
+    iy = max(min(__float2int_rz(gy), s.cmy), 0);
+    iz = max(min(__float2int_rz(gz), s.cmz), 0);
+  }
+  return (unsigned)iz * s.nxy + (unsigned)iy * s.nx + (unsigned)ix;
+}
+
 // A9: owner brick of an in-domain position (destinationID).
 // Same brick as before?  floor(g) per axis inside the owned box (g >= 0 here: truncation = floor).
 template <bool UNIT = false>

@@ -40,6 +40,7 @@ struct TraceArgs {
   // outputs (A6)
   float* verts; unsigned long long n; unsigned cap, stride;
   int vec_ok;                      // capacity % 8 == 0 and verts 32-byte aligned: full-sector vertex stores
+  int prefetch;                    // 1 = one-step-ahead cell prefetch (field.cuh), 0 = off
   int staging;                     // 1 = stage vertices in shared memory (default), 0 = store each directly
   unsigned* counts; unsigned* steps; unsigned* status; float* fin;
   unsigned long long* totals;      // [4]
@@ -56,6 +57,7 @@ struct Lane {
   float px, py, pz;
   unsigned id, n;
   unsigned slot, rec_cd;           // next vertex slot, steps until the next recorded vertex
+  unsigned pf;                     // cell most recently requested by the prefetcher
   unsigned stage0;                 // first slot held in the shared-memory staging group (<= slot)
   // DP5(4) only
   float t, h, k1x, k1y, k1z; bool rejected;
@@ -73,6 +75,11 @@ constexpr int REC_THREADS = 256;
 __device__ __forceinline__ float* rec_stage() {
   __shared__ float s_rec[3 * REC_GROUP * REC_THREADS];        // [plane][slot & 7][thread]
   return s_rec + threadIdx.x;
+}
+
+__device__ __forceinline__ float* rec_scratch() {              // never read: cp.async prefetch target
+  __shared__ float s_scr[REC_THREADS];
+  return s_scr + threadIdx.x;
 }
 
 __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
@@ -93,6 +100,7 @@ __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
       }
     } else {
       const unsigned j0 = L.stage0 & (REC_GROUP - 1);
+#pragma unroll 1
       for (unsigned j = 0; j < cnt; ++j) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) dst[c * plane + j] = s[(c * REC_GROUP + j0 + j) * REC_THREADS];
@@ -164,6 +172,20 @@ __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s,
   float nx = __fmaf_rn(a.h6, sx, L.px), ny = __fmaf_rn(a.h6, sy, L.py), nz = __fmaf_rn(a.h6, sz, L.pz);
   float gx, gy, gz;
   if (!to_index<UNIT>(a.g, nx, ny, nz, gx, gy, gz)) { done = 5; return ST_OUT; }  // A5.5: not recorded
+  if (CACHE && !UNSTEADY && a.prefetch) {
+    // predicted stage points of the NEXT step, in index space: g + 0.5 d and g + d
+    float ox, oy, oz;
+    index_pos<UNIT>(a.g, L.px, L.py, L.pz, ox, oy, oz);
+    const float dx = gx - ox, dy = gy - oy, dz = gz - oz;
+    const unsigned scratch = (unsigned)__cvta_generic_to_shared(rec_scratch());
+    const unsigned vf = clamped_cell<BRICK>(s, gx + dx, gy + dy, gz + dz);
+    if (a.prefetch == 2) {                      // also the half-step point (A/B: not worth its cost)
+      const unsigned vh = clamped_cell<BRICK>(s, __fmaf_rn(0.5f, dx, gx), __fmaf_rn(0.5f, dy, gy), __fmaf_rn(0.5f, dz, gz));
+      if (vh != cc.key && vh != L.pf && vh != vf) prefetch_cell32<LAYOUT>(s, vh, scratch);
+    }
+    if (vf != cc.key && vf != L.pf) prefetch_cell32<LAYOUT>(s, vf, scratch);
+    L.pf = vf;
+  }
   L.px = nx; L.py = ny; L.pz = nz; L.n++;                                       // A5.6
   record_vertex<REC>(a, L);
   return 0;

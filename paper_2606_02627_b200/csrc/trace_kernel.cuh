@@ -65,7 +65,7 @@ trace_kernel(const TraceArgs a) {
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xffffffffu;
   const unsigned long long nwork = a.nwork_dev ? (unsigned long long)*a.nwork_dev : a.nwork;
-  Lane L; L.rejected = false;
+  Lane L; L.rejected = false; L.pf = 0xffffffffu;
   CellCache cc; cc.invalidate();
   Store st = a.s;                 // brick mode: replaced per particle
   int my_brick = 0;
