@@ -13,7 +13,7 @@ namespace streami {
 typedef void (*TraceKernel)(const TraceArgs);
 TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache, bool unit);
 bool unit_geometry(const Geom& g);
-int trace_grid(TraceKernel k, unsigned long long nwork, int* grid);
+int trace_grid(TraceKernel k, unsigned long long nwork, int block, int* grid);
 int check_params(const streami_params* p, bool need_capacity);
 void fill_integrator(TraceArgs& a, const streami_params* p);
 
@@ -171,7 +171,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
     if (e == cudaSuccess) e = cudaMemsetAsync(d_qcount, 0, sizeof(unsigned), st);
     if (e != cudaSuccess) break;
     int grid = 0;
-    rc = trace_grid(k, nwork, &grid);
+    rc = trace_grid(k, nwork, TRACE_BLOCK, &grid);
     if (rc) { cleanup(); return rc; }
     timing_begin(st);
     k<<<grid, TRACE_BLOCK, 0, st>>>(a);

@@ -39,12 +39,13 @@ bool unit_geometry(const Geom& g) {
 }
 
 // Persistent grid: as many blocks as are resident at once (a multiple of the SM count).
-int trace_grid(TraceKernel k, unsigned long long nwork, int* grid) {
+int trace_grid(TraceKernel k, unsigned long long nwork, int block, int* grid) {
   int per_sm = 0;
-  STREAMI_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, TRACE_BLOCK, 0));
+  STREAMI_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, block, 0));
   int sms = num_sms();
   if (per_sm < 1 || sms < 1) return STREAMI_E_CUDA;
-  unsigned long long want = (nwork + TRACE_BLOCK - 1) / TRACE_BLOCK;
+  if (options().max_blocks_per_sm > 0) per_sm = std::min(per_sm, options().max_blocks_per_sm);
+  unsigned long long want = (nwork + block - 1) / block;
   unsigned long long full = (unsigned long long)per_sm * sms;
   *grid = (int)std::max(1ull, std::min(want, full));
   return STREAMI_OK;
@@ -95,7 +96,8 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   const bool cache = options().cell_cache && !unsteady;
   TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache, unit_geometry(f->g));
   int grid = 0;
-  rc = trace_grid(k, n, &grid);
+  const int block = trace_block(params->integrator);
+  rc = trace_grid(k, n, block, &grid);
   if (rc) return rc;
 
   // Segments: K step attempts per particle per launch, Morton re-sort of the survivors between
@@ -142,7 +144,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
   a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
   timing_begin(st);
-  k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+  k<<<grid, block, 0, st>>>(a);
   timing_end(st);
   launch_counter()++;
   e = cudaGetLastError();
@@ -170,7 +172,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
       a.seeds = nullptr; a.qin = q[in]; a.nwork_dev = qcount + in; a.qout = q[out]; a.qout_count = qcount + out;
       a.round = (int)r;
       timing_begin(st);
-      k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+      k<<<grid, block, 0, st>>>(a);
       timing_end(st);
       launch_counter()++;
       e = cudaGetLastError();
