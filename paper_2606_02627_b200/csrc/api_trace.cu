@@ -150,11 +150,11 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   e = cudaGetLastError();
 
   if (K && e == cudaSuccess) {
-    // RK4: a particle takes exactly K steps per segment, so ceil(max_steps / K) launches finish
-    // everything and no count has to come back to the host (the call stays asynchronous; a launch
+    // RK4: a particle takes exactly K steps per segment, so floor(max_steps / K) + 1 launches finish
+    // everything (floor(max_steps / K) + 1 launches) and no count has to come back to the host (the call stays asynchronous; a launch
     // whose queue is empty exits at once).  DP5(4): rejected attempts spend budget too, so the live
     // count is read back every few segments (this synchronises the stream).
-    const unsigned planned = (params->max_steps + K - 1) / K;
+    const unsigned planned = params->max_steps / K + 1;   // the last one also turns n == max_steps into MAX_STEPS
     for (unsigned r = 1; e == cudaSuccess; ++r) {
       if (!dp5 && r >= planned) break;
       const unsigned in = (r - 1) & 1u, out = r & 1u;

@@ -1,0 +1,78 @@
+"""Schedule-only options must not change any result: segments with Morton re-sort of the survivors
+(`segment_steps`), the one-step-ahead cell prefetch (`prefetch`), the staged vertex writer
+(`vertex_staging`), the occupancy limit (`max_blocks_per_sm`).  Each combination is compared bit for
+bit with the oracle (RK4 and DP5(4), every layout family), with capacities that are and are not a
+multiple of the 8-slot staging group, and with a stride that cuts groups at segment boundaries."""
+import numpy as np
+import pytest
+
+from helpers import assert_same, gpu_field, gpu_streamlines
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return t
+
+
+@pytest.fixture(scope="module")
+def S(torch):
+    import paper_2606_02627_b200 as s
+    s.lib()
+    return s
+
+
+@pytest.fixture(scope="module")
+def turb48(wl):
+    return wl.turb_field_cpu(48, 64, 1, 12)
+
+
+DEFAULTS = dict(segment_steps=0, prefetch=1, vertex_staging=1, max_blocks_per_sm=0, presort=1)
+
+
+def _with(S, opts, fn):
+    try:
+        for k, v in opts.items():
+            S.streami_set_option(k, v)
+        return fn()
+    finally:
+        for k, v in DEFAULTS.items():
+            S.streami_set_option(k, v)
+
+
+@pytest.mark.parametrize("layout", [1, 3, 4])
+@pytest.mark.parametrize("opts", [dict(segment_steps=16), dict(segment_steps=37, prefetch=0),
+                                  dict(vertex_staging=0), dict(prefetch=2, max_blocks_per_sm=1),
+                                  dict(segment_steps=5, vertex_staging=0, presort=1)])
+def test_rk4_schedule_options(S, torch, oracle, wl, turb48, layout, opts):
+    n = 70001                                      # >= 65536: sorting and segments are active
+    seeds = wl.seeds_uniform(11, n, [47.0] * 3)
+    g = oracle.grid(turb48.data, turb48.dims, turb48.origin, turb48.spacing)
+    f = gpu_field(S, torch, turb48, layout)
+    for kw in (dict(integrator=0, h=0.25, max_steps=150, vmin=1e-6, capacity=24, stride=3),
+               dict(integrator=0, h=0.25, max_steps=120, vmin=1e-6, capacity=13, stride=1)):
+        ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
+        out = _with(S, opts, lambda: gpu_streamlines(S, torch, f, seeds, **kw))
+        assert_same(out, ref, "rk4 %s %s" % (opts, kw))
+
+
+@pytest.mark.parametrize("layout", [3, 4])
+@pytest.mark.parametrize("opts", [dict(segment_steps=8), dict(segment_steps=25, vertex_staging=0),
+                                  dict(max_blocks_per_sm=2)])
+def test_dp5_schedule_options(S, torch, oracle, wl, turb48, layout, opts):
+    """DP5(4): a segment cut carries t and h and recomputes the FSAL k1; rejected attempts spend
+    budget but a cut waits for the next accepted step."""
+    n = 66000
+    seeds = wl.seeds_uniform(12, n, [47.0] * 3)
+    g = oracle.grid(turb48.data, turb48.dims, turb48.origin, turb48.spacing)
+    f = gpu_field(S, torch, turb48, layout)
+    kw = dict(integrator=1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=90,
+              vmin=1e-6, capacity=16, stride=2)
+    ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
+    out = _with(S, opts, lambda: gpu_streamlines(S, torch, f, seeds, **kw))
+    assert_same(out, ref, "dp5 %s" % opts)
+    assert int(ref.totals[0]) > int(ref.totals[1]), "the case must contain rejected attempts"
