@@ -157,6 +157,10 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
  *   out_handoff_log  [log_capacity]: one entry (round+1)<<48 | dest<<32 | id per hand-off, in
  *                    unspecified order; out_log_count (device, 1 x u64) = hand-offs in total
  *   out_nrounds      HOST pointer: rounds executed.
+ * out_nrounds counts launches: A9's rounds when the round table or the log is requested (or option
+ * "brick_round_steps" = -1); otherwise the library may also cut a round after a step budget (option
+ * "brick_round_steps": 0 = automatic, k > 0 = k steps per round; k = 1 is the paper's one-step
+ * schedule), which changes no per-particle result.
  * This call synchronises cuda_stream once per round (it reads the live count) and before
  * returning.  Returns STREAMI_E_TRUNCATED if the log or the round table overflowed (all other
  * results are still valid). */
@@ -167,11 +171,19 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream);
 
-/* Tuning knobs for measurement (process-wide, not part of the method): name is one of
- * "cell_cache" (0/1, reuse the 8 cell vertices in registers while a sample stays in the cell),
- * "presort" (0/1, order seeds by coarse Morton bin before tracing), "streak_window" (global
- * steps per launch, 0 = automatic), "kernel_timing" (0/1, record a CUDA event pair on the
- * launching stream around every advection-kernel launch).  Returns INVALID for unknown names. */
+/* Tuning knobs (process-wide).  None changes any result: they select schedules and staging only,
+ * and exist so that each design choice can be measured A/B in one process.  name is one of
+ *   "cell_cache"        0/1   keep the 8 cell vertices in registers while samples stay in the cell
+ *   "presort"           0/1   process work items in Morton order of their 4^3-cell block
+ *   "segment_steps"     K     streamlines: K step attempts per particle per launch, survivors are
+ *                             re-sorted between launches (0 = one launch; DP5(4) then synchronises)
+ *   "prefetch"          0/1/2 RK4: request the predicted next cell one step ahead (2: two points)
+ *   "vertex_staging"    0/1   stage vertices in shared memory and store full 32-byte sectors
+ *   "max_blocks_per_sm" B     limit resident blocks per SM (0 = as many as fit)
+ *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0)
+ *   "streak_window"     W     streaklines: global steps per launch (0 = automatic)
+ *   "kernel_timing"     0/1   record a CUDA event pair around every advection-kernel launch
+ * Returns INVALID for unknown names. */
 int streami_set_option(const char* name, int value);
 int streami_get_option(const char* name, int* value);
 

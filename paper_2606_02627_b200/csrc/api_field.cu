@@ -12,7 +12,7 @@
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0}; return o; }
+Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0}; return o; }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -295,6 +295,7 @@ int streami_set_option(const char* name, int value) {
   else if (!strcmp(name, "kernel_timing")) o.kernel_timing = value != 0;
   else if (!strcmp(name, "segment_steps")) o.segment_steps = value < 0 ? 0 : value;
   else if (!strcmp(name, "vertex_staging")) o.vertex_staging = value != 0;
+  else if (!strcmp(name, "brick_round_steps")) o.brick_round_steps = value < -1 ? -1 : value;
   else if (!strcmp(name, "max_blocks_per_sm")) o.max_blocks_per_sm = value < 0 ? 0 : value;
   else if (!strcmp(name, "prefetch")) o.prefetch = value < 0 ? 0 : (value > 2 ? 2 : value);
   else return STREAMI_E_INVALID;
@@ -310,6 +311,7 @@ int streami_get_option(const char* name, int* value) {
   else if (!strcmp(name, "kernel_timing")) *value = o.kernel_timing;
   else if (!strcmp(name, "segment_steps")) *value = o.segment_steps;
   else if (!strcmp(name, "vertex_staging")) *value = o.vertex_staging;
+  else if (!strcmp(name, "brick_round_steps")) *value = o.brick_round_steps;
   else if (!strcmp(name, "max_blocks_per_sm")) *value = o.max_blocks_per_sm;
   else if (!strcmp(name, "prefetch")) *value = o.prefetch;
   else return STREAMI_E_INVALID;

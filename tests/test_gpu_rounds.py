@@ -166,3 +166,39 @@ def test_bricks_halo_miss_and_truncation(S, torch, oracle, wl):
     # nothing inside: zero rounds
     out = gpu_bricks(S, torch, wl, fld, nb, np.full((5, 3), 99.0, dtype=np.float32), **kw)
     assert out["nrounds"] == 0 and list(out["status"]) == [1] * 5 and out["nlog"] == 0
+
+
+@pytest.mark.parametrize("k", [1, 7])
+def test_bricks_paper_step_rounds(S, torch, oracle, wl, k):
+    """the paper's schedule (every particle re-queued after every RK step,
+    PAPER.md:96-101, 142-144) via option brick_round_steps.  Trajectories, statuses, step counts and
+    the set of brick changes do not depend on the round structure (A9); the round table counts
+    every queued particle and the rounds equal the steps of the longest-lived particle."""
+    N, nb = 32, (2, 2, 2)
+    fld = wl.turb_field_cpu(N, 48, 1, 6)
+    n = 9001
+    seeds = wl.seeds_uniform(5, n, [N - 1.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=60, vmin=1e-6, capacity=61, stride=1)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    S.streami_set_option("brick_round_steps", k)
+    try:
+        out = gpu_bricks(S, torch, wl, fld, nb, seeds, max_rounds=128, **kw)
+    finally:
+        S.streami_set_option("brick_round_steps", 0)
+    assert not out["truncated"]
+    for key in ("status", "steps", "counts"):
+        assert np.array_equal(out[key], getattr(ref, key)), key
+    assert np.array_equal(out["final"].view(np.uint32), ref.final.view(np.uint32))
+    assert np.array_equal(out["vertices"].view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(out["totals"], ref.totals)
+    strip = lambda log: np.sort(log & np.uint64((1 << 48) - 1))          # (dest, id) without the round
+    assert np.array_equal(strip(out["log"]), strip(ref.log))
+    assert out["nrounds"] >= int(ref.steps.max()) // k
+    rc = out["round_counts"]
+    if k == 1:       # one step per round: round r holds exactly the particles that completed r steps
+        assert out["nrounds"] == int(ref.steps.max()) + 1
+        for r in (1, 2, 3, 30):
+            assert int(rc[r].sum()) == np.count_nonzero(ref.steps >= r), r
