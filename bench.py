@@ -517,13 +517,14 @@ def main():
                 "kernel_ms_per_launch": kms, "kernel_launches_per_step": launches_per_step,
                 "algorithmic_bytes_per_launch": alg / launches_per_step, "peak_source": peak_src,
                 "kernel_share_of_step": kern_ms / total_ms if world == 1 else None}
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram bytes per launch (profiles/traffic.md)
     if os.path.exists(tpath):
+        import csv
         with open(tpath) as f:
-            tr = json.load(f).get(args.workload)
-        if tr:
-            roofline["traffic"] = tr["dram_bytes_per_launch"]
-            roofline["traffic_source"] = tr["source"]
+            for row in csv.DictReader(f):
+                if row["workload"] == args.workload:
+                    roofline["traffic"] = float(row["dram_bytes_per_launch"])
+                    roofline["traffic_source"] = row["source"]
 
     cpu = None
     if world == 1 and not args.no_cpu and job.host_field is not None:
