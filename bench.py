@@ -12,7 +12,7 @@ recording (capacity 256, stride 8).
 
 metric  = RK particle-steps per second (step ATTEMPTS), whole job over all ranks.
 value   = device-resident inputs, CUDA events on the launching stream around each step.
-e2e     = the same through streami_trace_streamlines_host with pinned HOST buffers
+e2e     = the same through the C-ABI *_host calls with pinned HOST buffers
           (H2D of the seeds and D2H of every output inside the timed region).
 roofline= the advection kernel alone (event pair recorded by the library around its launch):
           algorithmic bytes / its duration, against MEASURED_PEAKS.json.
@@ -243,13 +243,13 @@ class Job:
                           counts=pin(self.counts), steps=pin(self.steps_o), status=pin(self.status_o),
                           final=None if self.final_o is None else pin(self.final_o),
                           totals=t.zeros(4, dtype=t.int64).pin_memory())
-            if self.kind not in ("gyre", "bricks"):
-                self.prm_h = self.S.params(out_steps=None, out_status=None, out_final=None,
-                                           out_totals=None, **self.w["prm"])
-                self.prm_h.out_steps = self.h["steps"].data_ptr()
-                self.prm_h.out_status = self.h["status"].data_ptr()
+            kw = dict(self.w["prm"])
+            self.prm_h = self.S.params(out_steps=None, out_status=None, out_final=None, out_totals=None, **kw)
+            self.prm_h.out_steps = self.h["steps"].data_ptr()
+            self.prm_h.out_status = self.h["status"].data_ptr()
+            if self.h["final"] is not None:
                 self.prm_h.out_final = self.h["final"].data_ptr()
-                self.prm_h.out_totals = self.h["totals"].data_ptr()
+            self.prm_h.out_totals = self.h["totals"].data_ptr()
         return self.h
 
     def e2e_bytes(self):
@@ -260,20 +260,15 @@ class Job:
         return bi, bo
 
     def step_host(self):
-        """Streamlines: the C-ABI host-buffer call does the copies itself.  Streaklines and
-        bricks have no host-buffer entry point yet: the same copies are issued here around the
-        device call (pinned host -> device, device -> pinned host, then a stream sync)."""
-        h = self._pinned()
-        if self.kind not in ("gyre", "bricks"):
-            self.S.streami_trace_streamlines_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
-            return
-        self.seeds.copy_(h["seeds"], non_blocking=True)
-        self.step_device()
-        for k, d in (("verts", self.verts), ("counts", self.counts), ("steps", self.steps_o),
-                     ("status", self.status_o), ("final", self.final_o), ("totals", self.totals_o)):
-            if d is not None:
-                h[k].copy_(d, non_blocking=True)
-        self.torch.cuda.current_stream().synchronize()
+        """One step through the C-ABI host-buffer calls: H2D of the seeds / rake points, the
+        trace, D2H of every output, stream sync -- all inside the library."""
+        h, S = self._pinned(), self.S
+        if self.kind == "gyre":
+            S.streami_trace_streaklines_host(self.field, h["seeds"], self.nsteps, self.prm_h, h["verts"], h["counts"])
+        elif self.kind == "bricks":
+            S.streami_brick_advect_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
+        else:
+            S.streami_trace_streamlines_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
 
     def work(self):
         """(attempted steps, accepted steps, field samples, hand-offs, stored vertices) of the

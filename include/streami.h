@@ -171,6 +171,21 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream);
 
+/* streami_trace_streaklines / streami_brick_advect with HOST buffers (points/seeds, out_vertices,
+ * out_counts, the optional outputs in params, the round table, the log and its count are host
+ * pointers; pinned memory makes the copies faster but is not required): copy host->device, run,
+ * copy device->host, synchronise cuda_stream before returning.  The round table keeps the caller's
+ * content in the rows the call does not write. */
+int streami_trace_streaklines_host(streami_field f, const float* points, size_t m, unsigned nsteps,
+                                   const streami_params* params, float* out_vertices,
+                                   unsigned* out_counts, void* cuda_stream);
+int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
+                              const streami_params* params, float* out_vertices, unsigned* out_counts,
+                              unsigned* out_round_counts, unsigned max_rounds,
+                              unsigned long long* out_handoff_log, size_t log_capacity,
+                              unsigned long long* out_log_count, unsigned* out_nrounds,
+                              void* cuda_stream);
+
 /* Tuning knobs (process-wide).  None changes any result: they select schedules and staging only,
  * and exist so that each design choice can be measured A/B in one process.  name is one of
  *   "cell_cache"        0/1   keep the 8 cell vertices in registers while samples stay in the cell

@@ -54,6 +54,8 @@ def lib():
         L.streami_trace_streamlines_host.argtypes = [P, P, Z, P, P, P, P]
         L.streami_trace_streaklines.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
+        L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
+        L.streami_brick_advect_host.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
         L.streami_set_option.argtypes = [ctypes.c_char_p, I]
         L.streami_get_option.argtypes = [ctypes.c_char_p, P]
         L.streami_launch_count.restype = ctypes.c_ulonglong
@@ -207,6 +209,38 @@ def streami_brick_advect(field, seeds, prm, out_vertices, out_counts, out_round_
                                            _ptr(out_round_counts), max_rounds, _ptr(out_handoff_log),
                                            log_cap, _ptr(out_log_count), ctypes.byref(nrounds),
                                            _stream(stream)), allow=(E_TRUNCATED,))
+    return nrounds.value, rc == E_TRUNCATED
+
+
+def _host(t, name):
+    if t is not None and (t.is_cuda or not t.is_contiguous()):
+        raise ValueError("%s: the host variants take contiguous CPU tensors" % name)
+
+
+def streami_trace_streaklines_host(field, points, nsteps, prm_host, out_vertices, out_counts, stream=None):
+    """Host-buffer variant; prm_host carries host pointers (or None) in its optional outputs."""
+    for t, nm in ((points, "points"), (out_vertices, "out_vertices"), (out_counts, "out_counts")):
+        _host(t, nm)
+    _check(lib().streami_trace_streaklines_host(field.handle, _ptr(points), points.shape[0], int(nsteps),
+                                                ctypes.byref(prm_host), _ptr(out_vertices),
+                                                _ptr(out_counts), _stream(stream)))
+
+
+def streami_brick_advect_host(field, seeds, prm_host, out_vertices, out_counts, out_round_counts=None,
+                              out_handoff_log=None, out_log_count=None, stream=None):
+    """Host-buffer variant.  Returns (nrounds, truncated)."""
+    for t, nm in ((seeds, "seeds"), (out_vertices, "out_vertices"), (out_counts, "out_counts"),
+                  (out_round_counts, "round_counts"), (out_handoff_log, "log"), (out_log_count, "log_count")):
+        _host(t, nm)
+    max_rounds = 0 if out_round_counts is None else out_round_counts.shape[0]
+    log_cap = 0 if out_handoff_log is None else out_handoff_log.numel()
+    nrounds = ctypes.c_uint(0)
+    rc = _check(lib().streami_brick_advect_host(field.handle, _ptr(seeds), seeds.shape[0],
+                                                ctypes.byref(prm_host), _ptr(out_vertices),
+                                                _ptr(out_counts), _ptr(out_round_counts), max_rounds,
+                                                _ptr(out_handoff_log), log_cap, _ptr(out_log_count),
+                                                ctypes.byref(nrounds), _stream(stream)),
+                allow=(E_TRUNCATED,))
     return nrounds.value, rc == E_TRUNCATED
 
 

@@ -221,3 +221,94 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
 }
 
 }  // extern "C"
+
+// ---- host-buffer variants (same calls, every buffer in host memory) -----------------------------
+namespace {
+// Device mirrors of host buffers on one stream: allocate (+ upload), download, free.
+struct Mirror {
+  cudaStream_t st;
+  std::vector<void*> dev;
+  std::vector<std::pair<void*, std::pair<void*, size_t>>> back;   // device -> (host, bytes)
+  cudaError_t err = cudaSuccess;
+  explicit Mirror(cudaStream_t s) : st(s) {}
+  void* make(const void* host_in, void* host_out, size_t bytes) {
+    if (err != cudaSuccess || bytes == 0 || (!host_in && !host_out)) return nullptr;
+    void* d = nullptr;
+    err = cudaMallocAsync(&d, bytes, st);
+    if (err != cudaSuccess) return nullptr;
+    dev.push_back(d);
+    if (host_in) err = cudaMemcpyAsync(d, host_in, bytes, cudaMemcpyHostToDevice, st);
+    if (host_out) back.push_back({d, {host_out, bytes}});
+    return d;
+  }
+  cudaError_t download() {
+    for (auto& b : back)
+      if (err == cudaSuccess) err = cudaMemcpyAsync(b.second.first, b.first, b.second.second, cudaMemcpyDeviceToHost, st);
+    return err;
+  }
+  ~Mirror() { for (void* d : dev) cudaFreeAsync(d, st); }
+};
+}  // namespace
+
+extern "C" {
+
+int streami_trace_streaklines_host(streami_field f, const float* points, size_t m, unsigned nsteps,
+                                   const streami_params* params, float* out_vertices,
+                                   unsigned* out_counts, void* cuda_stream) {
+  if (!f || !params || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t np = m * (size_t)nsteps;
+  int rc;
+  {
+    Mirror mr(st);
+    streami_params dp = *params;
+    float* d_pts = (float*)mr.make(points, nullptr, 3 * m * sizeof(float));
+    float* d_v = (float*)mr.make(nullptr, out_vertices, 3 * np * sizeof(float));
+    unsigned* d_c = (unsigned*)mr.make(nullptr, out_counts, m * sizeof(unsigned));
+    dp.out_steps = (unsigned*)mr.make(nullptr, params->out_steps, np * sizeof(unsigned));
+    dp.out_status = (unsigned*)mr.make(nullptr, params->out_status, np * sizeof(unsigned));
+    dp.out_final = nullptr;
+    dp.out_totals = (unsigned long long*)mr.make(nullptr, params->out_totals, 4 * sizeof(unsigned long long));
+    if (mr.err != cudaSuccess) return check(mr.err);
+    rc = streami_trace_streaklines(f, d_pts, m, nsteps, &dp, d_v, d_c, cuda_stream);
+    if (rc == STREAMI_OK && mr.download() != cudaSuccess) rc = check(mr.err);
+  }
+  if (rc == STREAMI_OK) rc = check(cudaStreamSynchronize(st));
+  return rc;
+}
+
+int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
+                              const streami_params* params, float* out_vertices, unsigned* out_counts,
+                              unsigned* out_round_counts, unsigned max_rounds,
+                              unsigned long long* out_handoff_log, size_t log_capacity,
+                              unsigned long long* out_log_count, unsigned* out_nrounds,
+                              void* cuda_stream) {
+  if (!f || !params || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
+  if (params->capacity == 0) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int nb = f->bricked ? (int)f->bricks.size() : 0;
+  int rc;
+  {
+    Mirror mr(st);
+    streami_params dp = *params;
+    float* d_seeds = (float*)mr.make(seeds, nullptr, 3 * n * sizeof(float));
+    float* d_v = (float*)mr.make(nullptr, out_vertices, 3 * n * (size_t)params->capacity * sizeof(float));
+    unsigned* d_c = (unsigned*)mr.make(nullptr, out_counts, n * sizeof(unsigned));
+    // the round table is only partly written by the call: upload the caller's content first
+    unsigned* d_rc = (unsigned*)mr.make(out_round_counts, out_round_counts, (size_t)max_rounds * nb * sizeof(unsigned));
+    unsigned long long* d_log = (unsigned long long*)mr.make(nullptr, out_handoff_log, log_capacity * sizeof(unsigned long long));
+    unsigned long long* d_lc = (unsigned long long*)mr.make(nullptr, out_log_count, sizeof(unsigned long long));
+    dp.out_steps = (unsigned*)mr.make(nullptr, params->out_steps, n * sizeof(unsigned));
+    dp.out_status = (unsigned*)mr.make(nullptr, params->out_status, n * sizeof(unsigned));
+    dp.out_final = (float*)mr.make(nullptr, params->out_final, 3 * n * sizeof(float));
+    dp.out_totals = (unsigned long long*)mr.make(nullptr, params->out_totals, 4 * sizeof(unsigned long long));
+    if (mr.err != cudaSuccess) return check(mr.err);
+    rc = streami_brick_advect(f, d_seeds, n, &dp, d_v, d_c, d_rc, max_rounds, d_log, log_capacity, d_lc,
+                              out_nrounds, cuda_stream);
+    if ((rc == STREAMI_OK || rc == STREAMI_E_TRUNCATED) && mr.download() != cudaSuccess) rc = check(mr.err);
+  }
+  if (rc == STREAMI_OK || rc == STREAMI_E_TRUNCATED) { int s = check(cudaStreamSynchronize(st)); if (s) rc = s; }
+  return rc;
+}
+
+}  // extern "C"

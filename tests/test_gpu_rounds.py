@@ -202,3 +202,64 @@ def test_bricks_paper_step_rounds(S, torch, oracle, wl, k):
         assert out["nrounds"] == int(ref.steps.max()) + 1
         for r in (1, 2, 3, 30):
             assert int(rc[r].sum()) == np.count_nonzero(ref.steps >= r), r
+
+
+def test_host_buffer_variants_of_streaklines_and_bricks(S, torch, oracle, wl):
+    """streami_trace_streaklines_host / streami_brick_advect_host: the same results with every
+    buffer in (pinned or pageable) host memory."""
+    import ctypes
+    # streaklines on a small double gyre
+    fld = wl.double_gyre_field(dims=(32, 16, 8), nslices=6, dt=0.25)
+    pts = wl.rake_c4(8, 8)
+    ns = 40
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+    ref = oracle.streaklines(g, pts, ns, oracle.params(integrator=0, h=0.05, vmin=1e-6, max_steps=ns), "f32")
+    f = gpu_field(S, torch, fld)
+    m = pts.shape[0]
+    h_pts = torch.from_numpy(pts.copy()).pin_memory()
+    h_v = torch.zeros((3, ns, m), dtype=torch.float32).pin_memory()
+    h_c = torch.zeros(m, dtype=torch.int32)
+    h_st = torch.zeros(ns * m, dtype=torch.int32)
+    prm = S.params(integrator=0, h=0.05, vmin=1e-6)
+    prm.out_status = h_st.data_ptr()
+    S.streami_trace_streaklines_host(f, h_pts, ns, prm, h_v, h_c)
+    assert np.array_equal(h_v.numpy().view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(h_c.numpy().astype(np.uint32), ref.counts)
+    assert np.array_equal(h_st.numpy().astype(np.uint32), ref.status)
+    # bricks
+    N, nb = 24, (2, 1, 2)
+    fld = wl.turb_field_cpu(N, 32, 1, 5)
+    n = 3000
+    seeds = wl.seeds_uniform(9, n, [N - 1.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=120, vmin=1e-6, capacity=16, stride=8)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    cut = wl.cut_bricks(fld, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi) for a, (lo, hi) in zip(cut, boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    fb = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, 1,
+                                        [torch.from_numpy(a).cuda() for a in cut])
+    h_seeds = torch.from_numpy(seeds.copy())
+    h_v = torch.full((3, n, 16), float("nan"), dtype=torch.float32)
+    h_c = torch.zeros(n, dtype=torch.int32)
+    h_steps = torch.zeros(n, dtype=torch.int32); h_status = torch.zeros(n, dtype=torch.int32)
+    h_final = torch.zeros((3, n), dtype=torch.float32); h_tot = torch.zeros(4, dtype=torch.int64)
+    h_rc = torch.full((32, 4), -1, dtype=torch.int32)
+    h_log = torch.zeros(64 * n, dtype=torch.int64); h_lc = torch.zeros(1, dtype=torch.int64)
+    prm = S.params(**kw)
+    prm.out_steps = h_steps.data_ptr(); prm.out_status = h_status.data_ptr()
+    prm.out_final = h_final.data_ptr(); prm.out_totals = h_tot.data_ptr()
+    nrounds, trunc = S.streami_brick_advect_host(fb, h_seeds, prm, h_v, h_c, h_rc, h_log, h_lc)
+    assert not trunc and nrounds == ref.nrounds
+    assert np.array_equal(h_status.numpy().astype(np.uint32), ref.status)
+    assert np.array_equal(h_steps.numpy().astype(np.uint32), ref.steps)
+    assert np.array_equal(h_c.numpy().astype(np.uint32), ref.counts)
+    assert np.array_equal(h_final.numpy().view(np.uint32), ref.final.view(np.uint32))
+    mask = np.arange(16)[None, :] < ref.counts[:, None]      # slots beyond the count hold whatever the
+    for c in range(3):                                       # device scratch array held (include/streami.h)
+        assert np.array_equal(h_v.numpy()[c].view(np.uint32)[mask], ref.vertices[c].view(np.uint32)[mask])
+    assert np.array_equal(h_tot.numpy().astype(np.uint64), ref.totals)
+    assert np.array_equal(h_rc.numpy()[:ref.nrounds].astype(np.uint32), ref.round_counts[:ref.nrounds])
+    assert (h_rc.numpy()[ref.nrounds + 1:] == -1).all()
+    nlog = int(h_lc.item())
+    assert nlog == ref.nlog
+    assert np.array_equal(np.sort(h_log.numpy().view(np.uint64)[:nlog]), ref.log)
