@@ -171,6 +171,40 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream);
 
+/* Step-synchronous streaklines: Tracer::step() of Listing 2 ("one advection step
+ * ... then a new batch of particles").  _begin binds the rake, the parameters and the caller's
+ * slot array out_vertices [3][nsteps][m] (device, as streami_trace_streaklines) and allocates one
+ * status byte per particle from the stream pool; _step advances k global steps (clamped to
+ * nsteps; asynchronous); after s steps slot (j, i), j < s, holds the CURRENT position of particle
+ * (i, j) (its last inside position if it died), identical to what streami_trace_streaklines would
+ * return for nsteps = s; _position reports s; _end writes out_counts [m] (may be NULL) and
+ * params->out_status, frees the handle and its scratch.  streami_trace_streaklines = begin,
+ * step(nsteps), end.  All calls of one handle must use the same stream. */
+typedef struct streami_streak_s* streami_streak;
+int streami_streak_begin(streami_field f, const float* points, size_t m, unsigned nsteps,
+                         const streami_params* params, float* out_vertices, void* cuda_stream,
+                         streami_streak* out);
+int streami_streak_step(streami_streak s, unsigned k, void* cuda_stream);
+int streami_streak_position(streami_streak s, unsigned* steps_done /*host*/);
+int streami_streak_end(streami_streak s, unsigned* out_counts, void* cuda_stream);
+
+/* Polyline assembly (the paper's getLines / assembleOutput): one
+ * contiguous AoS point buffer plus a per-line offset table, ready for a renderer or a writer.
+ *   streami_streamline_lines: line id = the stored vertices of particle id in step order;
+ *     vertices [3][n][capacity] and counts [n] as written by streami_trace_streamlines /
+ *     streami_brick_advect.
+ *   streami_streak_lines: line i = the particles of rake point i that are alive now, from the
+ *     youngest release to the oldest, at the current step of the handle.
+ * out_offsets [lines+1] device u64 (exclusive scan of the line lengths, last = total points);
+ * out_points [total][3] device, or NULL to compute the offsets only (call once with NULL to learn
+ * the total, allocate, call again); out_total HOST, may be NULL; when given the call synchronises
+ * the stream. */
+int streami_streamline_lines(const float* vertices, const unsigned* counts, size_t n, unsigned capacity,
+                             unsigned long long* out_offsets, float* out_points,
+                             unsigned long long* out_total, void* cuda_stream);
+int streami_streak_lines(streami_streak s, unsigned long long* out_offsets, float* out_points,
+                         unsigned long long* out_total, void* cuda_stream);
+
 /* streami_trace_streaklines / streami_brick_advect with HOST buffers (points/seeds, out_vertices,
  * out_counts, the optional outputs in params, the round table, the log and its count are host
  * pointers; pinned memory makes the copies faster but is not required): copy host->device, run,

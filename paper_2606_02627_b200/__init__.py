@@ -55,6 +55,12 @@ def lib():
         L.streami_trace_streaklines.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
+        L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
+        L.streami_streak_step.argtypes = [P, U, P]
+        L.streami_streak_position.argtypes = [P, P]
+        L.streami_streak_end.argtypes = [P, P, P]
+        L.streami_streak_lines.argtypes = [P, P, P, P, P]
+        L.streami_streamline_lines.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_brick_advect_host.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
         L.streami_set_option.argtypes = [ctypes.c_char_p, I]
         L.streami_get_option.argtypes = [ctypes.c_char_p, P]
@@ -212,6 +218,55 @@ def streami_brick_advect(field, seeds, prm, out_vertices, out_counts, out_round_
     return nrounds.value, rc == E_TRUNCATED
 
 
+class Streak:
+    """Step-synchronous streaklines (streami_streak_begin/_step/_lines/_end)."""
+
+    def __init__(self, field, points, nsteps, prm, out_vertices, stream=None):
+        _req(points, torch.float32, "points"); _req(out_vertices, torch.float32, "out_vertices")
+        self._keep = (field, points, prm, out_vertices)
+        self.m, self.nsteps = points.shape[0], int(nsteps)
+        self.handle = ctypes.c_void_p(None)
+        _check(lib().streami_streak_begin(field.handle, _ptr(points), self.m, self.nsteps, ctypes.byref(prm),
+                                          _ptr(out_vertices), _stream(stream), ctypes.byref(self.handle)))
+
+    def step(self, k=1, stream=None):
+        _check(lib().streami_streak_step(self.handle, int(k), _stream(stream)))
+
+    def position(self):
+        s = ctypes.c_uint(0)
+        _check(lib().streami_streak_position(self.handle, ctypes.byref(s)))
+        return s.value
+
+    def lines(self, stream=None):
+        """(offsets [m+1] int64 cuda, points [total, 3] float32 cuda) of the current snapshot."""
+        off = torch.empty(self.m + 1, dtype=torch.int64, device="cuda")
+        total = ctypes.c_ulonglong(0)
+        _check(lib().streami_streak_lines(self.handle, _ptr(off), None, ctypes.byref(total), _stream(stream)))
+        pts = torch.empty((total.value, 3), dtype=torch.float32, device="cuda")
+        _check(lib().streami_streak_lines(self.handle, _ptr(off), _ptr(pts), None, _stream(stream)))
+        return off, pts
+
+    def end(self, out_counts=None, stream=None):
+        _req(out_counts, torch.int32, "out_counts")
+        if self.handle:
+            _check(lib().streami_streak_end(self.handle, _ptr(out_counts), _stream(stream)))
+            self.handle = None
+
+
+def streami_streamline_lines(vertices, counts, stream=None):
+    """Polylines of a streamline result: (offsets [n+1] int64 cuda, points [total, 3] float32 cuda)."""
+    _req(vertices, torch.float32, "vertices"); _req(counts, torch.int32, "counts")
+    n, cap = counts.shape[0], vertices.shape[2]
+    off = torch.empty(n + 1, dtype=torch.int64, device="cuda")
+    total = ctypes.c_ulonglong(0)
+    _check(lib().streami_streamline_lines(_ptr(vertices), _ptr(counts), n, cap, _ptr(off), None,
+                                          ctypes.byref(total), _stream(stream)))
+    pts = torch.empty((total.value, 3), dtype=torch.float32, device="cuda")
+    _check(lib().streami_streamline_lines(_ptr(vertices), _ptr(counts), n, cap, _ptr(off), _ptr(pts), None,
+                                          _stream(stream)))
+    return off, pts
+
+
 def _host(t, name):
     if t is not None and (t.is_cuda or not t.is_contiguous()):
         raise ValueError("%s: the host variants take contiguous CPU tensors" % name)
@@ -264,3 +319,17 @@ def streami_kernel_time():
     ms, cnt = ctypes.c_float(0.0), ctypes.c_uint(0)
     _check(lib().streami_kernel_time(ctypes.byref(ms), ctypes.byref(cnt)))
     return ms.value, cnt.value
+
+
+def write_obj(path, offsets, points):
+    """Write assembled polylines as a Wavefront OBJ file (the paper hands its lines to a renderer or
+    an OBJ file): one `v x y z` per point, one `l i j k ...` per line with at least two
+    points (1-based indices).  offsets/points as returned by the *_lines calls (any device)."""
+    off = offsets.detach().cpu().tolist()
+    pts = points.detach().cpu().tolist()
+    with open(path, "w") as f:
+        for x, y, z in pts:
+            f.write("v %.9g %.9g %.9g\n" % (x, y, z))
+        for a, b in zip(off[:-1], off[1:]):
+            if b - a >= 2:
+                f.write("l " + " ".join(str(k + 1) for k in range(a, b)) + "\n")

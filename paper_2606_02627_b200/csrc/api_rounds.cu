@@ -5,6 +5,7 @@
 #include <vector>
 
 #include "internal.h"
+#include "lines.cuh"
 #include "misc_kernels.cuh"
 #include "sorter.cuh"
 #include "trace_kernel.cuh"
@@ -32,18 +33,27 @@ using namespace streami;
 
 extern "C" {
 
-int streami_trace_streaklines(streami_field f, const float* points, size_t m, unsigned nsteps,
-                              const streami_params* params, float* out_vertices,
-                              unsigned* out_counts, void* cuda_stream) {
-  if (!f || f->bricked || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
+// ---- step-synchronous streaklines (Tracer::step() of Listing 2) ---------------
+struct streami_streak_s {
+  streami::StreakArgs a;
+  streami::StreakKernel k;
+  unsigned done;          // global steps executed so far
+  unsigned window;        // global steps per launch
+  unsigned* out_status;   // optional [nsteps*m]
+};
+
+int streami_streak_begin(streami_field f, const float* points, size_t m, unsigned nsteps,
+                         const streami_params* params, float* out_vertices, void* cuda_stream,
+                         streami_streak* out) {
+  if (!out) return STREAMI_E_INVALID;
+  *out = nullptr;
+  if (!f || f->bricked || m == 0 || nsteps == 0 || !points || !out_vertices) return STREAMI_E_INVALID;
   int rc = check_params(params, false);
   if (rc) return rc;
   if (params->integrator != 0) return STREAMI_E_INVALID;      // shared stage times need a fixed step
   if ((unsigned long long)m * nsteps > 0xffffffffull) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
-  if (m == 0 || nsteps == 0) return STREAMI_OK;
-
   const bool unsteady = f->g.nslices > 1;
   // Window = global steps per launch.  Unsteady: about two slice intervals, so that the slices a
   // launch touches stay L2-resident; steady: everything in one launch.
@@ -56,33 +66,124 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
     }
   }
   unsigned char* state = nullptr;
-  const size_t total = (size_t)m * nsteps;
-  STREAMI_TRY(cudaMallocAsync((void**)&state, total, st));
-  StreakArgs a{};
+  STREAMI_TRY(cudaMallocAsync((void**)&state, (size_t)m * nsteps, st));
+  streami_streak_s* h = new streami_streak_s();
+  StreakArgs& a = h->a;
   a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
   a.points = points; a.m = m; a.nsteps = nsteps;
   a.h = params->h; a.h2 = 0.5f * params->h; a.h6 = params->h / 6.0f;
   a.vmin2 = params->vmin * params->vmin; a.t0 = params->t0;
   a.verts = out_vertices; a.state = state; a.steps = params->out_steps; a.totals = params->out_totals;
-  StreakKernel k = pick_streak(f->layout, unsteady);
+  h->k = pick_streak(f->layout, unsteady);
+  h->done = 0; h->window = K; h->out_status = params->out_status;
+  *out = h;
+  return STREAMI_OK;
+}
+
+int streami_streak_step(streami_streak h, unsigned k, void* cuda_stream) {
+  if (!h) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  StreakArgs& a = h->a;
+  const unsigned target = (unsigned)std::min<unsigned long long>((unsigned long long)h->done + k, a.nsteps);
   cudaError_t e = cudaSuccess;
-  for (unsigned s0 = 0; s0 < nsteps && e == cudaSuccess; s0 += K) {
-    a.s0 = s0; a.s1 = std::min(nsteps, s0 + K);
-    unsigned long long threads = (unsigned long long)m * a.s1;
+  while (h->done < target && e == cudaSuccess) {
+    a.s0 = h->done; a.s1 = std::min(target, h->done + h->window);
+    unsigned long long threads = a.m * (unsigned long long)a.s1;
     timing_begin(st);
-    k<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(a);
+    h->k<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(a);
     timing_end(st);
     launch_counter()++;
     e = cudaGetLastError();
+    h->done = a.s1;
   }
-  if (e == cudaSuccess) {
-    streak_finalize_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(state, m, nsteps, out_counts,
-                                                                       params->out_status);
+  return check(e);
+}
+
+int streami_streak_position(streami_streak h, unsigned* steps_done) {
+  if (!h || !steps_done) return STREAMI_E_INVALID;
+  *steps_done = h->done;
+  return STREAMI_OK;
+}
+
+int streami_streak_lines(streami_streak h, unsigned long long* out_offsets, float* out_points,
+                         unsigned long long* out_total, void* cuda_stream) {
+  if (!h || !out_offsets) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const StreakArgs& a = h->a;
+  unsigned* counts = nullptr;
+  STREAMI_TRY(cudaMallocAsync((void**)&counts, sizeof(unsigned) * a.m, st));
+  const unsigned blocks = (unsigned)((a.m + 255) / 256);
+  count_streak_kernel<<<blocks, 256, 0, st>>>(a.state, a.m, h->done, counts);
+  launch_counter()++;
+  int rc = check(cudaGetLastError());
+  if (rc == STREAMI_OK) rc = scan_counts(counts, a.m, out_offsets, st);
+  if (rc == STREAMI_OK && out_points) {
+    gather_streak_kernel<<<blocks, 256, 0, st>>>(a.verts, a.state, a.m, a.nsteps, h->done, out_offsets, out_points);
+    launch_counter()++;
+    rc = check(cudaGetLastError());
+  }
+  cudaFreeAsync(counts, st);
+  if (rc == STREAMI_OK && out_total) {
+    cudaError_t e = cudaMemcpyAsync(out_total, out_offsets + a.m, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    rc = check(e);
+  }
+  return rc;
+}
+
+int streami_streak_end(streami_streak h, unsigned* out_counts, void* cuda_stream) {
+  if (!h) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaSuccess;
+  if (out_counts) {
+    streak_finalize_kernel<<<(unsigned)((h->a.m + 255) / 256), 256, 0, st>>>(h->a.state, h->a.m, h->a.nsteps, h->done,
+                                                                             out_counts, h->out_status);
     launch_counter()++;
     e = cudaGetLastError();
   }
-  cudaFreeAsync(state, st);
+  cudaFreeAsync(h->a.state, st);
+  delete h;
   return check(e);
+}
+
+int streami_trace_streaklines(streami_field f, const float* points, size_t m, unsigned nsteps,
+                              const streami_params* params, float* out_vertices,
+                              unsigned* out_counts, void* cuda_stream) {
+  if (!f || f->bricked || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, false);
+  if (rc) return rc;
+  if (params->integrator != 0) return STREAMI_E_INVALID;
+  if ((unsigned long long)m * nsteps > 0xffffffffull) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (m == 0 || nsteps == 0) {
+    if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
+    return STREAMI_OK;
+  }
+  streami_streak h = nullptr;
+  rc = streami_streak_begin(f, points, m, nsteps, params, out_vertices, cuda_stream, &h);
+  if (rc) return rc;
+  rc = streami_streak_step(h, nsteps, cuda_stream);
+  int rc2 = streami_streak_end(h, rc ? nullptr : out_counts, cuda_stream);
+  return rc ? rc : rc2;
+}
+
+int streami_streamline_lines(const float* vertices, const unsigned* counts, size_t n, unsigned capacity,
+                             unsigned long long* out_offsets, float* out_points,
+                             unsigned long long* out_total, void* cuda_stream) {
+  if ((n > 0 && !counts) || !out_offsets || capacity == 0 || (n > 0 && out_points && !vertices)) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = scan_counts(counts, n, out_offsets, st);
+  if (rc == STREAMI_OK && out_points && n) {
+    gather_streamlines_kernel<<<148 * 8, 256, 0, st>>>(vertices, counts, n, capacity, out_offsets, out_points);
+    launch_counter()++;
+    rc = check(cudaGetLastError());
+  }
+  if (rc == STREAMI_OK && out_total) {
+    cudaError_t e = cudaMemcpyAsync(out_total, out_offsets + n, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    rc = check(e);
+  }
+  return rc;
 }
 
 int streami_brick_advect(streami_field f, const float* seeds, size_t n,

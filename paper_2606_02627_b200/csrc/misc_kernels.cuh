@@ -138,15 +138,17 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
 }
 
 // out_counts[i] = number of particles of point i alive at the end; copy status to u32.
+// `released` = global steps executed (= nsteps for a complete run): later releases do not exist
+// yet and report status 0; a particle still ALIVE in an unfinished run counts as alive.
 static __global__ void streak_finalize_kernel(const unsigned char* __restrict__ state, unsigned long long m,
-                                       unsigned nsteps, unsigned* __restrict__ counts,
+                                       unsigned nsteps, unsigned released, unsigned* __restrict__ counts,
                                        unsigned* __restrict__ status) {
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= m) return;
   unsigned c = 0;
   for (unsigned j = 0; j < nsteps; ++j) {
-    unsigned st = state[(unsigned long long)j * m + i];
-    c += (st == ST_MAXSTEPS);
+    unsigned st = j < released ? state[(unsigned long long)j * m + i] : 0u;
+    c += (j < released) && (st == ST_MAXSTEPS || st == ST_ALIVE);
     if (status) status[(unsigned long long)j * m + i] = st;
   }
   counts[i] = c;

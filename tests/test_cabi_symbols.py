@@ -54,3 +54,16 @@ def test_product_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text, f
                 assert "streami_oracle" not in text and "liboracle" not in text, f
+
+
+def test_obj_writer(tmp_path):
+    """Host-side OBJ writer of assembled lines (no GPU involved)."""
+    import torch
+    import paper_2606_02627_b200 as S
+    off = torch.tensor([0, 2, 2, 3, 6], dtype=torch.int64)
+    pts = torch.arange(18, dtype=torch.float32).reshape(6, 3)
+    p = tmp_path / "lines.obj"
+    S.write_obj(str(p), off, pts)
+    rows = p.read_text().splitlines()
+    assert rows[0] == "v 0 1 2" and rows[5] == "v 15 16 17"
+    assert rows[6:] == ["l 1 2", "l 4 5 6"]          # empty and single-point lines are skipped

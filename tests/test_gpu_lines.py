@@ -1,0 +1,88 @@
+"""the step-synchronous streakline API (Tracer::step(), Listing 2) with
+per-step snapshots, and polyline assembly (getLines).  After s global steps the slots equal what the
+oracle's A7 returns for nsteps = s; the assembled lines equal oracle/lines.py."""
+import numpy as np
+import pytest
+
+from helpers import gpu_field, gpu_streamlines
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return t
+
+
+@pytest.fixture(scope="module")
+def S(torch):
+    import paper_2606_02627_b200 as s
+    s.lib()
+    return s
+
+
+@pytest.mark.parametrize("window", [0, 3])
+def test_streak_step_snapshots(S, torch, oracle, wl, window):
+    from oracle import lines
+    fld = wl.double_gyre_field(dims=(48, 24, 12), nslices=8, dt=0.25)
+    pts = wl.rake_c4(12, 6)
+    pts[5] = [2.5, 0.2, 0.2]                               # a rake point outside: its particles are born dead
+    m, ns, h = pts.shape[0], 60, 0.05
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+    f = gpu_field(S, torch, fld)
+    d_pts = torch.from_numpy(pts).cuda()
+    verts = torch.zeros((3, ns, m), dtype=torch.float32, device="cuda")
+    status = torch.full((ns * m,), -1, dtype=torch.int32, device="cuda")
+    prm = S.params(integrator=0, h=h, vmin=1e-6, out_status=status)
+    S.streami_set_option("streak_window", window)
+    try:
+        tr = S.Streak(f, d_pts, ns, prm, verts)
+        done = 0
+        for k in (1, 9, 15, 35):                           # snapshots at s = 1, 10, 25, 60
+            tr.step(k)
+            done += k
+            assert tr.position() == done
+            ref = oracle.streaklines(g, pts, done, oracle.params(integrator=0, h=h, vmin=1e-6, max_steps=done), "f32")
+            torch.cuda.synchronize()
+            got = verts.cpu().numpy()[:, :done, :]
+            assert np.array_equal(got.view(np.uint32), ref.vertices.view(np.uint32)), "slots after %d steps" % done
+            off, lp = tr.lines()
+            roff, rp = lines.streak_lines(ref.vertices, ref.status)
+            assert np.array_equal(off.cpu().numpy().astype(np.uint64), roff)
+            assert np.array_equal(lp.cpu().numpy().view(np.uint32), rp.view(np.uint32)), "lines after %d steps" % done
+        tr.step(1000)                                      # clamped
+        assert tr.position() == ns
+        counts = torch.zeros(m, dtype=torch.int32, device="cuda")
+        tr.end(counts)
+        torch.cuda.synchronize()
+        assert np.array_equal(counts.cpu().numpy().astype(np.uint32), ref.counts)
+        assert np.array_equal(status.cpu().numpy().astype(np.uint32), ref.status)
+    finally:
+        S.streami_set_option("streak_window", 0)
+
+
+def test_streamline_lines(S, torch, oracle, wl):
+    from oracle import lines
+    fld = wl.turb_field_cpu(32, 32, 1, 6)
+    n = 5003                                               # several scan tiles and a ragged tail
+    seeds = wl.seeds_uniform(3, n, [31.0] * 3)
+    seeds[7] = [40.0, 1, 1]                                # an empty line
+    kw = dict(integrator=0, h=0.25, max_steps=90, vmin=1e-6, capacity=19, stride=5)
+    f = gpu_field(S, torch, fld)
+    d_seeds = torch.from_numpy(seeds).cuda()
+    verts = torch.full((3, n, 19), float("nan"), dtype=torch.float32, device="cuda")
+    counts = torch.zeros(n, dtype=torch.int32, device="cuda")
+    S.streami_trace_streamlines(f, d_seeds, S.params(**kw), verts, counts)
+    off, pts = S.streami_streamline_lines(verts, counts)
+    torch.cuda.synchronize()
+    ref = oracle.streamlines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), seeds, oracle.params(**kw), "f32")
+    roff, rp = lines.streamline_lines(ref.vertices, ref.counts)
+    assert np.array_equal(off.cpu().numpy().astype(np.uint64), roff)
+    assert np.array_equal(pts.cpu().numpy().view(np.uint32), rp.view(np.uint32))
+    assert int(roff[8]) == int(roff[7])                    # the empty line
+    # n = 0 and offsets-only
+    e_off, e_pts = S.streami_streamline_lines(verts[:, :0, :].contiguous(), counts[:0].contiguous())
+    assert e_off.cpu().tolist() == [0] and e_pts.shape[0] == 0

@@ -538,3 +538,25 @@ def test_p11_streakline_is_pathline_family(oracle, wl, precision):
     assert sk.status[2] == oracle.OUT_OF_DOMAIN and np.array_equal(sk.vertices[:, 0, 2], pts[2])
     # youngest release has taken exactly one step, the oldest nsteps
     assert sk.steps[(nsteps - 1) * len(pts)] == 1 and sk.steps[0] == nsteps
+
+
+def test_lines_assembly_hand_example():
+    """Pin of oracle/lines.py: a hand-written example of the paper's line order (PAPER.md:163:
+    streamlines in step order, streaklines youngest to oldest)."""
+    from oracle import lines
+    v = np.full((3, 3, 4), -1.0, dtype=np.float32)          # 3 particles, capacity 4
+    v[:, 0, :2] = [[1, 2], [10, 20], [100, 200]]            # particle 0: 2 vertices
+    v[:, 2, :3] = [[3, 4, 5], [30, 40, 50], [300, 400, 500]]  # particle 2: 3 vertices, particle 1: none
+    off, pts = lines.streamline_lines(v, np.array([2, 0, 3], dtype=np.uint32))
+    assert off.tolist() == [0, 2, 2, 5]
+    assert pts.tolist() == [[1, 10, 100], [2, 20, 200], [3, 30, 300], [4, 40, 400], [5, 50, 500]]
+    s = np.zeros((3, 3, 2), dtype=np.float32)               # 3 releases, 2 rake points
+    for j in range(3):
+        for i in range(2):
+            s[:, j, i] = [j, i, 10 * j + i]
+    status = np.array([2, 1, 2, 2, 3, 2], dtype=np.uint32)   # (j, i): (0,1) left the domain, (2,0) stagnated
+    off, pts = lines.streak_lines(s, status)
+    assert off.tolist() == [0, 2, 4]
+    assert pts.tolist() == [[1, 0, 10], [0, 0, 0], [2, 1, 21], [1, 1, 11]]   # youngest first
+    off, pts = lines.streak_lines(s, np.array([0, 1, 0, 0, 9, 9], dtype=np.uint32), released=2)
+    assert off.tolist() == [0, 2, 3] and pts.tolist() == [[1, 0, 10], [0, 0, 0], [1, 1, 11]]
