@@ -171,6 +171,18 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream);
 
+/* Seed generation on a control shape (the paper's convenience kernels: "uniformly distributed seed
+ * points given simple control shapes such as planes or lines").  The shape is
+ * origin + u*edge_u + v*edge_v + w*edge_w, (u,v,w) in [0,1)^3, sampled nu x nv x nw times (line:
+ * nv = nw = 1; plane: nw = 1); seed s = (k*nv + j)*nu + i goes to out_seeds [nu*nv*nw][3] (device,
+ * the seeds argument of the trace calls).  mode 0 = lattice at the sub-cell centres
+ * ((i+0.5)/nu, ...), mode 1 = uniformly random from a counter-based generator keyed by rng_seed
+ * (the same seeds for the same key on any launch geometry).  edge pointers are HOST arrays.
+ * Asynchronous on cuda_stream.  Errors: INVALID (null, unknown mode, more than 2^32-1 seeds). */
+int streami_seed_shape(const float origin[3], const float edge_u[3], const float edge_v[3],
+                       const float edge_w[3], unsigned nu, unsigned nv, unsigned nw, int mode,
+                       unsigned long long rng_seed, float* out_seeds, void* cuda_stream);
+
 /* Step-synchronous streaklines: Tracer::step() of Listing 2 ("one advection step
  * ... then a new batch of particles").  _begin binds the rake, the parameters and the caller's
  * slot array out_vertices [3][nsteps][m] (device, as streami_trace_streaklines) and allocates one

@@ -209,3 +209,13 @@ def dp5_tableau(precision="f64"):
     fn.argtypes = [ctypes.c_void_p]
     fn(_p(out))
     return dict(c=out[0:7], a=out[7:28], b=out[28:35], e=out[35:42])
+
+
+def seed_shape(o, eu, ev, ew, nu, nv=1, nw=1, mode=0, rng_seed=0):
+    """Seeds on a line / plane / box; see oracle_capi.cpp for the fp32 formula."""
+    f3 = lambda v: (ctypes.c_float * 3)(*[float(x) for x in v])
+    out = np.empty((nu * nv * nw, 3), dtype=np.float32)
+    fn = lib().oracle_seed_shape_f32
+    fn.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_uint32] * 3 + [ctypes.c_int, ctypes.c_uint64, ctypes.c_void_p]
+    fn(f3(o), f3(eu), f3(ev), f3(ew), nu, nv, nw, mode, rng_seed, _p(out))
+    return out

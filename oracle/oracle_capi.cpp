@@ -311,3 +311,41 @@ extern "C" void oracle_brick_advect_f64(
                      out_final, out_round_counts, max_rounds, out_log, log_capacity, out_nlog,
                      out_nrounds, totals);
 }
+
+// ---------------------------------------------------------------------------------------
+// Seed generation on a control shape (the paper's convenience kernels: "uniformly distributed seed
+// points given simple control shapes such as planes or lines").  The shape is
+// the parallelepiped o + u*eu + v*ev + w*ew, (u,v,w) in [0,1)^3, sampled nu x nv x nw times
+// (a line has nv = nw = 1, a plane nw = 1); seed index s = (k*nv + j)*nu + i.  fp32 formula:
+//   mode 0 (lattice): u = ((float)i + 0.5f) / (float)nu, likewise v, w (IEEE division);
+//   mode 1 (random):  u, v, w = U(s,0), U(s,1), U(s,2) with U(s,a) = (float)(z >> 40) * 2^-24,
+//                     z = splitmix64 finaliser of rng_seed + (3 s + a + 1) * 0x9E3779B97F4A7C15;
+//   p_c = fma(w, ew_c, fma(v, ev_c, fma(u, eu_c, o_c))).
+// ---------------------------------------------------------------------------------------
+static inline uint64_t oracle_mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+extern "C" void oracle_seed_shape_f32(const float o[3], const float eu[3], const float ev[3],
+                                      const float ew[3], uint32_t nu, uint32_t nv, uint32_t nw,
+                                      int mode, uint64_t rng_seed, float* out) {
+  for (uint32_t k = 0; k < nw; ++k)
+    for (uint32_t j = 0; j < nv; ++j)
+      for (uint32_t i = 0; i < nu; ++i) {
+        const uint64_t s = ((uint64_t)k * nv + j) * nu + i;
+        float u, v, w;
+        if (mode == 0) {
+          u = ((float)i + 0.5f) / (float)nu; v = ((float)j + 0.5f) / (float)nv; w = ((float)k + 0.5f) / (float)nw;
+        } else {
+          float r[3];
+          for (int a = 0; a < 3; ++a) {
+            uint64_t z = oracle_mix64(rng_seed + (3ull * s + (uint64_t)a + 1ull) * 0x9E3779B97F4A7C15ull);
+            r[a] = (float)(z >> 40) * 0x1.0p-24f;
+          }
+          u = r[0]; v = r[1]; w = r[2];
+        }
+        for (int c = 0; c < 3; ++c)
+          out[3 * s + c] = std::fma(w, ew[c], std::fma(v, ev[c], std::fma(u, eu[c], o[c])));
+      }
+}

@@ -56,6 +56,7 @@ def lib():
         L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
+        L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
         L.streami_streak_step.argtypes = [P, U, P]
         L.streami_streak_position.argtypes = [P, P]
         L.streami_streak_end.argtypes = [P, P, P]
@@ -265,6 +266,15 @@ def streami_streamline_lines(vertices, counts, stream=None):
     _check(lib().streami_streamline_lines(_ptr(vertices), _ptr(counts), n, cap, _ptr(off), _ptr(pts), None,
                                           _stream(stream)))
     return off, pts
+
+
+def streami_seed_shape(origin, edge_u, edge_v=(0, 0, 0), edge_w=(0, 0, 0), nu=1, nv=1, nw=1, mode=0,
+                       rng_seed=0, stream=None):
+    """Seeds on a line / plane / box; returns a CUDA float32 tensor [nu*nv*nw, 3]."""
+    out = torch.empty((nu * nv * nw, 3), dtype=torch.float32, device="cuda")
+    _check(lib().streami_seed_shape(_f3(origin), _f3(edge_u), _f3(edge_v), _f3(edge_w), nu, nv, nw, int(mode),
+                                    int(rng_seed), _ptr(out), _stream(stream)))
+    return out
 
 
 def _host(t, name):

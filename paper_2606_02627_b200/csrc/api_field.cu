@@ -286,6 +286,23 @@ int streami_sample(streami_field f, const float* points, size_t n, float t, int 
   return STREAMI_OK;
 }
 
+int streami_seed_shape(const float origin[3], const float edge_u[3], const float edge_v[3],
+                       const float edge_w[3], unsigned nu, unsigned nv, unsigned nw, int mode,
+                       unsigned long long rng_seed, float* out_seeds, void* cuda_stream) {
+  if (!origin || !edge_u || !edge_v || !edge_w || (mode != 0 && mode != 1)) return STREAMI_E_INVALID;
+  const unsigned long long total = (unsigned long long)nu * nv * nw;
+  if (total > 0xffffffffull) return STREAMI_E_INVALID;
+  if (total == 0) return STREAMI_OK;
+  if (!out_seeds) return STREAMI_E_INVALID;
+  SeedShape sh;
+  for (int c = 0; c < 3; ++c) { sh.o[c] = origin[c]; sh.eu[c] = edge_u[c]; sh.ev[c] = edge_v[c]; sh.ew[c] = edge_w[c]; }
+  sh.nu = nu; sh.nv = nv; sh.nw = nw; sh.mode = mode; sh.rng_seed = rng_seed;
+  const unsigned blocks = (unsigned)std::min<unsigned long long>((total + 255) / 256, 148ull * 16);
+  seed_shape_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(sh, out_seeds);
+  STREAMI_LAUNCHED();
+  return STREAMI_OK;
+}
+
 int streami_set_option(const char* name, int value) {
   if (!name) return STREAMI_E_INVALID;
   Options& o = options();

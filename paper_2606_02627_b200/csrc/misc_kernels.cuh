@@ -53,6 +53,42 @@ static __global__ void repack_cell_kernel(const float* __restrict__ src, float4*
   }
 }
 
+// ---- seed generation on a control shape (the paper's convenience kernels) ---
+// Shape = o + u*eu + v*ev + w*ew, (u,v,w) in [0,1)^3, nu x nv x nw seeds, s = (k*nv + j)*nu + i.
+// mode 0: lattice, u = ((float)i + 0.5f)/(float)nu (IEEE division).  mode 1: uniform random from a
+// counter-based generator: U(s, a) = (float)(z >> 40) * 2^-24 with z the splitmix64 finaliser of
+// rng_seed + (3 s + a + 1) * 0x9E3779B97F4A7C15.  p_c = fma(w, ew_c, fma(v, ev_c, fma(u, eu_c, o_c))).
+struct SeedShape { float o[3], eu[3], ev[3], ew[3]; unsigned nu, nv, nw; int mode; unsigned long long rng_seed; };
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+static __global__ void seed_shape_kernel(const SeedShape sh, float* __restrict__ out) {
+  const unsigned long long total = (unsigned long long)sh.nu * sh.nv * sh.nw;
+  unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; s < total; s += step) {
+    float u, v, w;
+    if (sh.mode == 0) {
+      const unsigned i = (unsigned)(s % sh.nu), j = (unsigned)((s / sh.nu) % sh.nv),
+                     k = (unsigned)(s / ((unsigned long long)sh.nu * sh.nv));
+      u = __fdiv_rn((float)i + 0.5f, (float)sh.nu); v = __fdiv_rn((float)j + 0.5f, (float)sh.nv);
+      w = __fdiv_rn((float)k + 0.5f, (float)sh.nw);
+    } else {
+      const float S24 = 5.9604644775390625e-08f;   // 2^-24
+      u = (float)(mix64(sh.rng_seed + (3ull * s + 1ull) * 0x9E3779B97F4A7C15ull) >> 40) * S24;
+      v = (float)(mix64(sh.rng_seed + (3ull * s + 2ull) * 0x9E3779B97F4A7C15ull) >> 40) * S24;
+      w = (float)(mix64(sh.rng_seed + (3ull * s + 3ull) * 0x9E3779B97F4A7C15ull) >> 40) * S24;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+      out[3 * s + c] = __fmaf_rn(w, sh.ew[c], __fmaf_rn(v, sh.ev[c], __fmaf_rn(u, sh.eu[c], sh.o[c])));
+  }
+}
+
 // ---- a2-a4 alone ----------------------------------------------------------------------------
 template <int LAYOUT, bool UNSTEADY>
 __global__ void sample_kernel(Geom g, Store s, const float* __restrict__ pts, unsigned long long n,

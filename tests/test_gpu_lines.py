@@ -86,3 +86,17 @@ def test_streamline_lines(S, torch, oracle, wl):
     # n = 0 and offsets-only
     e_off, e_pts = S.streami_streamline_lines(verts[:, :0, :].contiguous(), counts[:0].contiguous())
     assert e_off.cpu().tolist() == [0] and e_pts.shape[0] == 0
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_seed_shape(S, torch, oracle, mode):
+    """Seed-generation kernel against the oracle, bit for bit: line, skewed
+    plane, box; and the seeds feed a trace."""
+    shapes = [((0.5, 1.0, 2.0), (3.0, 0.25, -1.0), (0, 0, 0), (0, 0, 0), 1000, 1, 1),
+              ((1.0, 1.0, 1.0), (2.0, 2.0, 0.0), (0.0, 3.0, 5.0), (0, 0, 0), 37, 91, 1),
+              ((0.0, 0.0, 0.0), (31.0, 0, 0), (0, 31.0, 0), (0, 0, 31.0), 33, 17, 29)]
+    for o, eu, ev, ew, nu, nv, nw in shapes:
+        got = S.streami_seed_shape(o, eu, ev, ew, nu, nv, nw, mode, rng_seed=12345).cpu().numpy()
+        ref = oracle.seed_shape(o, eu, ev, ew, nu, nv, nw, mode, 12345)
+        assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (mode, nu, nv, nw)
+    assert S.streami_seed_shape((0, 0, 0), (1, 0, 0), nu=0).shape[0] == 0

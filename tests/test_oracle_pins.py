@@ -560,3 +560,30 @@ def test_lines_assembly_hand_example():
     assert pts.tolist() == [[1, 0, 10], [0, 0, 0], [2, 1, 21], [1, 1, 11]]   # youngest first
     off, pts = lines.streak_lines(s, np.array([0, 1, 0, 0, 9, 9], dtype=np.uint32), released=2)
     assert off.tolist() == [0, 2, 3] and pts.tolist() == [[1, 0, 10], [0, 0, 0], [1, 1, 11]]
+
+
+def test_seed_shape_pins(oracle):
+    """Lattice seeds have closed forms (dyadic counts: exact); random seeds are checked against
+    what uniformity means (inside the shape, Kolmogorov-Smirnov against U(0,1) with scipy, no
+    repeats, decorrelated axes) and against the degenerate shapes (line: v = w = const offsets)."""
+    from scipy import stats
+    o, eu, ev, ew = (1.0, 2.0, 3.0), (4.0, 0, 0), (0, 2.0, 0), (0, 0, 8.0)
+    p = oracle.seed_shape(o, eu, ev, ew, 4, 2, 8, mode=0)
+    assert p.shape == (64, 3)
+    i, j, k = np.meshgrid(np.arange(4), np.arange(2), np.arange(8), indexing="ij")
+    exp = np.stack([1 + (i + 0.5), 2 + (j + 0.5), 3 + (k + 0.5)], axis=-1).astype(np.float32)
+    got = p.reshape(8, 2, 4, 3).transpose(2, 1, 0, 3)          # index s = (k*nv + j)*nu + i
+    assert np.array_equal(got, exp)
+    # a skewed plane: p = o + u*eu + v*ev exactly in dyadic arithmetic
+    p = oracle.seed_shape((0, 0, 0), (2.0, 2.0, 0), (0, 4.0, 4.0), (9, 9, 9), 2, 4, 1, mode=0)
+    assert np.array_equal(p[0], np.float32([0.5, 1.0, 0.5]) + np.float32([4.5, 4.5, 4.5]))   # w = 0.5 of ew
+    # random mode
+    n = 40000
+    r = oracle.seed_shape((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), n, 1, 1, mode=1, rng_seed=7)
+    assert r.min() >= 0.0 and r.max() < 1.0
+    for c in range(3):
+        assert stats.kstest(r[:, c].astype(np.float64), "uniform").pvalue > 1e-3
+    assert abs(np.corrcoef(r[:, 0], r[:, 1])[0, 1]) < 0.02 and abs(np.corrcoef(r[:-1, 0], r[1:, 0])[0, 1]) < 0.02
+    assert len(np.unique(r.view([("x", "f4"), ("y", "f4"), ("z", "f4")]))) == n
+    r2 = oracle.seed_shape((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), n, 1, 1, mode=1, rng_seed=8)
+    assert not np.array_equal(r, r2)
