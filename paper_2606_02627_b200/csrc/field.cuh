@@ -250,6 +250,40 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
   return 0;
 }
 
+// Branch-free steady sample: the status comes back as a value and the caller decides ONCE per
+// step.  A position that fails the tests is clamped into the store, so the gather stays in bounds
+// and the interpolated value is simply never used (the particle ends in this step).  Early
+// returns cost more than they save here: every exit of the inlined step has to move the live
+// particle state into the registers of the merge point (measured: ~120 MOV/IMAD.MOV per
+// warp-iteration in the r1 kernel).  The arithmetic of a passing sample is unchanged.
+template <int LAYOUT, bool BRICK, bool CACHE, bool UNIT, bool KNOWN>
+__device__ __forceinline__ unsigned sample_nb(const Geom& g, const Store& s, CellCache& cc, float px,
+                                              float py, float pz, float& vx, float& vy, float& vz) {
+  float gx, gy, gz;
+  index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
+  unsigned rc = 0;
+  if (BRICK) {
+    const bool served = (gx >= s.flox) && (gx < s.fhix) && (gy >= s.floy) && (gy < s.fhiy) &&
+                        (gz >= s.floz) && (gz < s.fhiz);
+    rc = served ? 0u : (unsigned)ST_HALO;
+  }
+  if (!KNOWN) rc = in_domain(g, gx, gy, gz) ? rc : (unsigned)ST_OUT;      // OUT wins over HALO (A9)
+  int ix = min(__float2int_rz(gx), s.cmx), iy = min(__float2int_rz(gy), s.cmy), iz = min(__float2int_rz(gz), s.cmz);
+  if (!KNOWN || BRICK) { ix = max(ix, BRICK ? s.lox : 0); iy = max(iy, BRICK ? s.loy : 0); iz = max(iz, BRICK ? s.loz : 0); }
+  const float fx = gx - (float)ix, fy = gy - (float)iy, fz = gz - (float)iz;
+  if (BRICK) { ix -= s.lox; iy -= s.loy; iz -= s.loz; }
+  const unsigned v32 = (unsigned)iz * s.nxy + (unsigned)iy * s.nx + (unsigned)ix;
+  if (CACHE) {
+    if (v32 != cc.key) { load_cell32<LAYOUT>(s, v32, cc.V); cc.key = v32; }
+    interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, vx, vy, vz);
+  } else {
+    float V[24];
+    load_cell32<LAYOUT>(s, v32, V);
+    interp_cell<LayoutTraits<LAYOUT>::DIFF>(V, fx, fy, fz, vx, vy, vz);
+  }
+  return rc;
+}
+
 // ---- one-step-ahead cell prefetch (build's choice; results unchanged) ------------------------
 // The first touch of a new cell stalls the whole warp for an L2/DRAM round trip, and it happens
 // mid-step (stage 2 or 4), where the lane has nothing else to do.  At the END of a step the next
