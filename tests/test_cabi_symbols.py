@@ -67,3 +67,42 @@ def test_obj_writer(tmp_path):
     rows = p.read_text().splitlines()
     assert rows[0] == "v 0 1 2" and rows[5] == "v 15 16 17"
     assert rows[6:] == ["l 1 2", "l 4 5 6"]          # empty and single-point lines are skipped
+
+
+def test_argument_validation_without_a_gpu():
+    """Host logic of the boundary: every entry point rejects bad arguments with STREAMI_E_INVALID
+    before it touches CUDA (so this runs on a CPU-only box), and the option table round-trips."""
+    import ctypes
+    import paper_2606_02627_b200 as S
+    L = S.lib()
+    NULL = None
+    h = ctypes.c_void_p(None)
+    i3 = (ctypes.c_int * 3)(4, 4, 4); f3 = (ctypes.c_float * 3)(0, 0, 0); s3 = (ctypes.c_float * 3)(1, 1, 1)
+    bad_sp = (ctypes.c_float * 3)(1, -1, 1)
+    dummy = ctypes.c_void_p(16)                                   # never dereferenced on these paths
+    assert L.streami_field_create(NULL, f3, s3, 1, 1.0, dummy, 0, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_field_create(i3, f3, bad_sp, 1, 1.0, dummy, 0, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_field_create(i3, f3, s3, 0, 1.0, dummy, 0, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_field_create(i3, f3, s3, 1, 1.0, dummy, 99, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_field_create(i3, f3, s3, 1, 1.0, NULL, 0, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_field_destroy(NULL) == S.E_INVALID
+    prm = S.Params()
+    assert L.streami_trace_streamlines(NULL, dummy, 8, ctypes.byref(prm), NULL, dummy, NULL) == S.E_INVALID
+    assert L.streami_trace_streaklines(NULL, dummy, 8, 8, ctypes.byref(prm), dummy, dummy, NULL) == S.E_INVALID
+    assert L.streami_brick_advect(NULL, dummy, 8, ctypes.byref(prm), NULL, dummy, NULL, 0, NULL, 0, NULL, NULL, NULL) == S.E_INVALID
+    assert L.streami_streak_begin(NULL, dummy, 8, 8, ctypes.byref(prm), dummy, NULL, ctypes.byref(h)) == S.E_INVALID
+    assert L.streami_streak_step(NULL, 1, NULL) == S.E_INVALID
+    assert L.streami_streak_end(NULL, NULL, NULL) == S.E_INVALID
+    assert L.streami_streamline_lines(dummy, dummy, 8, 0, dummy, NULL, NULL, NULL) == S.E_INVALID   # capacity 0
+    assert L.streami_streamline_lines(dummy, dummy, 8, 4, NULL, NULL, NULL, NULL) == S.E_INVALID
+    assert L.streami_seed_shape(NULL, f3, f3, f3, 2, 2, 2, 0, 0, dummy, NULL) == S.E_INVALID
+    assert L.streami_seed_shape(f3, f3, f3, f3, 2, 2, 2, 7, 0, dummy, NULL) == S.E_INVALID          # unknown mode
+    assert L.streami_seed_shape(f3, f3, f3, f3, 0, 2, 2, 0, 0, NULL, NULL) == S.OK                  # no seeds: nothing to do
+    assert L.streami_set_option(b"no_such_option", 1) == S.E_INVALID
+    for name, v in (("segment_steps", 17), ("prefetch", 2), ("vertex_staging", 0), ("max_blocks_per_sm", 2),
+                    ("brick_round_steps", -1), ("presort", 0), ("cell_cache", 0)):
+        old = S.streami_get_option(name)
+        S.streami_set_option(name, v)
+        assert S.streami_get_option(name) == v, name
+        S.streami_set_option(name, old)
+    assert L.streami_error_string(-4).startswith(b"hand-off log")
