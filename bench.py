@@ -520,6 +520,8 @@ def main():
                 if row["workload"] == args.workload:
                     roofline["traffic"] = float(row["dram_bytes_per_launch"])
                     roofline["traffic_source"] = row["source"]
+                    roofline["ncu"] = {k: float(v) for k, v in row.items()
+                                       if k not in ("workload", "source", "dram_bytes_per_launch")}
 
     cpu = None
     if world == 1 and not args.no_cpu and job.host_field is not None:
