@@ -76,3 +76,24 @@ def test_dp5_schedule_options(S, torch, oracle, wl, turb48, layout, opts):
     out = _with(S, opts, lambda: gpu_streamlines(S, torch, f, seeds, **kw))
     assert_same(out, ref, "dp5 %s" % opts)
     assert int(ref.totals[0]) > int(ref.totals[1]), "the case must contain rejected attempts"
+
+
+def test_unaligned_vertex_array_uses_scalar_stores(S, torch, oracle, wl, turb48):
+    """The full-sector vertex stores need a 32-byte aligned out_vertices and capacity % 8 == 0; an
+    array that starts 4 bytes off must take the scalar path and give the same vertices."""
+    n, cap = 4099, 24
+    seeds = wl.seeds_uniform(13, n, [47.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=100, vmin=1e-6, capacity=cap, stride=2)
+    ref = oracle.streamlines(oracle.grid(turb48.data, turb48.dims, turb48.origin, turb48.spacing),
+                             seeds, oracle.params(**kw), "f32")
+    f = gpu_field(S, torch, turb48)
+    flat = torch.full((3 * n * cap + 8,), float("nan"), dtype=torch.float32, device="cuda")
+    for shift in (0, 1):
+        verts = flat[shift:shift + 3 * n * cap].view(3, n, cap)
+        assert verts.data_ptr() % 32 == 4 * shift and verts.is_contiguous()
+        counts = torch.zeros(n, dtype=torch.int32, device="cuda")
+        flat.fill_(float("nan"))
+        S.streami_trace_streamlines(f, torch.from_numpy(seeds).cuda(), S.params(**kw), verts, counts)
+        torch.cuda.synchronize()
+        assert np.array_equal(counts.cpu().numpy().astype(np.uint32), ref.counts)
+        assert np.array_equal(verts.cpu().numpy().view(np.uint32), ref.vertices.view(np.uint32)), shift
