@@ -127,7 +127,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
-    ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 packed3, 2 float4, 3 xpair, 4 cell")
+    ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 packed3, 2 float4, 3 xpair, 4 cell, 5 xyquad")
     ap.add_argument("--opt", action="append", default=[], help="library option name=value")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -531,7 +531,7 @@ def main():
                "sample": "every %d-th particle of the same workload (%d particles, %d step attempts, %.1f s)"
                          % (stride, npart, a, dt)}
 
-    lay = {1: "packed3", 2: "float4", 3: "xpair", 4: "cell"}.get(job.layout, str(job.layout))
+    lay = {1: "packed3", 2: "float4", 3: "xpair", 4: "cell", 5: "xyquad"}.get(job.layout, str(job.layout))
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

@@ -59,6 +59,8 @@ extern "C" {
 #define STREAMI_LAYOUT_FLOAT4  2   /* library-owned copy padded to 16 B per vertex */
 #define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: {V[x], V[x+1], pad}: one
                                       aligned sector per trilinear row */
+#define STREAMI_LAYOUT_XYQUAD  5   /* library-owned copy, 64 B per vertex: the XPAIR rows (x, y) and (x, y+1):
+                                      a cell is two aligned 64-byte pieces (4x the packed size) */
 #define STREAMI_LAYOUT_CELL    4   /* library-owned copy, 128 B per CELL: its 8 corner vertices in one
                                       aligned L2 line (8x the packed size) */
 

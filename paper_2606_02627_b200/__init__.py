@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 OK, E_INVALID, E_NOMEM, E_CUDA, E_TRUNCATED = 0, -1, -2, -3, -4
 OUT_OF_DOMAIN, MAX_STEPS, STAGNANT, HALO_MISS = 1, 2, 3, 4
-LAYOUT_AUTO, LAYOUT_PACKED3, LAYOUT_FLOAT4, LAYOUT_XPAIR, LAYOUT_CELL = 0, 1, 2, 3, 4
+LAYOUT_AUTO, LAYOUT_PACKED3, LAYOUT_FLOAT4, LAYOUT_XPAIR, LAYOUT_CELL, LAYOUT_XYQUAD = 0, 1, 2, 3, 4, 5
 
 
 class StreamiError(RuntimeError):

@@ -70,7 +70,7 @@ static unsigned long long layout_records(int layout, unsigned nx, unsigned ny, u
   return (unsigned long long)nx * ny * nz * nslices;
 }
 static size_t layout_record_bytes(int layout) {
-  return layout == LAYOUT_FLOAT4 ? 16 : (layout == LAYOUT_XPAIR ? 32 : (layout == LAYOUT_CELL ? 128 : 12));
+  return layout == LAYOUT_FLOAT4 ? 16 : (layout == LAYOUT_XPAIR ? 32 : (layout == LAYOUT_CELL ? 128 : (layout == LAYOUT_XYQUAD ? 64 : 12)));
 }
 
 // Build the library-owned copy of one packed float3 array (stored box nx*ny*nz, nslices slices).
@@ -88,6 +88,8 @@ static int repack(const float* src, unsigned nx, unsigned ny, unsigned nz, unsig
     repack_float4_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert);
   else if (layout == LAYOUT_XPAIR)
     repack_xpair_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert, nx);
+  else if (layout == LAYOUT_XYQUAD)
+    repack_xyquad_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert, nx, ny);
   else
     repack_cell_kernel<<<blocks, 256>>>(src, (float4*)dst, nx, ny, nz, nslices);
   launch_counter()++;
@@ -123,10 +125,22 @@ static int fill_geom(Geom& g, const int dims[3], const float origin[3], const fl
   return STREAMI_OK;
 }
 
+// AUTO: XPAIR; for a steady field of 1 GiB or more of packed vertices --
+// far beyond L2, where the gathers are bound by DRAM accesses (C5) -- XYQUAD, whose 64-byte pieces
+// use both halves of every DRAM fetch, provided its 64 B per vertex fit comfortably.
+static int auto_layout(unsigned long long nvert, int nslices) {
+  if (nslices == 1 && 12ull * nvert >= (1ull << 30)) {
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && 64ull * nvert <= free_b / 2) return LAYOUT_XYQUAD;
+    cudaGetLastError();
+  }
+  return LAYOUT_XPAIR;
+}
+
 static int pick_layout(int hint) {
-  if (hint == STREAMI_LAYOUT_AUTO) return LAYOUT_XPAIR;   // measured fastest
+  if (hint == STREAMI_LAYOUT_AUTO) return 0;              // decided per stored array (auto_layout)
   if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR ||
-      hint == STREAMI_LAYOUT_CELL)
+      hint == STREAMI_LAYOUT_CELL || hint == STREAMI_LAYOUT_XYQUAD)
     return hint;
   return -1;
 }
@@ -157,6 +171,8 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
+  if (layout == 0) layout = auto_layout(s.slice_stride, nslices);
+  f->layout = layout;
   rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
   if (rc) { delete f; return rc; }
   if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
@@ -175,6 +191,9 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
   *out = nullptr;
   int layout = pick_layout(layout_hint);
   if (layout < 0 || ghost_cells < 1) return STREAMI_E_INVALID;
+  if (layout == 0) {       // one layout for all bricks (one kernel serves them): decided on the whole grid
+    layout = auto_layout((unsigned long long)global_dims[0] * global_dims[1] * global_dims[2], 1);
+  }
   for (int a = 0; a < 3; ++a)
     if (brick_grid[a] < 1 || brick_grid[a] > global_dims[a] - 1) return STREAMI_E_INVALID;
   const int nb = brick_grid[0] * brick_grid[1] * brick_grid[2];
@@ -279,7 +298,9 @@ int streami_sample(streami_field f, const float* points, size_t n, float t, int 
     case LAYOUT_XPAIR * 2: GO(LAYOUT_XPAIR, false); break;
     case LAYOUT_XPAIR * 2 + 1: GO(LAYOUT_XPAIR, true); break;
     case LAYOUT_CELL * 2: GO(LAYOUT_CELL, false); break;
-    default: GO(LAYOUT_CELL, true); break;
+    case LAYOUT_CELL * 2 + 1: GO(LAYOUT_CELL, true); break;
+    case LAYOUT_XYQUAD * 2: GO(LAYOUT_XYQUAD, false); break;
+    default: GO(LAYOUT_XYQUAD, true); break;
   }
 #undef GO
   STREAMI_LAUNCHED();

@@ -24,6 +24,7 @@ static StreakKernel pick_streak(int layout, bool unsteady) {
     case LAYOUT_PACKED3: return unsteady ? streak_kernel<LAYOUT_PACKED3, true> : streak_kernel<LAYOUT_PACKED3, false>;
     case LAYOUT_FLOAT4: return unsteady ? streak_kernel<LAYOUT_FLOAT4, true> : streak_kernel<LAYOUT_FLOAT4, false>;
     case LAYOUT_CELL: return unsteady ? streak_kernel<LAYOUT_CELL, true> : streak_kernel<LAYOUT_CELL, false>;
+    case LAYOUT_XYQUAD: return unsteady ? streak_kernel<LAYOUT_XYQUAD, true> : streak_kernel<LAYOUT_XYQUAD, false>;
     default: return unsteady ? streak_kernel<LAYOUT_XPAIR, true> : streak_kernel<LAYOUT_XPAIR, false>;
   }
 }

@@ -30,6 +30,7 @@ TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, 
     case LAYOUT_PACKED3: return pick_l<LAYOUT_PACKED3>(integ, unsteady, brick, cache, unit);
     case LAYOUT_FLOAT4: return pick_l<LAYOUT_FLOAT4>(integ, unsteady, brick, cache, unit);
     case LAYOUT_CELL: return pick_l<LAYOUT_CELL>(integ, unsteady, brick, cache, unit);
+    case LAYOUT_XYQUAD: return pick_l<LAYOUT_XYQUAD>(integ, unsteady, brick, cache, unit);
     default: return pick_l<LAYOUT_XPAIR>(integ, unsteady, brick, cache, unit);
   }
 }

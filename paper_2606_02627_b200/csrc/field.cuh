@@ -12,7 +12,7 @@
 
 namespace streami {
 
-enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3, LAYOUT_CELL = 4 };
+enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3, LAYOUT_CELL = 4, LAYOUT_XYQUAD = 5 };
 enum : unsigned { ST_ALIVE = 0, ST_OUT = 1, ST_MAXSTEPS = 2, ST_STAGNANT = 3, ST_HALO = 4 };
 
 // Global geometry (A1), uniform over the launch.
@@ -100,10 +100,31 @@ template <> struct CellLoad<LAYOUT_CELL> {
   }
 };
 
+// LAYOUT_XYQUAD: one aligned 64-byte record per VERTEX = the XPAIR rows (x, y) and (x, y+1) back to
+// back: a cell is two 64-byte pieces (z and z+1).  DRAM brings 64 bytes per missed 32-byte sector
+// (ncu on C5: 3.7 TB read for 1.8 TB of missed sectors); here both halves of every fetch are used.
+template <> struct CellLoad<LAYOUT_XYQUAD> {
+  static __device__ __forceinline__ void pair(const void* data, unsigned long long v, float* o) {
+    const char* p = reinterpret_cast<const char*>(data) + 64ull * v;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      float p6, p7;
+      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=f"(o[6 * r]), "=f"(o[6 * r + 1]), "=f"(o[6 * r + 2]), "=f"(o[6 * r + 3]),
+                     "=f"(o[6 * r + 4]), "=f"(o[6 * r + 5]), "=f"(p6), "=f"(p7)
+                   : "l"(p + 32 * r));
+      (void)p6; (void)p7;
+    }
+  }
+};
+
 template <int LAYOUT>
 __device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, float* V) {
   if constexpr (LAYOUT == LAYOUT_CELL) {
     CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+  } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
+    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v, V);
+    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v + s.nxy, V + 12);
   } else {
     CellLoad<LAYOUT>::row(s.data, v, V);
     CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
@@ -118,6 +139,9 @@ template <int LAYOUT>
 __device__ __forceinline__ void load_cell32(const Store& s, unsigned v, float* V) {
   if constexpr (LAYOUT == LAYOUT_CELL) {
     CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+  } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
+    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v, V);
+    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v + s.nxy, V + 12);
   } else {
     CellLoad<LAYOUT>::row(s.data, v, V);
     CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
@@ -130,7 +154,7 @@ __device__ __forceinline__ void load_cell32(const Store& s, unsigned v, float* V
 // the x-lerp, lerp(a, b, w) = fma(w, b - a, a), does not depend on the sample point, so the
 // repack does it once per vertex pair (the same fp32 operation, the same bits) and every sample
 // saves 12 of its 42 interpolation instructions.
-template <int LAYOUT> struct LayoutTraits { static constexpr bool DIFF = LAYOUT == LAYOUT_XPAIR || LAYOUT == LAYOUT_CELL; };
+template <int LAYOUT> struct LayoutTraits { static constexpr bool DIFF = LAYOUT == LAYOUT_XPAIR || LAYOUT == LAYOUT_CELL || LAYOUT == LAYOUT_XYQUAD; };
 
 // A2.5: x first, then y, then z; 7 lerps per component.
 template <bool DIFF>
@@ -301,6 +325,12 @@ __device__ __forceinline__ void prefetch_cell32(const Store& s, unsigned v, unsi
     const char* p = reinterpret_cast<const char*>(s.data) + 128ull * v;
 #pragma unroll
     for (int r = 0; r < 4; ++r) prefetch_sector(p + 32 * r, smem_addr);
+  } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
+    const char* p = reinterpret_cast<const char*>(s.data);
+    prefetch_sector(p + 64ull * v, smem_addr);
+    prefetch_sector(p + 64ull * v + 32, smem_addr);
+    prefetch_sector(p + 64ull * (v + s.nxy), smem_addr);
+    prefetch_sector(p + 64ull * (v + s.nxy) + 32, smem_addr);
   } else {
     constexpr unsigned long long REC = LAYOUT == LAYOUT_XPAIR ? 32ull : (LAYOUT == LAYOUT_FLOAT4 ? 16ull : 12ull);
     const char* p = reinterpret_cast<const char*>(s.data);

@@ -30,6 +30,24 @@ static __global__ void repack_xpair_kernel(const float* __restrict__ src, float4
   }
 }
 
+// XYQUAD record v = {XPAIR row of vertex v, XPAIR row of the vertex one y-row up}: 64 bytes.  The
+// last x of a row and the last y-row of a plane pair with themselves (never used: i <= N-2).
+static __global__ void repack_xyquad_kernel(const float* __restrict__ src, float4* __restrict__ dst,
+                                            unsigned long long nvert, unsigned nx, unsigned ny) {
+  unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;   // (vertex, half)
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; t < 2ull * nvert; t += step) {
+    unsigned long long v = t >> 1;
+    const unsigned x = (unsigned)(v % nx), y = (unsigned)((v / nx) % ny);
+    if ((t & 1ull) && y + 1 < ny) v += nx;
+    const unsigned long long w = (x == nx - 1) ? v : v + 1;
+    const float a0 = src[3 * v], a1 = src[3 * v + 1], a2 = src[3 * v + 2];
+    const float b0 = src[3 * w], b1 = src[3 * w + 1], b2 = src[3 * w + 2];
+    dst[2 * t] = make_float4(a0, a1, a2, b0 - a0);
+    dst[2 * t + 1] = make_float4(b1 - a1, b2 - a2, 0.0f, 0.0f);
+  }
+}
+
 // CELL record c = the four XPAIR rows (dz*2+dy) of cell c back to back: 128 bytes, 8 corners.
 // One thread per (cell, row): 6 source floats in, 32 bytes out; consecutive threads write
 // consecutive 32-byte pieces.
