@@ -54,7 +54,9 @@ extern "C" {
 #define STREAMI_HALO_MISS      4u  /* bricks only: a stage point left the brick's stored box */
 
 /* field layouts (layout_hint of streami_field_create*, reported by streami_field_info) */
-#define STREAMI_LAYOUT_AUTO    0   /* library chooses (DESIGN.md section 6 says how) */
+#define STREAMI_LAYOUT_AUTO    0   /* library chooses: XPAIR; XYQUAD for steady fields of
+                                      1 GiB or more when it fits half the free device memory; falls back to a
+                                      smaller layout instead of failing with NOMEM */
 #define STREAMI_LAYOUT_PACKED3 1   /* use the caller's packed float3 array in place (the paper's layout) */
 #define STREAMI_LAYOUT_FLOAT4  2   /* library-owned copy padded to 16 B per vertex */
 #define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: {V[x], V[x+1], pad}: one

@@ -171,9 +171,18 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
-  if (layout == 0) layout = auto_layout(s.slice_stride, nslices);
-  f->layout = layout;
+  const bool automatic = layout == 0;
+  if (automatic) layout = auto_layout(s.slice_stride, nslices);
   rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
+  if (rc == STREAMI_E_NOMEM && automatic && layout != LAYOUT_XPAIR) {     // AUTO never fails for its own ambition
+    layout = LAYOUT_XPAIR;
+    rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
+  }
+  if (rc == STREAMI_E_NOMEM && automatic) {                               // last resort: the caller's array in place
+    layout = LAYOUT_PACKED3;
+    rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
+  }
+  f->layout = layout;
   if (rc) { delete f; return rc; }
   if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
   s.data = data;
