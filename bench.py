@@ -12,7 +12,8 @@ recording (capacity 256, stride 8).
 
 metric  = RK particle-steps per second (step ATTEMPTS), whole job over all ranks.
 value   = device-resident inputs, CUDA events on the launching stream around each step.
-e2e     = the same through the C-ABI *_host calls with pinned HOST buffers
+e2e     = the same through the C-ABI *_host calls with pinned HOST buffers (streamlines: seeds in,
+          assembled polylines out -- streami_trace_streamlines_lines_host)
           (H2D of the seeds and D2H of every output inside the timed region).
 roofline= the advection kernel alone (event pair recorded by the library around its launch):
           algorithmic bytes / its duration, against MEASURED_PEAKS.json.
@@ -243,6 +244,12 @@ class Job:
                           counts=pin(self.counts), steps=pin(self.steps_o), status=pin(self.status_o),
                           final=None if self.final_o is None else pin(self.final_o),
                           totals=t.zeros(4, dtype=t.int64).pin_memory())
+            if self.kind != "gyre":
+                # polyline buffers instead of the capacity-padded slot array
+                self.h["verts"] = None; self.h["counts"] = None
+                self.h["offsets"] = t.zeros(self.n + 1, dtype=t.int64).pin_memory()
+                self.h["points"] = t.empty((self.n * self.w["prm"]["capacity"], 3), dtype=t.float32).pin_memory()
+                self.e2e_points = 0
             kw = dict(self.w["prm"])
             self.prm_h = self.S.params(out_steps=None, out_status=None, out_final=None, out_totals=None, **kw)
             self.prm_h.out_steps = self.h["steps"].data_ptr()
@@ -257,6 +264,8 @@ class Job:
         nb = lambda x: 0 if x is None else x.numel() * x.element_size()
         bi = nb(h["seeds"])
         bo = sum(nb(h[k]) for k in ("verts", "counts", "steps", "status", "final", "totals"))
+        if self.kind != "gyre":                        # offsets + the points actually delivered
+            bo += nb(h["offsets"]) + 12 * int(self.e2e_points)
         return bi, bo
 
     def step_host(self):
@@ -265,10 +274,11 @@ class Job:
         h, S = self._pinned(), self.S
         if self.kind == "gyre":
             S.streami_trace_streaklines_host(self.field, h["seeds"], self.nsteps, self.prm_h, h["verts"], h["counts"])
-        elif self.kind == "bricks":
-            S.streami_brick_advect_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
         else:
-            S.streami_trace_streamlines_host(self.field, h["seeds"], self.prm_h, h["verts"], h["counts"])
+            # streamlines: the host application's end product is the assembled polylines (the paper's
+            # getLines): offsets + points; only stored vertices cross the bus
+            self.e2e_points, _ = S.streami_trace_streamlines_lines_host(self.field, h["seeds"], self.prm_h,
+                                                                        h["offsets"], h["points"])
 
     def work(self):
         """(attempted steps, accepted steps, field samples, hand-offs, stored vertices) of the
@@ -482,8 +492,8 @@ def main():
     # ---- e2e: host buffers, copies inside the timed region --------------------------------------
     e2e = None
     if not args.no_e2e:
-        bi, bo = job.e2e_bytes()
         job.step_host()
+        bi, bo = job.e2e_bytes()
         barrier()
         w0 = time.perf_counter()
         for _ in range(args.steps):

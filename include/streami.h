@@ -221,6 +221,18 @@ int streami_streamline_lines(const float* vertices, const unsigned* counts, size
 int streami_streak_lines(streami_streak s, unsigned long long* out_offsets, float* out_points,
                          unsigned long long* out_total, void* cuda_stream);
 
+/* Streamlines end to end for a host application: seeds (host) in, assembled polylines (host) out
+ * (f may be a monolithic or a bricked field: streami_trace_streamlines or streami_brick_advect runs):
+ * out_offsets [n+1] u64 and out_points [max_points][3]; only the stored vertices cross the bus, not
+ * the capacity-padded slot array.  params->capacity/stride select the vertices as usual; the
+ * optional outputs in params are host pointers.  *out_total (host, may be NULL) = points of all
+ * lines.  Synchronises cuda_stream (twice: the total sizes the device buffer).  Returns
+ * STREAMI_E_TRUNCATED if total > max_points (the first max_points points are then delivered). */
+int streami_trace_streamlines_lines_host(streami_field f, const float* seeds, size_t n,
+                                         const streami_params* params, unsigned long long* out_offsets,
+                                         float* out_points, unsigned long long max_points,
+                                         unsigned long long* out_total, void* cuda_stream);
+
 /* streami_trace_streaklines / streami_brick_advect with HOST buffers (points/seeds, out_vertices,
  * out_counts, the optional outputs in params, the round table, the log and its count are host
  * pointers; pinned memory makes the copies faster but is not required): copy host->device, run,

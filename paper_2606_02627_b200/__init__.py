@@ -57,6 +57,7 @@ def lib():
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
+        L.streami_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
         L.streami_streak_step.argtypes = [P, U, P]
         L.streami_streak_position.argtypes = [P, P]
         L.streami_streak_end.argtypes = [P, P, P]
@@ -275,6 +276,21 @@ def streami_seed_shape(origin, edge_u, edge_v=(0, 0, 0), edge_w=(0, 0, 0), nu=1,
     _check(lib().streami_seed_shape(_f3(origin), _f3(edge_u), _f3(edge_v), _f3(edge_w), nu, nv, nw, int(mode),
                                     int(rng_seed), _ptr(out), _stream(stream)))
     return out
+
+
+def streami_trace_streamlines_lines_host(field, seeds, prm_host, out_offsets, out_points, stream=None):
+    """Host seeds in, host polylines out (offsets int64 [n+1], points float32 [max_points, 3]).
+    Returns (total_points, truncated)."""
+    for t, nm in ((seeds, "seeds"), (out_offsets, "out_offsets"), (out_points, "out_points")):
+        if t is not None and (t.is_cuda or not t.is_contiguous()):
+            raise ValueError("%s: contiguous CPU tensor expected" % nm)
+    total = ctypes.c_ulonglong(0)
+    rc = _check(lib().streami_trace_streamlines_lines_host(field.handle, _ptr(seeds), seeds.shape[0],
+                                                           ctypes.byref(prm_host), _ptr(out_offsets),
+                                                           _ptr(out_points), out_points.shape[0],
+                                                           ctypes.byref(total), _stream(stream)),
+                allow=(E_TRUNCATED,))
+    return total.value, rc == E_TRUNCATED
 
 
 def _host(t, name):

@@ -64,6 +64,21 @@ void timing_end(cudaStream_t st) {
 
 static bool finite_pos(float x) { return std::isfinite(x) && x > 0.0f; }
 
+// Scratch comes from the stream-ordered allocator.  Its default pool hands freed memory back to
+// the driver at every synchronisation (release threshold 0), so a call that needs gigabytes of
+// scratch (the host-buffer variants) would pay for fresh mappings each time; keep it cached.
+static void keep_pool_cached() {
+  static std::once_flag once;
+  std::call_once(once, [] {
+    int dev = 0; cudaMemPool_t pool = nullptr;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      unsigned long long keep = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    cudaGetLastError();
+  });
+}
+
 // Records of the library-owned copy of a stored box of nx*ny*nz vertices x nslices.
 static unsigned long long layout_records(int layout, unsigned nx, unsigned ny, unsigned nz, unsigned nslices) {
   if (layout == LAYOUT_CELL) return (unsigned long long)(nx - 1) * (ny - 1) * (nz - 1) * nslices;
@@ -158,6 +173,7 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   *out = nullptr;
   int layout = pick_layout(layout_hint);
   if (layout < 0) return STREAMI_E_INVALID;
+  keep_pool_cached();
   streami_field_s* f = new streami_field_s();
   int rc = fill_geom(f->g, dims, origin, spacing, nslices, slice_dt);
   if (rc) { delete f; return rc; }
@@ -207,6 +223,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
     if (brick_grid[a] < 1 || brick_grid[a] > global_dims[a] - 1) return STREAMI_E_INVALID;
   const int nb = brick_grid[0] * brick_grid[1] * brick_grid[2];
   if (nb > 65535) return STREAMI_E_INVALID;   // the hand-off log packs dest into 16 bits
+  keep_pool_cached();
   streami_field_s* f = new streami_field_s();
   int rc = fill_geom(f->g, global_dims, origin, spacing, 1, 1.0f);
   if (rc) { delete f; return rc; }

@@ -414,3 +414,57 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
 }
 
 }  // extern "C"
+
+extern "C" {
+
+// Streamlines end to end for a host application: seeds in host memory in, assembled polylines
+// (offsets + AoS points, the paper's getLines) in host memory out.  Only the stored vertices cross
+// the bus, not the capacity-padded slot array.
+int streami_trace_streamlines_lines_host(streami_field f, const float* seeds, size_t n,
+                                         const streami_params* params, unsigned long long* out_offsets,
+                                         float* out_points, unsigned long long max_points,
+                                         unsigned long long* out_total, void* cuda_stream) {
+  if (!f || !params || !out_offsets || (n > 0 && !seeds) || (max_points > 0 && !out_points)) return STREAMI_E_INVALID;
+  if (params->capacity == 0) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (out_total) *out_total = 0;
+  if (n == 0) { out_offsets[0] = 0; return STREAMI_OK; }
+  int rc;
+  unsigned long long total = 0;
+  {
+    Mirror mr(st);
+    streami_params dp = *params;
+    float* d_seeds = (float*)mr.make(seeds, nullptr, 3 * n * sizeof(float));
+    dp.out_steps = (unsigned*)mr.make(nullptr, params->out_steps, n * sizeof(unsigned));
+    dp.out_status = (unsigned*)mr.make(nullptr, params->out_status, n * sizeof(unsigned));
+    dp.out_final = (float*)mr.make(nullptr, params->out_final, 3 * n * sizeof(float));
+    dp.out_totals = (unsigned long long*)mr.make(nullptr, params->out_totals, 4 * sizeof(unsigned long long));
+    unsigned long long* d_off = (unsigned long long*)mr.make(nullptr, out_offsets, (n + 1) * sizeof(unsigned long long));
+    if (mr.err != cudaSuccess) return check(mr.err);
+    float* d_v = nullptr; unsigned* d_c = nullptr; float* d_pts = nullptr;
+    cudaError_t e = cudaMallocAsync((void**)&d_v, 3 * n * (size_t)params->capacity * sizeof(float), st);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&d_c, n * sizeof(unsigned), st);
+    auto drop = [&]() { if (d_v) cudaFreeAsync(d_v, st); if (d_c) cudaFreeAsync(d_c, st); if (d_pts) cudaFreeAsync(d_pts, st); };
+    if (e != cudaSuccess) { drop(); return check(e); }
+    rc = f->bricked ? streami_brick_advect(f, d_seeds, n, &dp, d_v, d_c, nullptr, 0, nullptr, 0, nullptr, nullptr,
+                                           cuda_stream)
+                    : streami_trace_streamlines(f, d_seeds, n, &dp, d_v, d_c, cuda_stream);
+    if (rc == STREAMI_OK) rc = streami_streamline_lines(d_v, d_c, n, params->capacity, d_off, nullptr, &total, cuda_stream);
+    if (rc == STREAMI_OK && total > 0) {
+      e = cudaMallocAsync((void**)&d_pts, 3 * total * sizeof(float), st);
+      if (e != cudaSuccess) { drop(); return check(e); }
+      rc = streami_streamline_lines(d_v, d_c, n, params->capacity, d_off, d_pts, nullptr, cuda_stream);
+      const unsigned long long copy = total < max_points ? total : max_points;
+      if (rc == STREAMI_OK && copy)
+        rc = check(cudaMemcpyAsync(out_points, d_pts, 3 * copy * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
+    if (rc == STREAMI_OK && mr.download() != cudaSuccess) rc = check(mr.err);
+    drop();
+  }
+  if (rc == STREAMI_OK) rc = check(cudaStreamSynchronize(st));
+  if (out_total) *out_total = total;
+  if (rc == STREAMI_OK && total > max_points) rc = STREAMI_E_TRUNCATED;
+  return rc;
+}
+
+}  // extern "C"

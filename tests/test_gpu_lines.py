@@ -100,3 +100,52 @@ def test_seed_shape(S, torch, oracle, mode):
         ref = oracle.seed_shape(o, eu, ev, ew, nu, nv, nw, mode, 12345)
         assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (mode, nu, nv, nw)
     assert S.streami_seed_shape((0, 0, 0), (1, 0, 0), nu=0).shape[0] == 0
+
+
+def test_streamlines_lines_host(S, torch, oracle, wl):
+    """Host seeds in, host polylines out: equals the oracle's trace + the line definition; a point
+    buffer that is too small reports TRUNCATED and still delivers the first points."""
+    from oracle import lines
+    fld = wl.turb_field_cpu(32, 32, 1, 6)
+    n = 3001
+    seeds = wl.seeds_uniform(21, n, [31.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=80, vmin=1e-6, capacity=16, stride=4)
+    ref = oracle.streamlines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), seeds, oracle.params(**kw), "f32")
+    roff, rp = lines.streamline_lines(ref.vertices, ref.counts)
+    f = gpu_field(S, torch, fld)
+    h_seeds = torch.from_numpy(seeds.copy())
+    off = torch.zeros(n + 1, dtype=torch.int64)
+    pts = torch.full((n * 16, 3), float("nan"), dtype=torch.float32)
+    h_status = torch.zeros(n, dtype=torch.int32)
+    prm = S.params(**kw)
+    prm.out_status = h_status.data_ptr()
+    total, trunc = S.streami_trace_streamlines_lines_host(f, h_seeds, prm, off, pts)
+    assert not trunc and total == int(roff[-1])
+    assert np.array_equal(off.numpy().astype(np.uint64), roff)
+    assert np.array_equal(pts.numpy()[:total].view(np.uint32), rp.view(np.uint32))
+    assert np.isnan(pts.numpy()[total:]).all()
+    assert np.array_equal(h_status.numpy().astype(np.uint32), ref.status)
+    small = torch.zeros((100, 3), dtype=torch.float32)
+    total2, trunc2 = S.streami_trace_streamlines_lines_host(f, h_seeds, S.params(**kw), off, small)
+    assert trunc2 and total2 == total
+    assert np.array_equal(small.numpy().view(np.uint32), rp[:100].view(np.uint32))
+
+
+def test_streamlines_lines_host_on_bricks(S, torch, oracle, wl):
+    """The same host call on a bricked field runs the brick rounds."""
+    from oracle import lines
+    N, nb = 24, (2, 2, 1)
+    fld = wl.turb_field_cpu(N, 32, 1, 5)
+    n = 2500
+    seeds = wl.seeds_uniform(22, n, [N - 1.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=100, vmin=1e-6, capacity=16, stride=8)
+    ref = oracle.streamlines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), seeds, oracle.params(**kw), "f32")
+    roff, rp = lines.streamline_lines(ref.vertices, ref.counts)
+    fb = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, 1,
+                                        [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nb, 1)])
+    off = torch.zeros(n + 1, dtype=torch.int64)
+    pts = torch.zeros((n * 16, 3), dtype=torch.float32)
+    total, trunc = S.streami_trace_streamlines_lines_host(fb, torch.from_numpy(seeds.copy()), S.params(**kw), off, pts)
+    assert not trunc and total == int(roff[-1])
+    assert np.array_equal(off.numpy().astype(np.uint64), roff)
+    assert np.array_equal(pts.numpy()[:total].view(np.uint32), rp.view(np.uint32))      # P9: bricks == monolithic
