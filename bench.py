@@ -130,6 +130,7 @@ def parse_args():
     ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 packed3, 2 float4, 3 xpair, 4 cell, 5 xyquad")
     ap.add_argument("--opt", action="append", default=[], help="library option name=value")
+    ap.add_argument("--probe", action="store_true", help="print the gather ceilings (L2 / DRAM, 32-128 B pieces) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -443,6 +444,18 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         reference_arm(args, rank)
+        return
+    if args.probe:
+        if rank == 0:
+            import torch
+            import paper_2606_02627_b200 as S
+            torch.cuda.set_device(local)
+            rows = []
+            for span_mb in (48, 537, 8192, 34400):
+                for piece in (32, 64, 128):
+                    rows.append({"span_mb": span_mb, "piece_bytes": piece,
+                                 "gbs": S.streami_probe_gather(span_mb << 20, piece, 3000)})
+            print(json.dumps({"probe": "random aligned gathers, useful GB/s", "rows": rows}))
         return
     import torch
     import torch.distributed as dist

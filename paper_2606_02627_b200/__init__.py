@@ -57,6 +57,7 @@ def lib():
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
+        L.streami_probe_gather.argtypes = [Z, I, I, P, P]
         L.streami_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
         L.streami_streak_step.argtypes = [P, U, P]
         L.streami_streak_position.argtypes = [P, P]
@@ -291,6 +292,13 @@ def streami_trace_streamlines_lines_host(field, seeds, prm_host, out_offsets, ou
                                                            ctypes.byref(total), _stream(stream)),
                 allow=(E_TRUNCATED,))
     return total.value, rc == E_TRUNCATED
+
+
+def streami_probe_gather(span_bytes, piece_bytes, iters=2000, stream=None):
+    """Useful GB/s of random aligned reads (the gather ceiling, include/streami.h)."""
+    out = ctypes.c_float(0.0)
+    _check(lib().streami_probe_gather(int(span_bytes), int(piece_bytes), int(iters), ctypes.byref(out), _stream(stream)))
+    return out.value
 
 
 def _host(t, name):

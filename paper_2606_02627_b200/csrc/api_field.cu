@@ -419,3 +419,74 @@ const char* streami_error_string(int code) {
 }
 
 }  // extern "C"
+
+// ---- gather probe: what the memory system gives a field-line tracer ---------------------------
+// Every thread reads random aligned pieces of `piece` bytes (32, 64 or 128: one, two or four
+// 256-bit loads) inside a buffer of `span` bytes filled with non-repeating data, with as many
+// pieces in flight as resident threads.  span below the L2 size measures the L2 gather rate,
+// span far above it the DRAM gather rate.  This is the roofline a trilinear gather can be held
+// against; the streaming copy peak of MEASURED_PEAKS.json is not reachable
+// by 32-byte gathers.
+namespace streami {
+static __global__ void probe_fill_kernel(unsigned* __restrict__ p, size_t nwords) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t step = (size_t)gridDim.x * blockDim.x;
+  for (; i < nwords; i += step) p[i] = (unsigned)(i * 2654435761ull) ^ (unsigned)(i >> 13);
+}
+template <int NV8>
+static __global__ void __launch_bounds__(256) probe_gather_kernel(const char* __restrict__ buf, size_t nslots, int iters,
+                                                                  float* __restrict__ sink) {
+  unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+  float acc = 0.0f;
+  for (int it = 0; it < iters; ++it) {
+    s = s * 1664525u + 1013904223u;
+    const size_t r = ((size_t)s * 40503ull + (s >> 7)) % nslots;
+    const char* p = buf + r * (32 * NV8);
+#pragma unroll
+    for (int j = 0; j < NV8; ++j) {
+      float v0, v1, v2, v3, v4, v5, v6, v7;
+      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=f"(v0), "=f"(v1), "=f"(v2), "=f"(v3), "=f"(v4), "=f"(v5), "=f"(v6), "=f"(v7)
+                   : "l"(p + 32 * j));
+      acc += v0 + v7;
+    }
+  }
+  if (acc == 123.456f) sink[0] = acc;
+}
+}  // namespace streami
+
+extern "C" int streami_probe_gather(size_t span_bytes, int piece_bytes, int iters, float* out_gbs,
+                                    void* cuda_stream) {
+  if (!out_gbs || (piece_bytes != 32 && piece_bytes != 64 && piece_bytes != 128) || iters < 1 ||
+      span_bytes < 4096)
+    return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* buf = nullptr; float* sink = nullptr;
+  STREAMI_TRY(cudaMalloc((void**)&buf, span_bytes));
+  cudaError_t e = cudaMalloc((void**)&sink, sizeof(float));
+  cudaEvent_t a = nullptr, b = nullptr;
+  if (e == cudaSuccess) e = cudaEventCreate(&a);
+  if (e == cudaSuccess) e = cudaEventCreate(&b);
+  float ms = 0.0f;
+  const int blocks = num_sms() * 8, threads = 256;
+  if (e == cudaSuccess) {
+    probe_fill_kernel<<<blocks, threads, 0, st>>>((unsigned*)buf, span_bytes / 4);
+    const size_t nslots = span_bytes / (size_t)piece_bytes;
+    for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {          // first pass warms up
+      cudaEventRecord(a, st);
+      if (piece_bytes == 32) probe_gather_kernel<1><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
+      else if (piece_bytes == 64) probe_gather_kernel<2><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
+      else probe_gather_kernel<4><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
+      cudaEventRecord(b, st);
+      e = cudaEventSynchronize(b);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    }
+    launch_counter() += 3;
+  }
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
+  cudaFree(buf); if (sink) cudaFree(sink);
+  if (e != cudaSuccess) return check(e);
+  *out_gbs = (float)((double)blocks * threads * iters * piece_bytes / (ms * 1e6));
+  return STREAMI_OK;
+}
