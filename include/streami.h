@@ -152,7 +152,7 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
                               unsigned* out_counts, void* cuda_stream);
 
 /* Brick advection with hand-off (P1/K1/K3/K4 of SURVEY.md; A9).
- * f must come from streami_field_create_bricked; RK4 only.  In round r every particle queued for
+ * f must come from streami_field_create_bricked; RK4 or DP5(4).  In round r every particle queued for
  * brick b is advected inside b until it ends or its new position is owned by another brick; it
  * is then appended to that brick's queue for round r+1 (the device-side stand-in for
  * emitOutgoing + the all-to-all forward).  Rounds run until no particle is queued anywhere.

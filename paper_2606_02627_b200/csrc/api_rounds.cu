@@ -196,7 +196,6 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   if (!f || !f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, true);
   if (rc) return rc;
-  if (params->integrator != 0) return STREAMI_E_INVALID;      // RK4 only
   if (n > 0xffffffffull) return STREAMI_E_INVALID;
   if (out_round_counts && max_rounds == 0) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -207,7 +206,8 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   if (n == 0) return check(cudaStreamSynchronize(st));
 
   const bool cache = options().cell_cache != 0;
-  TraceKernel k = pick_trace_kernel(f->layout, 0, false, true, cache, unit_geometry(f->g));
+  TraceKernel k = pick_trace_kernel(f->layout, params->integrator, false, true, cache, unit_geometry(f->g));
+  const int block = trace_block(params->integrator);
 
   // scratch: [next u64][log count u64][qcount u32][pad u32][row0: nb x u32], two queues of n records
   const size_t ctr_bytes = 24 + sizeof(unsigned) * (size_t)nb;
@@ -285,10 +285,10 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
     if (e == cudaSuccess) e = cudaMemsetAsync(d_qcount, 0, sizeof(unsigned), st);
     if (e != cudaSuccess) break;
     int grid = 0;
-    rc = trace_grid(k, nwork, TRACE_BLOCK, &grid);
+    rc = trace_grid(k, nwork, block, &grid);
     if (rc) { cleanup(); return rc; }
     timing_begin(st);
-    k<<<grid, TRACE_BLOCK, 0, st>>>(a);
+    k<<<grid, block, 0, st>>>(a);
     timing_end(st);
     launch_counter()++;
     e = cudaGetLastError();

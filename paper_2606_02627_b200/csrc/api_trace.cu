@@ -13,6 +13,7 @@ typedef void (*TraceKernel)(const TraceArgs);
 
 template <int L, bool U>
 static TraceKernel pick_lu(int integ, bool brick, bool cache) {      // steady
+  if (brick && integ) return cache ? trace_kernel<L, 1, false, true, true, U> : trace_kernel<L, 1, false, true, false, U>;
   if (brick) return cache ? trace_kernel<L, 0, false, true, true, U> : trace_kernel<L, 0, false, true, false, U>;
   if (integ) return cache ? trace_kernel<L, 1, false, false, true, U> : trace_kernel<L, 1, false, false, false, U>;
   return cache ? trace_kernel<L, 0, false, false, true, U> : trace_kernel<L, 0, false, false, false, U>;

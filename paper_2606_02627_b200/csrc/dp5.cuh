@@ -53,12 +53,12 @@ __device__ __forceinline__ float rp10(float x) {
 }
 
 #define STREAMI_S(PX, PY, PZ, T, KX, KY, KZ)                                                   \
-  rc = sample<LAYOUT, UNSTEADY, false, CACHE, UNIT>(a.g, s, cc, PX, PY, PZ, T, KX, KY, KZ);    \
+  rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a.g, s, cc, PX, PY, PZ, T, KX, KY, KZ);    \
   n_samples++;                                                                                 \
   if (rc) return rc;
 
 // One DP5(4) attempt.  L.k1 holds k1 (FSAL).  Returns 0 to continue, else the final status.
-template <int LAYOUT, bool UNSTEADY, bool CACHE, bool UNIT>
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
 __device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store& s, CellCache& cc,
                                                 Lane& L, unsigned& n_samples, unsigned& n_attempts) {
   if (L.n == a.max_steps) return ST_MAXSTEPS;

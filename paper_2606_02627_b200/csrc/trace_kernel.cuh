@@ -130,7 +130,7 @@ trace_kernel(const TraceArgs a) {
             if (INTEG == 1) {
               // k1 of the first attempt.  For a continued particle this recomputes the FSAL value
               // S(p, t) it carried (same operands, same operations), so it is not counted again.
-              unsigned rc = sample<LAYOUT, UNSTEADY, false, CACHE, UNIT, true>(a.g, st, cc, L.px, L.py, L.pz, L.t,
+              unsigned rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT, true>(a.g, st, cc, L.px, L.py, L.pz, L.t,
                                                                                L.k1x, L.k1y, L.k1z);
               if (fresh) n_samples++;
               if (rc) { finish_particle(a, L, rc); active = false; atomicAdd(&s_tot[2], 1ull); }
@@ -148,7 +148,7 @@ trace_kernel(const TraceArgs a) {
     if (active) {
       unsigned rc, done = 0;
       if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, done);
-      else            rc = dp5_attempt<LAYOUT, UNSTEADY, CACHE, UNIT>(a, st, cc, L, n_samples, n_attempts);
+      else            rc = dp5_attempt<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, n_samples, n_attempts);
       if (BRICK && rc == 0) {                                                   // a8: owner of p_new
         if (!still_owned<UNIT>(a.g, st, L.px, L.py, L.pz)) dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
         if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; handoff = rc == RC_HANDOFF; }

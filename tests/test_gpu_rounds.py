@@ -263,3 +263,42 @@ def test_host_buffer_variants_of_streaklines_and_bricks(S, torch, oracle, wl):
     nlog = int(h_lc.item())
     assert nlog == ref.nlog
     assert np.array_equal(np.sort(h_log.numpy().view(np.uint64)[:nlog]), ref.log)
+
+
+@pytest.mark.parametrize("layout,budget", [(3, -1), (5, 0), (1, 9)])
+def test_bricks_dp5(S, torch, oracle, wl, layout, budget):
+    """DP5(4) through the brick rounds: the hand-off record carries t and h, the FSAL k1 is
+    recomputed in the new brick (bit-identical by A9).  Against the oracle's brick rounds and
+    against the monolithic GPU trace."""
+    N, nb = 32, (2, 2, 2)
+    fld = wl.turb_field_cpu(N, 48, 1, 6)
+    n = 12007
+    seeds = wl.seeds_uniform(31, n, [N - 1.0] * 3)
+    kw = dict(integrator=1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=150,
+              vmin=1e-6, capacity=40, stride=3)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    S.streami_set_option("brick_round_steps", budget)
+    try:
+        out = gpu_bricks(S, torch, wl, fld, nb, seeds, layout=layout, max_rounds=128, **kw)
+    finally:
+        S.streami_set_option("brick_round_steps", 0)
+    for key in ("status", "steps", "counts"):
+        assert np.array_equal(out[key], getattr(ref, key)), key
+    assert np.array_equal(out["final"].view(np.uint32), ref.final.view(np.uint32))
+    assert np.array_equal(out["vertices"].view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(out["totals"], ref.totals)
+    if budget == -1:                                   # A9's rounds: queue membership bit exact
+        assert out["nrounds"] == ref.nrounds
+        assert np.array_equal(out["log"], ref.log)
+        assert np.array_equal(out["round_counts"][:ref.nrounds].astype(np.uint32), ref.round_counts[:ref.nrounds])
+    assert ref.nlog > n // 20 and int(ref.totals[0]) > int(ref.totals[1])      # hand-offs and rejections occur
+    halo = ref.status == 4                             # steps of up to 1 cell may overrun a 1-cell halo (Q14)
+    from helpers import gpu_streamlines
+    mono = gpu_streamlines(S, torch, gpu_field(S, torch, fld, layout), seeds, **kw)
+    ok = ~halo
+    for key in ("status", "steps", "counts"):
+        assert np.array_equal(out[key][ok], mono[key][ok]), key
+    assert np.array_equal(out["final"].view(np.uint32)[:, ok], mono["final"].view(np.uint32)[:, ok])
