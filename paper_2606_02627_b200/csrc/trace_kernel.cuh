@@ -176,6 +176,7 @@ trace_kernel(const TraceArgs a) {
       if (any) emit_outgoing<INTEG>(a, L, dest, emit, handoff);
     }
   }
+  asm volatile("cp.async.wait_all;" ::: "memory");   // prefetch copies still in flight target our shared memory
   __syncthreads();
   if (a.totals && threadIdx.x < 4 && s_tot[threadIdx.x]) atomicAdd(a.totals + threadIdx.x, s_tot[threadIdx.x]);
 }
