@@ -47,6 +47,8 @@ WORKLOADS = {
     "c3": dict(kind="bricks", N=512, M=512, kmax=64, n=1 << 22, nb=(2, 2, 2), prm=dict(integrator=0,
                h=0.25, max_steps=4000, vmin=1e-6, capacity=256, stride=16)),
     "c4": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6)),
+    # C4 with the paper's own time handling, fields[(int)simTime]: one slice per sample
+    "c4p": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6, time_mode=1)),
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
                stride=128)),
@@ -64,6 +66,7 @@ DESCR = {
     "c3": "C3 turbulence 512^3 in 2x2x2 bricks (ghost 1), 4,194,304 seeds, RK4 h=0.25, max 4,000",
     "c4": "C4 double gyre 256x128x64 x 64 slices, 4,096-point rake, 1,000 steps, streaklines",
     "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
+    "c4p": "C4 with the paper's hold-floor-slice time handling (comparison only)",
     "c2s": "C2 with an L2-resident 64^3 field (profiling aid only)",
     "tiny": "tiny turbulence 48^3 (script self-check only)",
 }
@@ -291,7 +294,7 @@ class Job:
     def algorithmic_bytes(self, samples, stored):
         """useful gather bytes (8 vertices x 12 B per sample and slice) +
         12 B per stored vertex + per-particle fetch (12 B) and results (24 B)."""
-        per_sample = 192 if self.kind == "gyre" else 96
+        per_sample = 192 if (self.kind == "gyre" and not self.w["prm"].get("time_mode")) else 96
         return samples * per_sample + stored * 12 + self.npart * 36
 
 
@@ -309,6 +312,7 @@ class OracleRun:
         self.seeds = seeds
         oracle.build()
         prm = dict(self.w["prm"])
+        time_mode = prm.pop("time_mode", 0)
         if self.kind == "gyre":
             prm.update(capacity=1, stride=1, max_steps=self.w["nsteps"])
         self.prm = oracle.params(**prm)
@@ -319,7 +323,7 @@ class OracleRun:
             self.field = [oracle.grid(c, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
                           for c, (lo, hi) in zip(cut, boxes)]
         else:
-            self.field = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+            self.field = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt, time_mode)
         self.cores = oracle.num_threads()
 
     def run(self, stride):
