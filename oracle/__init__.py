@@ -14,7 +14,8 @@ import subprocess
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(HERE, "oracle_capi.cpp"), os.path.join(HERE, "streami_oracle.hpp")]
+_SRC = [os.path.join(HERE, "oracle_capi.cpp"), os.path.join(HERE, "streami_oracle.hpp"),
+        os.path.join(HERE, "hexmesh_oracle.hpp")]
 _SO = os.path.join(HERE, "liboracle.so")
 
 OUT_OF_DOMAIN, MAX_STEPS, STAGNANT, HALO_MISS = 1, 2, 3, 4
@@ -219,3 +220,49 @@ def seed_shape(o, eu, ev, ew, nu, nv=1, nw=1, mode=0, rng_seed=0):
     fn.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_uint32] * 3 + [ctypes.c_int, ctypes.c_uint64, ctypes.c_void_p]
     fn(f3(o), f3(eu), f3(ev), f3(ew), nu, nv, nw, mode, rng_seed, _p(out))
     return out
+
+
+# ---- hexahedral meshes (oracle/hexmesh_oracle.hpp) --------------------------------------------
+class HexMesh:
+    """X [nv,3] f32 vertex positions, V [nv,3] f32 values, H [nc,8] u32 (corner l = dx+2dy+4dz),
+    bin grid nb over the box lo..hi."""
+
+    def __init__(self, X, V, H, lo, hi, nb):
+        self.X = np.ascontiguousarray(X, dtype=np.float32)
+        self.V = np.ascontiguousarray(V, dtype=np.float32)
+        self.H = np.ascontiguousarray(H, dtype=np.uint32)
+        self.lo = np.ascontiguousarray(lo, dtype=np.float32)
+        self.hi = np.ascontiguousarray(hi, dtype=np.float32)
+        self.nb = np.ascontiguousarray(nb, dtype=np.int32)
+
+    def _args(self):
+        return [ctypes.c_size_t(self.X.shape[0]), ctypes.c_size_t(self.H.shape[0]), _p(self.X), _p(self.V),
+                _p(self.H), _p(self.lo), _p(self.hi), _p(self.nb)]
+
+
+def hexmesh_sample(mesh, pts, precision="f32", brute=False):
+    """(v [n,3], cell [n] (-1 = outside), xi [n,3]); brute = search all cells (the definition)."""
+    T, sfx = _dt(precision)
+    pts = np.ascontiguousarray(pts, dtype=T).reshape(-1, 3)
+    n = pts.shape[0]
+    v = np.zeros((n, 3), dtype=T); cell = np.zeros(n, dtype=np.int64); xi = np.zeros((n, 3), dtype=T)
+    fn = getattr(lib(), "oracle_hexmesh_sample_" + sfx)
+    fn.argtypes = None
+    fn(*mesh._args(), _p(pts), ctypes.c_size_t(n), ctypes.c_int(1 if brute else 0), _p(v), _p(cell), _p(xi))
+    return v, cell, xi
+
+
+def hexmesh_streamlines(mesh, seeds, prm, precision="f32", record=True):
+    T, sfx = _dt(precision)
+    seeds = np.ascontiguousarray(seeds, dtype=T).reshape(-1, 3)
+    n = seeds.shape[0]
+    cap = prm.capacity
+    verts = np.full((3, n, cap), np.nan, dtype=T) if record else None
+    counts = np.zeros(n, dtype=np.uint32)
+    steps = np.zeros(n, dtype=np.uint32); status = np.zeros(n, dtype=np.uint32)
+    final = np.zeros((3, n), dtype=T); totals = np.zeros(4, dtype=np.uint64)
+    fn = getattr(lib(), "oracle_hexmesh_streamlines_" + sfx)
+    fn.argtypes = None
+    fn(*mesh._args(), _p(seeds), ctypes.c_size_t(n), ctypes.byref(prm), _p(verts), _p(counts), _p(steps),
+       _p(status), _p(final), _p(totals))
+    return Result(vertices=verts, counts=counts, steps=steps, status=status, final=final, totals=totals)

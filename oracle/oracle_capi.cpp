@@ -349,3 +349,38 @@ extern "C" void oracle_seed_shape_f32(const float o[3], const float eu[3], const
           out[3 * s + c] = std::fma(w, ew[c], std::fma(v, ev[c], std::fma(u, eu[c], o[c])));
       }
 }
+
+// ---------------------------------------------------------------------------------------
+// Hexahedral meshes (oracle/hexmesh_oracle.hpp, formula sheet U1-U4).
+// ---------------------------------------------------------------------------------------
+#include "hexmesh_oracle.hpp"
+
+#define HEXMESH_CAPI(T, SFX)                                                                         \
+  extern "C" void oracle_hexmesh_sample_##SFX(size_t nv, size_t nc, const float* X, const float* V,  \
+      const uint32_t* H, const float* lo, const float* hi, const int* nb, const T* pts, size_t n,    \
+      int brute, T* out_v, long long* out_cell, T* out_xi) {                                         \
+    oracle::HexMesh<T> m; m.init(nv, nc, X, V, H, lo, hi, nb);                                       \
+    oracle::HexField<T> f{&m};                                                                       \
+    for (size_t i = 0; i < n; ++i) {                                                                 \
+      T xi[3] = {0, 0, 0}; long long c = -1;                                                         \
+      if (brute) {  /* definition of point location: the lowest-numbered cell that contains p */     \
+        int b[3];                                                                                    \
+        if (m.bin_of(pts + 3 * i, b))                                                                \
+          for (size_t k = 0; k < nc && c < 0; ++k) if (oracle::hx_invert(m, k, pts + 3 * i, xi)) c = (long long)k; \
+      } else c = oracle::hx_locate(m, pts + 3 * i, xi);                                              \
+      out_cell[i] = c;                                                                               \
+      for (int a = 0; a < 3; ++a) { out_xi[3 * i + a] = xi[a]; out_v[3 * i + a] = 0; }                \
+      if (c >= 0 && !brute) f.sample(pts + 3 * i, T(0), out_v + 3 * i);                              \
+    }                                                                                                \
+  }                                                                                                  \
+  extern "C" void oracle_hexmesh_streamlines_##SFX(size_t nv, size_t nc, const float* X,             \
+      const float* V, const uint32_t* H, const float* lo, const float* hi, const int* nb,            \
+      const T* seeds, size_t n, const OParams* p, T* out_vertices, uint32_t* out_counts,             \
+      uint32_t* out_steps, uint32_t* out_status, T* out_final, unsigned long long* totals) {         \
+    oracle::HexMesh<T> m; m.init(nv, nc, X, V, H, lo, hi, nb);                                       \
+    oracle::HexField<T> f{&m};                                                                       \
+    run_streamlines<T>(f, seeds, n, p, out_vertices, out_counts, out_steps, out_status, out_final,   \
+                       totals);                                                                      \
+  }
+HEXMESH_CAPI(float, f32)
+HEXMESH_CAPI(double, f64)

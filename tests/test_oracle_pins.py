@@ -587,3 +587,76 @@ def test_seed_shape_pins(oracle):
     assert len(np.unique(r.view([("x", "f4"), ("y", "f4"), ("z", "f4")]))) == n
     r2 = oracle.seed_shape((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), n, 1, 1, mode=1, rng_seed=8)
     assert not np.array_equal(r, r2)
+
+
+# ---- hexahedral meshes (oracle/hexmesh_oracle.hpp, formula sheet U1-U4) ------------------------
+def _lin(A, b):
+    return lambda X: X @ np.asarray(A, dtype=np.float64).T + np.asarray(b, dtype=np.float64)
+
+
+def test_hexmesh_reproduces_the_structured_sampler(oracle, wl):
+    """The paper's own check: a structured grid re-expressed as hexahedra must
+    give the structured results.  Sample: 1e-12 in fp64, a few ulp of the field scale in fp32."""
+    fld = wl.turb_field_cpu(12, 16, 1, 3)
+    X, V, H, lo, hi = wl.hexmesh_from_grid(fld.dims, fld.origin, fld.spacing, fld.data[0])
+    mesh = oracle.HexMesh(X, V, H, lo, hi, (5, 4, 3))                      # bins unrelated to the cells
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing)
+    rng = np.random.default_rng(5)
+    pts = rng.uniform(0.0, 11.0, size=(3000, 3))
+    pts[:8] = [[0, 0, 0], [11, 11, 11], [3, 4, 5], [11, 0, 5.5], [2.5, 3, 11], [0, 7.25, 0], [6, 6, 6], [10.999, 0.001, 5]]
+    for prec, tol in (("f64", 1e-12), ("f32", 2e-5)):
+        v, cell, xi = oracle.hexmesh_sample(mesh, pts, prec)
+        rv, rc = oracle.sample(g, pts, 0.0, prec)
+        assert (cell >= 0).all() and (rc == 0).all()
+        assert np.abs(v - rv).max() <= tol, prec
+    v, cell, xi = oracle.hexmesh_sample(mesh, [[-0.1, 1, 1], [1, 11.2, 1], [np.nan, 1, 1]], "f32")
+    assert (cell == -1).all()
+
+
+def test_hexmesh_linear_field_on_distorted_cells(oracle, wl):
+    """Isoparametric trilinear interpolation reproduces a linear field exactly on ANY hexahedron
+    (the inverse map and the fp32 storage of the vertex values are then the only error sources)."""
+    A = [[1.0, -2.0, 0.5], [0.25, 3.0, -1.0], [2.0, 0.0, 1.5]]; b = [0.5, -1.0, 2.0]
+    X, V, H, lo, hi = wl.hexmesh_from_grid((9, 8, 7), (0.0, 1.0, -1.0), (0.5, 0.25, 1.0), jitter=0.3, seed=3,
+                                           value_fn=_lin(A, b))
+    mesh = oracle.HexMesh(X, V, H, lo, hi, (4, 4, 4))
+    rng = np.random.default_rng(6)
+    pts = lo + rng.uniform(0.0, 1.0, size=(4000, 3)) * (hi - lo)
+    # vertex values are stored in fp32 (rounded once, |V| < 20: 1e-6), which bounds the fp64 check
+    for prec, tol in (("f64", 3e-6), ("f32", 2e-4)):
+        v, cell, xi = oracle.hexmesh_sample(mesh, pts, prec)
+        assert (cell >= 0).all()
+        exact = _lin(A, b)(pts.astype(np.float32).astype(np.float64) if prec == "f32" else pts)
+        assert np.abs(v - exact).max() <= tol, (prec, np.abs(v - exact).max())
+        assert xi.min() >= -2.1e-5 and xi.max() <= 1.0 + 2.1e-5
+
+
+def test_hexmesh_bins_equal_brute_force_location(oracle, wl):
+    """Point location through the bins == the definition (the lowest-numbered cell, of ALL cells,
+    that contains the point), on distorted cells, including points outside the mesh."""
+    X, V, H, lo, hi = wl.hexmesh_from_grid((7, 6, 8), (0, 0, 0), (1.0, 1.5, 0.75), jitter=0.35, seed=9,
+                                           value_fn=_lin(np.eye(3), [0, 0, 0]))
+    rng = np.random.default_rng(7)
+    pts = lo - 0.2 + rng.uniform(0.0, 1.0, size=(2500, 3)) * (hi - lo + 0.4)
+    for nb in ((1, 1, 1), (3, 5, 2), (13, 11, 17)):
+        mesh = oracle.HexMesh(X, V, H, lo, hi, nb)
+        for prec in ("f32", "f64"):
+            _, cell, _ = oracle.hexmesh_sample(mesh, pts, prec)
+            _, brute, _ = oracle.hexmesh_sample(mesh, pts, prec, brute=True)
+            assert np.array_equal(cell, brute), (nb, prec)
+    assert np.count_nonzero(cell < 0) > 100 and np.count_nonzero(cell >= 0) > 1000
+
+
+def test_hexmesh_streamlines_follow_the_structured_ones(oracle, wl):
+    """RK4 on the hexahedral re-expression of a grid tracks the structured trace (fp64: 1e-9 over
+    60 steps); statuses and step counts agree."""
+    fld = wl.turb_field_cpu(16, 16, 1, 3)
+    X, V, H, lo, hi = wl.hexmesh_from_grid(fld.dims, fld.origin, fld.spacing, fld.data[0])
+    mesh = oracle.HexMesh(X, V, H, lo, hi, (6, 6, 6))
+    seeds = wl.seeds_uniform(4, 300, [15.0] * 3)
+    prm = oracle.params(integrator=0, h=0.25, max_steps=60, vmin=1e-6, capacity=61, stride=1)
+    a = oracle.hexmesh_streamlines(mesh, seeds, prm, "f64")
+    b = oracle.streamlines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), seeds, prm, "f64")
+    assert np.array_equal(a.status, b.status) and np.array_equal(a.steps, b.steps)
+    assert np.nanmax(np.abs(a.vertices - b.vertices)) < 1e-9
+    assert np.array_equal(a.totals[:3], b.totals[:3])

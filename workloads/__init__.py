@@ -236,3 +236,33 @@ def cut_bricks_cuda(vol, global_dims, brick_grid, ghost=1):
         out.append(t)
     torch.cuda.synchronize()
     return out
+
+
+# ---- hexahedral meshes (the paper's other field type; input generation only) -------------------
+def hexmesh_from_grid(dims, origin, spacing, values=None, jitter=0.0, seed=1, value_fn=None):
+    """Re-express a structured grid as hexahedral cells (what the paper's own experiment does with
+    its structured data).  Vertices sit at the grid points; `jitter` > 0 displaces the
+    interior vertices by up to +-jitter*spacing per axis (uniform, mt19937_64) to make the cells
+    general hexahedra.  Values: `values` [Nz,Ny,Nx,3] taken as they are, or value_fn(X) evaluated
+    at the (displaced) vertices in fp64 and rounded once.  Returns X [nv,3] f32, V [nv,3] f32,
+    H [nc,8] u32 with corner l = dx + 2*dy + 4*dz, and the bounding box (lo, hi)."""
+    nx, ny, nz = dims
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    X = np.stack([origin[0] + x * float(spacing[0]), origin[1] + y * float(spacing[1]),
+                  origin[2] + z * float(spacing[2])], axis=-1).astype(np.float64)
+    if jitter > 0.0:
+        u = uniform(seed, 3 * nx * ny * nz).reshape(nz, ny, nx, 3)
+        d = (2.0 * u - 1.0) * jitter * np.asarray(spacing, dtype=np.float64)
+        interior = np.zeros((nz, ny, nx, 1), dtype=bool)
+        interior[1:-1, 1:-1, 1:-1] = True
+        X = X + np.where(interior, d, 0.0)
+    Xf = X.reshape(-1, 3).astype(np.float32)
+    if value_fn is not None:
+        V = np.asarray(value_fn(Xf.astype(np.float64)), dtype=np.float64).astype(np.float32)
+    else:
+        V = np.ascontiguousarray(values, dtype=np.float32).reshape(-1, 3)
+    vid = (z * ny + y) * nx + x
+    corners = [vid[dz:nz - 1 + dz, dy:ny - 1 + dy, dx:nx - 1 + dx] for dz in (0, 1) for dy in (0, 1) for dx in (0, 1)]
+    H = np.stack(corners, axis=-1).reshape(-1, 8).astype(np.uint32)     # l = dx + 2 dy + 4 dz
+    lo = Xf.min(axis=0); hi = Xf.max(axis=0)
+    return Xf, V, H, lo, hi
