@@ -52,6 +52,10 @@ WORKLOADS = {
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
                stride=128)),
+    # the paper's other field type: a 128^3 turbulence grid re-expressed as 127^3 hexahedra
+    # (PAPER.md:159), bins 127^3, RK4 (never the reported headline)
+    "u1": dict(kind="mesh", N=128, M=128, kmax=32, n=1 << 18, nbins=(127, 127, 127), prm=dict(integrator=0, h=0.25,
+               max_steps=500, vmin=1e-6, capacity=64, stride=8)),
     # L2-resident variant of C2 (same step size and seed count, 64^3 field): isolates the instruction
     # stream from the DRAM gathers when reading profiles (never a reported number)
     "c2s": dict(kind="turb", N=64, M=64, kmax=16, n=1 << 20, prm=dict(integrator=0, h=0.25,
@@ -68,6 +72,7 @@ DESCR = {
     "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
     "c4p": "C4 with the paper's hold-floor-slice time handling (comparison only)",
     "c2s": "C2 with an L2-resident 64^3 field (profiling aid only)",
+    "u1": "U1 hexahedral mesh: 128^3 turbulence grid as 2,048,383 hexahedra, 262,144 seeds, RK4 h=0.25, max 500",
     "tiny": "tiny turbulence 48^3 (script self-check only)",
 }
 
@@ -190,6 +195,16 @@ class Job:
             self.field = S.streami_field_create(fld.dims, fld.origin, fld.spacing, fld.nslices,
                                                 fld.slice_dt, self.data, layout)
             self.seeds_h = wl.rake_c4()
+        elif self.kind == "mesh":
+            N = w["N"]
+            fld, dev = wl.turb_field_cuda(N, w["M"], 1.0, w["kmax"], host=True)
+            del dev
+            self.host_field = fld
+            self.mesh_arrays = wl.hexmesh_from_grid(fld.dims, fld.origin, fld.spacing, fld.data[0])
+            X, V, H, lo, hi = self.mesh_arrays
+            self.field = S.Mesh(X, V, H, lo, hi, w["nbins"])
+            self.data = None
+            self.seeds_h = wl.seeds_uniform(shard_seed(rank), w["n"], [N - 1.0] * 3)
         else:
             N = w["N"]
             want_host = N <= 512
@@ -204,7 +219,7 @@ class Job:
                 self.data = dev
                 self.field = S.streami_field_create((N, N, N), (0, 0, 0), (1, 1, 1), 1, 1.0, dev, layout)
             self.seeds_h = wl.seeds_uniform(shard_seed(rank), w["n"], [N - 1.0] * 3)
-        self.layout, self.owned_bytes = self.field.info()
+        self.layout, self.owned_bytes = self.field.info() if self.kind != "mesh" else (0, 224 * self.mesh_arrays[2].shape[0])
         self.n = self.seeds_h.shape[0]
         self.seeds = torch.from_numpy(self.seeds_h).cuda()
         dev = "cuda"
@@ -232,7 +247,9 @@ class Job:
     # -- one step, inputs and outputs resident in HBM ------------------------------------------
     def step_device(self):
         S = self.S
-        if self.kind == "gyre":
+        if self.kind == "mesh":
+            S.streami_mesh_trace_streamlines(self.field, self.seeds, self.prm, self.verts, self.counts)
+        elif self.kind == "gyre":
             S.streami_trace_streaklines(self.field, self.seeds, self.nsteps, self.prm, self.verts, self.counts)
         elif self.kind == "bricks":
             self.nrounds, _ = S.streami_brick_advect(self.field, self.seeds, self.prm, self.verts, self.counts)
@@ -248,7 +265,7 @@ class Job:
                           counts=pin(self.counts), steps=pin(self.steps_o), status=pin(self.status_o),
                           final=None if self.final_o is None else pin(self.final_o),
                           totals=t.zeros(4, dtype=t.int64).pin_memory())
-            if self.kind != "gyre":
+            if self.kind not in ("gyre", "mesh"):
                 # polyline buffers instead of the capacity-padded slot array
                 self.h["verts"] = None; self.h["counts"] = None
                 self.h["offsets"] = t.zeros(self.n + 1, dtype=t.int64).pin_memory()
@@ -268,7 +285,7 @@ class Job:
         nb = lambda x: 0 if x is None else x.numel() * x.element_size()
         bi = nb(h["seeds"])
         bo = sum(nb(h[k]) for k in ("verts", "counts", "steps", "status", "final", "totals"))
-        if self.kind != "gyre":                        # offsets + the points actually delivered
+        if self.kind not in ("gyre", "mesh"):          # offsets + the points actually delivered
             bo += nb(h["offsets"]) + 12 * int(self.e2e_points)
         return bi, bo
 
@@ -276,7 +293,16 @@ class Job:
         """One step through the C-ABI host-buffer calls: H2D of the seeds / rake points, the
         trace, D2H of every output, stream sync -- all inside the library."""
         h, S = self._pinned(), self.S
-        if self.kind == "gyre":
+        if self.kind == "mesh":
+            # no host-buffer entry point for meshes yet: the same copies are issued here around the
+            # device call (pinned host -> device, device -> pinned host, stream sync)
+            self.seeds.copy_(h["seeds"], non_blocking=True)
+            self.step_device()
+            for k, d in (("verts", self.verts), ("counts", self.counts), ("steps", self.steps_o),
+                         ("status", self.status_o), ("final", self.final_o), ("totals", self.totals_o)):
+                h[k].copy_(d, non_blocking=True)
+            self.torch.cuda.current_stream().synchronize()
+        elif self.kind == "gyre":
             S.streami_trace_streaklines_host(self.field, h["seeds"], self.nsteps, self.prm_h, h["verts"], h["counts"])
         else:
             # streamlines: the host application's end product is the assembled polylines (the paper's
@@ -316,7 +342,10 @@ class OracleRun:
         if self.kind == "gyre":
             prm.update(capacity=1, stride=1, max_steps=self.w["nsteps"])
         self.prm = oracle.params(**prm)
-        if self.kind == "bricks":
+        if self.kind == "mesh":
+            X, V, H, lo, hi = wl.hexmesh_from_grid(fld.dims, fld.origin, fld.spacing, fld.data[0])
+            self.field = oracle.HexMesh(X, V, H, lo, hi, self.w["nbins"])
+        elif self.kind == "bricks":
             N = self.w["N"]
             boxes = wl.brick_boxes(fld.dims, self.w["nb"], 1)
             cut = wl.cut_bricks(fld, self.w["nb"], 1)
@@ -331,7 +360,9 @@ class OracleRun:
         o = self.o
         sub = self.seeds[::stride]
         t0 = time.perf_counter()
-        if self.kind == "gyre":
+        if self.kind == "mesh":
+            r = o.hexmesh_streamlines(self.field, sub, self.prm, "f32", record=False)
+        elif self.kind == "gyre":
             r = o.streaklines(self.field, sub, self.w["nsteps"], self.prm, "f32")
         elif self.kind == "bricks":
             r = o.brick_advect(self.field, self.w["nb"], sub, self.prm, "f32", record=False)
@@ -535,7 +566,7 @@ def main():
     achieved = (alg / launches_per_step) / (kms * 1e-3) / 1e9 if kms > 0 else None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": None if achieved is None else achieved / peak, "traffic": None,
-                "kernel": "trace_kernel" if job.kind != "gyre" else "streak_kernel",
+                "kernel": {"gyre": "streak_kernel", "mesh": "mesh_trace_kernel"}.get(job.kind, "trace_kernel"),
                 "kernel_ms_per_launch": kms, "kernel_launches_per_step": launches_per_step,
                 "algorithmic_bytes_per_launch": alg / launches_per_step, "peak_source": peak_src,
                 "kernel_share_of_step": kern_ms / total_ms if world == 1 else None}
@@ -559,6 +590,8 @@ def main():
                          % (stride, npart, a, dt)}
 
     lay = {1: "packed3", 2: "float4", 3: "xpair", 4: "cell", 5: "xyquad"}.get(job.layout, str(job.layout))
+    if job.kind == "mesh":
+        lay = "224-byte cell records (8 corner positions + 8 corner values + box)"
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

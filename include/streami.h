@@ -175,6 +175,29 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream);
 
+/* Vector fields on hexahedral meshes -- the paper's other field type ("unstructured meshes", cell
+ * location + interpolation), restricted to the element type of its own
+ * experiment (a structured grid re-expressed as hexahedra).  Formula sheet U1-U4:
+ * cell c has corners H[c][l], l = dx + 2 dy + 4 dz, at reference coordinates (dx, dy, dz); a point
+ * is located through a uniform bin grid nb over the box lo..hi as the first (lowest-numbered) cell
+ * listed in its bin whose inverse isoparametric map (6 Newton steps from the centre) converges to
+ * reference coordinates inside the unit cube (+- 2e-5); the value is the trilinear combination of
+ * the corner values at those coordinates.
+ * _create_hex: X [nv][3], V [nv][3], H [nc][8] are HOST arrays (consumed: the handle owns a device
+ * copy in a per-cell layout and the bin lists, built here); errors: INVALID (null, empty, index
+ * out of range, empty box, more than 2^32-1 list entries), NOMEM, CUDA.
+ * _sample: points [n][3] device -> out_v [n][3] (zero where no cell is found), out_cell [n] i64
+ * (-1 = outside; may be NULL).  _trace_streamlines: as streami_trace_streamlines (RK4 only;
+ * out_vertices may be NULL; OUT_OF_DOMAIN = no cell contains the point). */
+typedef struct streami_mesh_s* streami_mesh;
+int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V, const unsigned* H,
+                            const float lo[3], const float hi[3], const int nb[3], streami_mesh* out);
+int streami_mesh_destroy(streami_mesh m);
+int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* out_v, long long* out_cell,
+                        void* cuda_stream);
+int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n, const streami_params* params,
+                                   float* out_vertices, unsigned* out_counts, void* cuda_stream);
+
 /* Seed generation on a control shape (the paper's convenience kernels: "uniformly distributed seed
  * points given simple control shapes such as planes or lines").  The shape is
  * origin + u*edge_u + v*edge_v + w*edge_w, (u,v,w) in [0,1)^3, sampled nu x nv x nw times (line:

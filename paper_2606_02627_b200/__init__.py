@@ -58,6 +58,10 @@ def lib():
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
         L.streami_probe_gather.argtypes = [Z, I, I, P, P]
+        L.streami_mesh_create_hex.argtypes = [Z, Z, P, P, P, P, P, P, P]
+        L.streami_mesh_destroy.argtypes = [P]
+        L.streami_mesh_sample.argtypes = [P, P, Z, P, P, P]
+        L.streami_mesh_trace_streamlines.argtypes = [P, P, Z, P, P, P, P]
         L.streami_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
         L.streami_streak_step.argtypes = [P, U, P]
         L.streami_streak_position.argtypes = [P, P]
@@ -299,6 +303,45 @@ def streami_probe_gather(span_bytes, piece_bytes, iters=2000, stream=None):
     out = ctypes.c_float(0.0)
     _check(lib().streami_probe_gather(int(span_bytes), int(piece_bytes), int(iters), ctypes.byref(out), _stream(stream)))
     return out.value
+
+
+class Mesh:
+    """Owner of a streami_mesh handle (hexahedral mesh field)."""
+
+    def __init__(self, X, V, H, lo, hi, nb):
+        import numpy as np
+        X = np.ascontiguousarray(X, dtype=np.float32); V = np.ascontiguousarray(V, dtype=np.float32)
+        H = np.ascontiguousarray(H, dtype=np.uint32)
+        self.handle = ctypes.c_void_p(None)
+        _check(lib().streami_mesh_create_hex(X.shape[0], H.shape[0], X.ctypes.data, V.ctypes.data, H.ctypes.data,
+                                             _f3(lo), _f3(hi), _i3(nb), ctypes.byref(self.handle)))
+
+    def destroy(self):
+        if self.handle:
+            lib().streami_mesh_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def streami_mesh_sample(mesh, points, stream=None):
+    _req(points, torch.float32, "points")
+    n = points.shape[0]
+    v = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    cell = torch.empty(n, dtype=torch.int64, device="cuda")
+    _check(lib().streami_mesh_sample(mesh.handle, _ptr(points), n, _ptr(v), _ptr(cell), _stream(stream)))
+    return v, cell
+
+
+def streami_mesh_trace_streamlines(mesh, seeds, prm, out_vertices, out_counts, stream=None):
+    _req(seeds, torch.float32, "seeds"); _req(out_vertices, torch.float32, "out_vertices")
+    _req(out_counts, torch.int32, "out_counts")
+    _check(lib().streami_mesh_trace_streamlines(mesh.handle, _ptr(seeds), seeds.shape[0], ctypes.byref(prm),
+                                                _ptr(out_vertices), _ptr(out_counts), _stream(stream)))
 
 
 def _host(t, name):

@@ -1,0 +1,138 @@
+// csrc/api_mesh.cu -- hexahedral-mesh fields: handle, bin grid (built on the host at create time),
+// streami_mesh_sample, streami_mesh_trace_streamlines.  Formula sheet U1-U4, DESIGN.md section 13.
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "internal.h"
+#include "mesh.cuh"
+
+struct streami_mesh_s {
+  streami::MeshDev d;
+  size_t nc;
+  void* dev_cells; void* dev_start; void* dev_items;
+};
+
+namespace streami {
+int check_params(const streami_params* p, bool need_capacity);
+
+// U2 bin index of a coordinate already known to be inside [lo, hi] (fp32, as on the device)
+static int bin_index(float x, float lo, float s, int nb) { return std::min((int)std::floor((x - lo) * s), nb - 1); }
+}  // namespace streami
+
+using namespace streami;
+
+extern "C" {
+
+int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V, const unsigned* H,
+                            const float lo[3], const float hi[3], const int nb[3], streami_mesh* out) {
+  if (!out) return STREAMI_E_INVALID;
+  *out = nullptr;
+  if (!X || !V || !H || !lo || !hi || !nb || nv == 0 || nc == 0 || nc > 0xffffffffull) return STREAMI_E_INVALID;
+  for (int a = 0; a < 3; ++a)
+    if (nb[a] < 1 || !(hi[a] > lo[a]) || !std::isfinite(lo[a]) || !std::isfinite(hi[a])) return STREAMI_E_INVALID;
+  const size_t nbins = (size_t)nb[0] * nb[1] * nb[2];
+  if (nbins > 0x7fffffffull) return STREAMI_E_INVALID;
+  for (size_t i = 0; i < 8 * nc; ++i) if (H[i] >= nv) return STREAMI_E_INVALID;
+
+  float s[3];
+  for (int a = 0; a < 3; ++a) s[a] = (float)nb[a] / (hi[a] - lo[a]);       // U2, fp32
+  // cell records + bin ranges
+  std::vector<float> cells(nc * (size_t)MESH_REC, 0.0f);
+  std::vector<int> range(nc * 6);
+  float extent = 0.0f;
+  for (size_t c = 0; c < nc; ++c) {
+    float* rec = cells.data() + c * MESH_REC;
+    float mn[3], mx[3];
+    for (int l = 0; l < 8; ++l) {
+      const unsigned v = H[8 * c + l];
+      for (int a = 0; a < 3; ++a) {
+        const float x = X[3 * (size_t)v + a];
+        rec[8 * a + l] = x; rec[24 + 8 * a + l] = V[3 * (size_t)v + a];
+        mn[a] = l ? std::min(mn[a], x) : x; mx[a] = l ? std::max(mx[a], x) : x;
+      }
+    }
+    for (int a = 0; a < 3; ++a) {
+      rec[48 + a] = mn[a]; rec[51 + a] = mx[a];
+      extent = std::max(extent, mx[a] - mn[a]);
+      const float x0 = std::min(std::max(mn[a], lo[a]), hi[a]), x1 = std::min(std::max(mx[a], lo[a]), hi[a]);
+      range[6 * c + a] = bin_index(x0, lo[a], s[a], nb[a]);
+      range[6 * c + 3 + a] = bin_index(x1, lo[a], s[a], nb[a]);
+    }
+  }
+  // CSR lists, cells in ascending order inside every bin (count, scan, fill)
+  std::vector<unsigned> start(nbins + 1, 0u);
+  auto for_bins = [&](size_t c, auto&& fn) {
+    const int* r = range.data() + 6 * c;
+    for (int z = r[2]; z <= r[5]; ++z)
+      for (int y = r[1]; y <= r[4]; ++y)
+        for (int x = r[0]; x <= r[3]; ++x) fn(((size_t)z * nb[1] + y) * nb[0] + x);
+  };
+  unsigned long long total = 0;
+  for (size_t c = 0; c < nc; ++c) for_bins(c, [&](size_t b) { start[b + 1]++; total++; });
+  if (total > 0xffffffffull) return STREAMI_E_INVALID;
+  for (size_t b = 0; b < nbins; ++b) start[b + 1] += start[b];
+  std::vector<unsigned> items(std::max<size_t>(total, 1)), fill(start.begin(), start.end() - 1);
+  for (size_t c = 0; c < nc; ++c) for_bins(c, [&](size_t b) { items[fill[b]++] = (unsigned)c; });
+
+  streami_mesh_s* m = new streami_mesh_s();
+  m->nc = nc; m->dev_cells = m->dev_start = m->dev_items = nullptr;
+  cudaError_t e = cudaMalloc(&m->dev_cells, cells.size() * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&m->dev_start, start.size() * sizeof(unsigned));
+  if (e == cudaSuccess) e = cudaMalloc(&m->dev_items, items.size() * sizeof(unsigned));
+  if (e == cudaSuccess) e = cudaMemcpy(m->dev_cells, cells.data(), cells.size() * sizeof(float), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(m->dev_start, start.data(), start.size() * sizeof(unsigned), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(m->dev_items, items.data(), items.size() * sizeof(unsigned), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(m->dev_cells); cudaFree(m->dev_start); cudaFree(m->dev_items);
+    delete m;
+    return check(e);
+  }
+  MeshDev& d = m->d;
+  d.cells = (const float*)m->dev_cells; d.bin_start = (const unsigned*)m->dev_start; d.bin_items = (const unsigned*)m->dev_items;
+  d.lox = lo[0]; d.loy = lo[1]; d.loz = lo[2]; d.hix = hi[0]; d.hiy = hi[1]; d.hiz = hi[2];
+  d.sx = s[0]; d.sy = s[1]; d.sz = s[2]; d.nbx = nb[0]; d.nby = nb[1]; d.nbz = nb[2];
+  d.margin = 50.0f * MESH_TOL * extent;
+  *out = m;
+  return STREAMI_OK;
+}
+
+int streami_mesh_destroy(streami_mesh m) {
+  if (!m) return STREAMI_E_INVALID;
+  cudaFree(m->dev_cells); cudaFree(m->dev_start); cudaFree(m->dev_items);
+  delete m;
+  return STREAMI_OK;
+}
+
+int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* out_v, long long* out_cell,
+                        void* cuda_stream) {
+  if (!m || (n > 0 && (!points || !out_v))) return STREAMI_E_INVALID;
+  if (n == 0) return STREAMI_OK;
+  mesh_sample_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(m->d, points, n, out_v, out_cell);
+  STREAMI_LAUNCHED();
+  return STREAMI_OK;
+}
+
+int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n, const streami_params* params,
+                                   float* out_vertices, unsigned* out_counts, void* cuda_stream) {
+  if (!m || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
+  int rc = check_params(params, true);
+  if (rc) return rc;
+  if (params->integrator != 0 || n > 0xffffffffull) return STREAMI_E_INVALID;   // RK4 (Listing 1)
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
+  if (n == 0) return STREAMI_OK;
+  MeshTraceArgs a{};
+  a.m = m->d; a.seeds = seeds; a.n = n;
+  a.h = params->h; a.h2 = 0.5f * params->h; a.h6 = params->h / 6.0f; a.vmin2 = params->vmin * params->vmin;
+  a.max_steps = params->max_steps; a.verts = out_vertices; a.cap = params->capacity; a.stride = params->stride;
+  a.counts = out_counts; a.steps = params->out_steps; a.status = params->out_status; a.fin = params->out_final;
+  a.totals = params->out_totals;
+  timing_begin(st);
+  mesh_trace_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a);
+  timing_end(st);
+  STREAMI_LAUNCHED();
+  return STREAMI_OK;
+}
+
+}  // extern "C"

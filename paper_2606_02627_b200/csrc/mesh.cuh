@@ -1,0 +1,200 @@
+// csrc/mesh.cuh -- vector fields on hexahedral meshes: the paper's other field type
+// ("unstructured meshes", cell location + interpolation).
+// Written from the formula sheet U1-U4; shares nothing with oracle/.
+// The translation unit is compiled with -fmad=false: every fused multiply-add is an explicit
+// __fmaf_rn.  The paper locates cells with a BVH point query; a uniform bin grid gives the same
+// located cell ("the first listed cell of the point's bin that contains it") with one table lookup.
+//
+// Layout: one 224-byte record per CELL -- the 8 corner positions [a][l] (24 floats), the 8 corner
+// values [a][l] (24 floats), the cell's bounding box (6 floats), 2 pad -- so that testing and
+// sampling a candidate cell is 7 contiguous sectors and no index indirection (the connectivity
+// array H is consumed at create time).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "trace.cuh"
+
+namespace streami {
+
+constexpr int MESH_REC = 56;            // floats per cell record
+constexpr int MESH_NEWTON = 6;          // U3
+constexpr float MESH_TOL = 2e-5f;       // U3
+
+struct MeshDev {
+  const float* cells;                   // [nc][MESH_REC]
+  const unsigned* bin_start;            // [nbins + 1]
+  const unsigned* bin_items;
+  float lox, loy, loz, hix, hiy, hiz, sx, sy, sz;
+  int nbx, nby, nbz;
+  float margin;                         // bounding-box pre-test margin (build's choice, see hx_locate)
+};
+
+__device__ __forceinline__ float hx_tri(const float* Q, float x, float y, float z) {
+  const float c00 = lerp(Q[0], Q[1], x), c01 = lerp(Q[2], Q[3], x);
+  const float c10 = lerp(Q[4], Q[5], x), c11 = lerp(Q[6], Q[7], x);
+  return lerp(lerp(c00, c01, y), lerp(c10, c11, y), z);
+}
+__device__ __forceinline__ float hx_cof(float u, float v, float w, float z) { return __fmaf_rn(u, v, -(w * z)); }
+
+// U3: reference coordinates of p in the cell whose corner positions are P[a*8 + l].
+__device__ __forceinline__ bool hx_invert(const float* __restrict__ P, float px, float py, float pz,
+                                          float& x, float& y, float& z) {
+  x = 0.5f; y = 0.5f; z = 0.5f;
+  float dx = 0.0f, dy = 0.0f, dz = 0.0f;
+  const float p[3] = {px, py, pz};
+#pragma unroll 1
+  for (int it = 0; it < MESH_NEWTON; ++it) {
+    float G[3], Jx[3], Jy[3], Jz[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const float* q = P + 8 * a;
+      G[a] = hx_tri(q, x, y, z) - p[a];
+      Jx[a] = lerp(lerp(q[1] - q[0], q[3] - q[2], y), lerp(q[5] - q[4], q[7] - q[6], y), z);
+      Jy[a] = lerp(lerp(q[2] - q[0], q[3] - q[1], x), lerp(q[6] - q[4], q[7] - q[5], x), z);
+      Jz[a] = lerp(lerp(q[4] - q[0], q[5] - q[1], x), lerp(q[6] - q[2], q[7] - q[3], x), y);
+    }
+    const float cxx = hx_cof(Jy[1], Jz[2], Jz[1], Jy[2]), cxy = hx_cof(Jz[0], Jy[2], Jy[0], Jz[2]),
+                cxz = hx_cof(Jy[0], Jz[1], Jz[0], Jy[1]);
+    const float cyx = hx_cof(Jz[1], Jx[2], Jx[1], Jz[2]), cyy = hx_cof(Jx[0], Jz[2], Jz[0], Jx[2]),
+                cyz = hx_cof(Jz[0], Jx[1], Jx[0], Jz[1]);
+    const float czx = hx_cof(Jx[1], Jy[2], Jy[1], Jx[2]), czy = hx_cof(Jy[0], Jx[2], Jx[0], Jy[2]),
+                czz = hx_cof(Jx[0], Jy[1], Jy[0], Jx[1]);
+    const float det = __fmaf_rn(Jx[2], cxz, __fmaf_rn(Jx[1], cxy, Jx[0] * cxx));
+    const float r = __fdiv_rn(1.0f, det);
+    dx = r * __fmaf_rn(G[2], cxz, __fmaf_rn(G[1], cxy, G[0] * cxx));
+    dy = r * __fmaf_rn(G[2], cyz, __fmaf_rn(G[1], cyy, G[0] * cyx));
+    dz = r * __fmaf_rn(G[2], czz, __fmaf_rn(G[1], czy, G[0] * czx));
+    x = x - dx; y = y - dy; z = z - dz;
+  }
+  const float t = MESH_TOL;
+  const bool converged = fabsf(dx) <= t && fabsf(dy) <= t && fabsf(dz) <= t;
+  return converged && (x >= -t && x <= 1.0f + t) && (y >= -t && y <= 1.0f + t) && (z >= -t && z <= 1.0f + t);
+}
+
+// U2 + U3.  Returns the located cell or -1; xi is valid when a cell is returned.
+// The bounding-box pre-test only skips cells that cannot pass U3 (a converged xi inside the unit
+// cube +- TOL maps into the box +- TOL x its extent, and `margin` is 50 times that), so the located
+// cell is the same with and without it.
+__device__ __forceinline__ long long hx_locate(const MeshDev& m, float px, float py, float pz, float& x,
+                                               float& y, float& z) {
+  if (!((px >= m.lox && px <= m.hix) && (py >= m.loy && py <= m.hiy) && (pz >= m.loz && pz <= m.hiz))) return -1;
+  const int bx = min(__float2int_rd((px - m.lox) * m.sx), m.nbx - 1);
+  const int by = min(__float2int_rd((py - m.loy) * m.sy), m.nby - 1);
+  const int bz = min(__float2int_rd((pz - m.loz) * m.sz), m.nbz - 1);
+  const unsigned id = ((unsigned)bz * m.nby + by) * m.nbx + bx;
+  const unsigned k1 = m.bin_start[id + 1];
+  for (unsigned k = m.bin_start[id]; k < k1; ++k) {
+    const unsigned c = m.bin_items[k];
+    const float* rec = m.cells + (size_t)c * MESH_REC;
+    const float g = m.margin;
+    if (px < rec[48] - g || px > rec[51] + g || py < rec[49] - g || py > rec[52] + g || pz < rec[50] - g ||
+        pz > rec[53] + g)
+      continue;
+    float P[24];
+#pragma unroll
+    for (int i = 0; i < 24; i += 4) {
+      const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
+      P[i] = q.x; P[i + 1] = q.y; P[i + 2] = q.z; P[i + 3] = q.w;
+    }
+    if (hx_invert(P, px, py, pz, x, y, z)) return (long long)c;
+  }
+  return -1;
+}
+
+// U4: value at reference coordinates xi of cell c.
+__device__ __forceinline__ void hx_value(const MeshDev& m, long long c, float x, float y, float z, float& vx,
+                                         float& vy, float& vz) {
+  const float* rec = m.cells + (size_t)c * MESH_REC + 24;
+  float Q[24];
+#pragma unroll
+  for (int i = 0; i < 24; i += 4) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
+    Q[i] = q.x; Q[i + 1] = q.y; Q[i + 2] = q.z; Q[i + 3] = q.w;
+  }
+  vx = hx_tri(Q, x, y, z); vy = hx_tri(Q + 8, x, y, z); vz = hx_tri(Q + 16, x, y, z);
+}
+
+// a2-a4 alone on a mesh
+static __global__ void mesh_sample_kernel(const MeshDev m, const float* __restrict__ pts, unsigned long long n,
+                                          float* __restrict__ out_v, long long* __restrict__ out_cell) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float x, y, z, vx = 0.f, vy = 0.f, vz = 0.f;
+  const long long c = hx_locate(m, pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], x, y, z);
+  if (c >= 0) hx_value(m, c, x, y, z, vx, vy, vz);
+  out_v[3 * i] = vx; out_v[3 * i + 1] = vy; out_v[3 * i + 2] = vz;
+  if (out_cell) out_cell[i] = c;
+}
+
+struct MeshTraceArgs {
+  MeshDev m;
+  const float* seeds; unsigned long long n;
+  float h, h2, h6, vmin2; unsigned max_steps;
+  float* verts; unsigned cap, stride;
+  unsigned* counts; unsigned* steps; unsigned* status; float* fin;
+  unsigned long long* totals;
+};
+
+// RK4 streamlines on a mesh (A4-A6 with S := the mesh sample, "inside" := a cell is located).
+// One thread per particle.  The cell and xi located for p_new are reused for the next step's k1
+// (the same point: the same result).
+static __global__ void __launch_bounds__(128) mesh_trace_kernel(const MeshTraceArgs a) {
+  __shared__ unsigned long long s_tot[3];
+  if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
+  __syncthreads();
+  const unsigned long long id = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id < a.n) {
+    float px = a.seeds[3 * id], py = a.seeds[3 * id + 1], pz = a.seeds[3 * id + 2];
+    const unsigned long long plane = a.n * a.cap;
+    unsigned n = 0, slot = 0, st = ST_ALIVE, samples = 0, attempts = 0;
+    float x, y, z;
+    long long c = hx_locate(a.m, px, py, pz, x, y, z);
+    auto record = [&](unsigned k) {
+      if (k % a.stride == 0u && k / a.stride < a.cap) {
+        if (a.verts) { const unsigned long long o = id * a.cap + k / a.stride; a.verts[o] = px; a.verts[plane + o] = py; a.verts[2 * plane + o] = pz; }
+        slot = k / a.stride + 1u;
+      }
+    };
+    if (c < 0) st = ST_OUT;                                                     // A5.1
+    else record(0u);
+    while (st == ST_ALIVE) {
+      if (n == a.max_steps) { st = ST_MAXSTEPS; break; }                        // A5.2
+      float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z, qx, qy, qz;
+      hx_value(a.m, c, x, y, z, k1x, k1y, k1z); samples++;                      // A5.3
+      const float mm = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));
+      if (mm < a.vmin2) { st = ST_STAGNANT; break; }
+      attempts++;
+      qx = __fmaf_rn(a.h2, k1x, px); qy = __fmaf_rn(a.h2, k1y, py); qz = __fmaf_rn(a.h2, k1z, pz);
+      long long cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+      if (cq < 0) { st = ST_OUT; break; }
+      hx_value(a.m, cq, x, y, z, k2x, k2y, k2z);
+      qx = __fmaf_rn(a.h2, k2x, px); qy = __fmaf_rn(a.h2, k2y, py); qz = __fmaf_rn(a.h2, k2z, pz);
+      cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+      if (cq < 0) { st = ST_OUT; break; }
+      hx_value(a.m, cq, x, y, z, k3x, k3y, k3z);
+      qx = __fmaf_rn(a.h, k3x, px); qy = __fmaf_rn(a.h, k3y, py); qz = __fmaf_rn(a.h, k3z, pz);
+      cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+      if (cq < 0) { st = ST_OUT; break; }
+      hx_value(a.m, cq, x, y, z, k4x, k4y, k4z);
+      const float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
+      const float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
+      const float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
+      const float nx = __fmaf_rn(a.h6, sx, px), ny = __fmaf_rn(a.h6, sy, py), nz = __fmaf_rn(a.h6, sz, pz);
+      cq = hx_locate(a.m, nx, ny, nz, x, y, z);                                 // A5.5
+      if (cq < 0) { st = ST_OUT; break; }
+      px = nx; py = ny; pz = nz; c = cq; n++;                                   // A5.6
+      record(n);
+    }
+    if (a.counts) a.counts[id] = slot;
+    if (a.steps) a.steps[id] = n;
+    if (a.status) a.status[id] = st;
+    if (a.fin) { a.fin[id] = px; a.fin[a.n + id] = py; a.fin[2 * a.n + id] = pz; }
+    atomicAdd(&s_tot[0], (unsigned long long)attempts);
+    atomicAdd(&s_tot[1], (unsigned long long)n);
+    atomicAdd(&s_tot[2], (unsigned long long)samples);
+  }
+  __syncthreads();
+  if (a.totals && threadIdx.x < 3 && s_tot[threadIdx.x]) atomicAdd(a.totals + threadIdx.x, s_tot[threadIdx.x]);
+}
+
+}  // namespace streami
