@@ -6,6 +6,7 @@
 
 #include "internal.h"
 #include "mesh.cuh"
+#include "sorter.cuh"
 
 struct streami_mesh_s {
   streami::MeshDev d;
@@ -128,11 +129,29 @@ int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n,
   a.max_steps = params->max_steps; a.verts = out_vertices; a.cap = params->capacity; a.stride = params->stride;
   a.counts = out_counts; a.steps = params->out_steps; a.status = params->out_status; a.fin = params->out_final;
   a.totals = params->out_totals;
+  // a12: process the seeds in Morton order of their bins (order only; outputs are indexed by id)
+  unsigned* perm = nullptr; MortonSorter sorter{}; bool have_sorter = false;
+  if (options().presort && n >= 65536) {
+    streami_field_s shape{};               // the bin grid as an index space for the sort keys
+    shape.dims[0] = m->d.nbx + 1; shape.dims[1] = m->d.nby + 1; shape.dims[2] = m->d.nbz + 1;
+    shape.g.ox = m->d.lox; shape.g.oy = m->d.loy; shape.g.oz = m->d.loz;
+    shape.g.rx = m->d.sx; shape.g.ry = m->d.sy; shape.g.rz = m->d.sz;
+    shape.g.topx = (float)m->d.nbx; shape.g.topy = (float)m->d.nby; shape.g.topz = (float)m->d.nbz;
+    cudaError_t e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+    if (e != cudaSuccess) return check(e);
+    rc = sorter.init(&shape, n, st);
+    if (rc == STREAMI_OK) { have_sorter = true; rc = sorter.sort(shape.g, seeds, 3, n, nullptr, perm); }
+    if (rc) { cudaFreeAsync(perm, st); if (have_sorter) sorter.release(); return rc; }
+    a.perm = perm;
+  }
   timing_begin(st);
   mesh_trace_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a);
   timing_end(st);
-  STREAMI_LAUNCHED();
-  return STREAMI_OK;
+  launch_counter()++;
+  cudaError_t e = cudaGetLastError();
+  if (perm) cudaFreeAsync(perm, st);
+  if (have_sorter) sorter.release();
+  return check(e);
 }
 
 }  // extern "C"

@@ -129,6 +129,7 @@ static __global__ void mesh_sample_kernel(const MeshDev m, const float* __restri
 struct MeshTraceArgs {
   MeshDev m;
   const float* seeds; unsigned long long n;
+  const unsigned* perm;                 // optional processing order (Morton sort of the seeds' bins), or NULL
   float h, h2, h6, vmin2; unsigned max_steps;
   float* verts; unsigned cap, stride;
   unsigned* counts; unsigned* steps; unsigned* status; float* fin;
@@ -142,8 +143,9 @@ static __global__ void __launch_bounds__(128) mesh_trace_kernel(const MeshTraceA
   __shared__ unsigned long long s_tot[3];
   if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
   __syncthreads();
-  const unsigned long long id = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (id < a.n) {
+  const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid < a.n) {
+    const unsigned long long id = a.perm ? a.perm[tid] : tid;
     float px = a.seeds[3 * id], py = a.seeds[3 * id + 1], pz = a.seeds[3 * id + 2];
     const unsigned long long plane = a.n * a.cap;
     unsigned n = 0, slot = 0, st = ST_ALIVE, samples = 0, attempts = 0;
