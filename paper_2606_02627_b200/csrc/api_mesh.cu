@@ -137,18 +137,28 @@ int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n,
     shape.g.ox = m->d.lox; shape.g.oy = m->d.loy; shape.g.oz = m->d.loz;
     shape.g.rx = m->d.sx; shape.g.ry = m->d.sy; shape.g.rz = m->d.sz;
     shape.g.topx = (float)m->d.nbx; shape.g.topy = (float)m->d.nby; shape.g.topz = (float)m->d.nbz;
-    cudaError_t e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
-    if (e != cudaSuccess) return check(e);
+    cudaError_t e0 = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+    if (e0 != cudaSuccess) return check(e0);
     rc = sorter.init(&shape, n, st);
     if (rc == STREAMI_OK) { have_sorter = true; rc = sorter.sort(shape.g, seeds, 3, n, nullptr, perm); }
     if (rc) { cudaFreeAsync(perm, st); if (have_sorter) sorter.release(); return rc; }
     a.perm = perm;
   }
-  timing_begin(st);
-  mesh_trace_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a);
-  timing_end(st);
-  launch_counter()++;
-  cudaError_t e = cudaGetLastError();
+  unsigned long long* next = nullptr;
+  cudaError_t e = cudaMallocAsync((void**)&next, sizeof(unsigned long long), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(next, 0, sizeof(unsigned long long), st);
+  int per_sm = 0;
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mesh_trace_kernel, 128, 0);
+  if (e == cudaSuccess) {
+    a.next = next;
+    const unsigned long long want = (n + 127) / 128, full = (unsigned long long)std::max(per_sm, 1) * num_sms();
+    timing_begin(st);
+    mesh_trace_kernel<<<(unsigned)std::max(1ull, std::min(want, full)), 128, 0, st>>>(a);   // persistent grid
+    timing_end(st);
+    launch_counter()++;
+    e = cudaGetLastError();
+  }
+  if (next) cudaFreeAsync(next, st);
   if (perm) cudaFreeAsync(perm, st);
   if (have_sorter) sorter.release();
   return check(e);

@@ -130,6 +130,7 @@ struct MeshTraceArgs {
   MeshDev m;
   const float* seeds; unsigned long long n;
   const unsigned* perm;                 // optional processing order (Morton sort of the seeds' bins), or NULL
+  unsigned long long* next;             // global work counter (zeroed by the host)
   float h, h2, h6, vmin2; unsigned max_steps;
   float* verts; unsigned cap, stride;
   unsigned* counts; unsigned* steps; unsigned* status; float* fin;
@@ -137,56 +138,26 @@ struct MeshTraceArgs {
 };
 
 // RK4 streamlines on a mesh (A4-A6 with S := the mesh sample, "inside" := a cell is located).
-// One thread per particle.  The cell and xi located for p_new are reused for the next step's k1
-// (the same point: the same result).
+// Persistent grid, one lane per particle; a lane whose particle has ended takes the next work item
+// from a global counter, so that all lanes of a warp take one RK4 step per iteration.  The cell
+// and xi located for p_new are reused for the next step's k1 (the same point: the same result).
 static __global__ void __launch_bounds__(128) mesh_trace_kernel(const MeshTraceArgs a) {
   __shared__ unsigned long long s_tot[3];
   if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
   __syncthreads();
-  const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid < a.n) {
-    const unsigned long long id = a.perm ? a.perm[tid] : tid;
-    float px = a.seeds[3 * id], py = a.seeds[3 * id + 1], pz = a.seeds[3 * id + 2];
-    const unsigned long long plane = a.n * a.cap;
-    unsigned n = 0, slot = 0, st = ST_ALIVE, samples = 0, attempts = 0;
-    float x, y, z;
-    long long c = hx_locate(a.m, px, py, pz, x, y, z);
-    auto record = [&](unsigned k) {
-      if (k % a.stride == 0u && k / a.stride < a.cap) {
-        if (a.verts) { const unsigned long long o = id * a.cap + k / a.stride; a.verts[o] = px; a.verts[plane + o] = py; a.verts[2 * plane + o] = pz; }
-        slot = k / a.stride + 1u;
-      }
-    };
-    if (c < 0) st = ST_OUT;                                                     // A5.1
-    else record(0u);
-    while (st == ST_ALIVE) {
-      if (n == a.max_steps) { st = ST_MAXSTEPS; break; }                        // A5.2
-      float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z, qx, qy, qz;
-      hx_value(a.m, c, x, y, z, k1x, k1y, k1z); samples++;                      // A5.3
-      const float mm = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));
-      if (mm < a.vmin2) { st = ST_STAGNANT; break; }
-      attempts++;
-      qx = __fmaf_rn(a.h2, k1x, px); qy = __fmaf_rn(a.h2, k1y, py); qz = __fmaf_rn(a.h2, k1z, pz);
-      long long cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-      if (cq < 0) { st = ST_OUT; break; }
-      hx_value(a.m, cq, x, y, z, k2x, k2y, k2z);
-      qx = __fmaf_rn(a.h2, k2x, px); qy = __fmaf_rn(a.h2, k2y, py); qz = __fmaf_rn(a.h2, k2z, pz);
-      cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-      if (cq < 0) { st = ST_OUT; break; }
-      hx_value(a.m, cq, x, y, z, k3x, k3y, k3z);
-      qx = __fmaf_rn(a.h, k3x, px); qy = __fmaf_rn(a.h, k3y, py); qz = __fmaf_rn(a.h, k3z, pz);
-      cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-      if (cq < 0) { st = ST_OUT; break; }
-      hx_value(a.m, cq, x, y, z, k4x, k4y, k4z);
-      const float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
-      const float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
-      const float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
-      const float nx = __fmaf_rn(a.h6, sx, px), ny = __fmaf_rn(a.h6, sy, py), nz = __fmaf_rn(a.h6, sz, pz);
-      cq = hx_locate(a.m, nx, ny, nz, x, y, z);                                 // A5.5
-      if (cq < 0) { st = ST_OUT; break; }
-      px = nx; py = ny; pz = nz; c = cq; n++;                                   // A5.6
-      record(n);
+  const unsigned long long plane = a.n * a.cap;
+  unsigned long long id = 0;
+  float px = 0.f, py = 0.f, pz = 0.f, x = 0.f, y = 0.f, z = 0.f;
+  long long c = -1;
+  unsigned n = 0, slot = 0, samples = 0, attempts = 0;
+  bool active = false, exhausted = false;
+  auto record = [&](unsigned k) {
+    if (k % a.stride == 0u && k / a.stride < a.cap) {
+      if (a.verts) { const unsigned long long o = id * a.cap + k / a.stride; a.verts[o] = px; a.verts[plane + o] = py; a.verts[2 * plane + o] = pz; }
+      slot = k / a.stride + 1u;
     }
+  };
+  auto finish = [&](unsigned st) {
     if (a.counts) a.counts[id] = slot;
     if (a.steps) a.steps[id] = n;
     if (a.status) a.status[id] = st;
@@ -194,6 +165,57 @@ static __global__ void __launch_bounds__(128) mesh_trace_kernel(const MeshTraceA
     atomicAdd(&s_tot[0], (unsigned long long)attempts);
     atomicAdd(&s_tot[1], (unsigned long long)n);
     atomicAdd(&s_tot[2], (unsigned long long)samples);
+    active = false;
+  };
+  for (;;) {
+    if (!active && !exhausted) {                                                // a1: refill
+      const unsigned long long w = atomicAdd(a.next, 1ull);
+      if (w >= a.n) exhausted = true;
+      else {
+        id = a.perm ? a.perm[w] : w;
+        px = a.seeds[3 * id]; py = a.seeds[3 * id + 1]; pz = a.seeds[3 * id + 2];
+        n = 0; slot = 0; samples = 0; attempts = 0; active = true;
+        c = hx_locate(a.m, px, py, pz, x, y, z);
+        if (c < 0) finish(ST_OUT);                                              // A5.1
+        else record(0u);
+      }
+    }
+    if (__all_sync(0xffffffffu, !active)) {
+      if (__all_sync(0xffffffffu, exhausted)) break;
+      continue;
+    }
+    if (active) {
+      unsigned st = ST_ALIVE;
+      do {
+        if (n == a.max_steps) { st = ST_MAXSTEPS; break; }                      // A5.2
+        float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z, qx, qy, qz;
+        hx_value(a.m, c, x, y, z, k1x, k1y, k1z); samples++;                    // A5.3
+        const float mm = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));
+        if (mm < a.vmin2) { st = ST_STAGNANT; break; }
+        attempts++;
+        qx = __fmaf_rn(a.h2, k1x, px); qy = __fmaf_rn(a.h2, k1y, py); qz = __fmaf_rn(a.h2, k1z, pz);
+        long long cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+        if (cq < 0) { st = ST_OUT; break; }
+        hx_value(a.m, cq, x, y, z, k2x, k2y, k2z);
+        qx = __fmaf_rn(a.h2, k2x, px); qy = __fmaf_rn(a.h2, k2y, py); qz = __fmaf_rn(a.h2, k2z, pz);
+        cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+        if (cq < 0) { st = ST_OUT; break; }
+        hx_value(a.m, cq, x, y, z, k3x, k3y, k3z);
+        qx = __fmaf_rn(a.h, k3x, px); qy = __fmaf_rn(a.h, k3y, py); qz = __fmaf_rn(a.h, k3z, pz);
+        cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
+        if (cq < 0) { st = ST_OUT; break; }
+        hx_value(a.m, cq, x, y, z, k4x, k4y, k4z);
+        const float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
+        const float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
+        const float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
+        const float nx = __fmaf_rn(a.h6, sx, px), ny = __fmaf_rn(a.h6, sy, py), nz = __fmaf_rn(a.h6, sz, pz);
+        cq = hx_locate(a.m, nx, ny, nz, x, y, z);                               // A5.5
+        if (cq < 0) { st = ST_OUT; break; }
+        px = nx; py = ny; pz = nz; c = cq; n++;                                 // A5.6
+        record(n);
+      } while (false);
+      if (st != ST_ALIVE) finish(st);
+    }
   }
   __syncthreads();
   if (a.totals && threadIdx.x < 3 && s_tot[threadIdx.x]) atomicAdd(a.totals + threadIdx.x, s_tot[threadIdx.x]);
