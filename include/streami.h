@@ -278,6 +278,7 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
  *   "segment_steps"     K     streamlines: K step attempts per particle per launch, survivors are
  *                             re-sorted between launches (0 = one launch; DP5(4) then synchronises)
  *   "prefetch"          0/1/2 RK4: request the predicted next cell one step ahead (2: two points)
+ *   "integer_accept"    0/1   steady RK4 on a field of finite values: decide "inside" from floor(g)
  *   "vertex_staging"    0/1   stage vertices in shared memory and store full 32-byte sectors
  *   "max_blocks_per_sm" B     limit resident blocks per SM (0 = as many as fit)
  *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0)

@@ -12,7 +12,7 @@
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0}; return o; }
+Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0, 1}; return o; }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -184,6 +184,7 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.hix = dims[0] - 1; s.hiy = dims[1] - 1; s.hiz = dims[2] - 1;
   s.topflagx = s.topflagy = s.topflagz = 1;
   s.cmx = s.hix - 1; s.cmy = s.hiy - 1; s.cmz = s.hiz - 1;
+  s.fastx = s.fasty = s.fastz = 0u;
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
@@ -200,6 +201,20 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   }
   f->layout = layout;
   if (rc) { delete f; return rc; }
+  f->tame = false;
+  if (nslices == 1) {                 // only the steady RK4 path asks (sample_nb)
+    unsigned* flag = nullptr; unsigned bad = 1u;
+    cudaError_t e = cudaMalloc((void**)&flag, sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemset(flag, 0, sizeof(unsigned));
+    if (e == cudaSuccess) {
+      tame_scan_kernel<<<148 * 8, 256>>>(dev_ptr, 3ull * s.slice_stride, flag);
+      launch_counter()++;
+      e = cudaMemcpy(&bad, flag, sizeof(unsigned), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(flag);
+    if (e != cudaSuccess) { if (bytes) cudaFree(data); delete f; return check(e); }
+    f->tame = bad == 0u;
+  }
   if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
   s.data = data;
   if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
@@ -269,6 +284,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
           }
           s.olox = ol[0]; s.oloy = ol[1]; s.oloz = ol[2]; s.ohix = oh[0]; s.ohiy = oh[1]; s.ohiz = oh[2];
         }
+        s.fastx = s.fasty = s.fastz = 0u;
         s.nx = (unsigned)(hi[0] - lo[0] + 1);
         s.nxy = s.nx * (unsigned)(hi[1] - lo[1] + 1);
         s.slice_stride = (unsigned long long)s.nxy * (unsigned)(hi[2] - lo[2] + 1);
@@ -362,6 +378,7 @@ int streami_set_option(const char* name, int value) {
   else if (!strcmp(name, "brick_round_steps")) o.brick_round_steps = value < -1 ? -1 : value;
   else if (!strcmp(name, "max_blocks_per_sm")) o.max_blocks_per_sm = value < 0 ? 0 : value;
   else if (!strcmp(name, "prefetch")) o.prefetch = value < 0 ? 0 : (value > 2 ? 2 : value);
+  else if (!strcmp(name, "integer_accept")) o.integer_accept = value != 0;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }
@@ -378,6 +395,7 @@ int streami_get_option(const char* name, int* value) {
   else if (!strcmp(name, "brick_round_steps")) *value = o.brick_round_steps;
   else if (!strcmp(name, "max_blocks_per_sm")) *value = o.max_blocks_per_sm;
   else if (!strcmp(name, "prefetch")) *value = o.prefetch;
+  else if (!strcmp(name, "integer_accept")) *value = o.integer_accept;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }

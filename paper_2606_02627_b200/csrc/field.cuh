@@ -39,6 +39,9 @@ struct Store {
   // an axis): floor(g) inside it <=> owner(g) == this brick, without the integer divisions of A9.
   int olox, oloy, oloz, ohix, ohiy, ohiz;
   unsigned nx, nxy;        // row and plane strides in records (vertices; LAYOUT_CELL: cells)
+  // Monolithic steady stores: cells per axis if every stored value is tame (finite, |v| <= 2^60),
+  // else 0.  See sample_nb: floor(g) < fast on all axes then decides "inside" with integers.
+  unsigned fastx, fasty, fastz;
   unsigned long long slice_stride;   // records per slice
 };
 
@@ -291,9 +294,27 @@ __device__ __forceinline__ unsigned sample_nb(const Geom& g, const Store& s, Cel
                         (gz >= s.floz) && (gz < s.fhiz);
     rc = served ? 0u : (unsigned)ST_HALO;
   }
-  if (!KNOWN) rc = in_domain(g, gx, gy, gz) ? rc : (unsigned)ST_OUT;      // OUT wins over HALO (A9)
-  int ix = min(__float2int_rz(gx), s.cmx), iy = min(__float2int_rz(gy), s.cmy), iz = min(__float2int_rz(gz), s.cmz);
-  if (!KNOWN || BRICK) { ix = max(ix, BRICK ? s.lox : 0); iy = max(iy, BRICK ? s.loy : 0); iz = max(iz, BRICK ? s.loz : 0); }
+  int ix, iy, iz;
+  if constexpr (!BRICK && !KNOWN) {
+    // Integer accept: 0 <= floor(g) <= N-2 on every axis <=> 0 <= g < N-1, which is inside the
+    // closed box and needs no clamp (floor = truncation there).  Everything else -- outside, on
+    // the top face g == N-1, +-inf (the conversion saturates) -- takes the exact float test.  A NaN
+    // converts to 0 and would be accepted, so `fast` is 0 unless the field is tame: with finite
+    // values <= 2^60 no lerp forms inf - inf or 0 * inf, and a stage point fma(h, k, p) of finite
+    // operands is finite or +-inf, never NaN.  3 integer compares replace 6 float compares and 6
+    // clamps per stage sample.
+    ix = __float2int_rd(gx); iy = __float2int_rd(gy); iz = __float2int_rd(gz);
+    const bool fast = ((unsigned)ix < s.fastx) & ((unsigned)iy < s.fasty) & ((unsigned)iz < s.fastz);
+    if (__builtin_expect(!fast, 0)) {
+      rc = in_domain(g, gx, gy, gz) ? 0u : (unsigned)ST_OUT;
+      ix = max(min(__float2int_rz(gx), s.cmx), 0); iy = max(min(__float2int_rz(gy), s.cmy), 0);
+      iz = max(min(__float2int_rz(gz), s.cmz), 0);
+    }
+  } else {
+    if (!KNOWN) rc = in_domain(g, gx, gy, gz) ? rc : (unsigned)ST_OUT;      // OUT wins over HALO (A9)
+    ix = min(__float2int_rz(gx), s.cmx); iy = min(__float2int_rz(gy), s.cmy); iz = min(__float2int_rz(gz), s.cmz);
+    if (!KNOWN || BRICK) { ix = max(ix, BRICK ? s.lox : 0); iy = max(iy, BRICK ? s.loy : 0); iz = max(iz, BRICK ? s.loz : 0); }
+  }
   const float fx = gx - (float)ix, fy = gy - (float)iy, fz = gz - (float)iz;
   if (BRICK) { ix -= s.lox; iy -= s.loy; iz -= s.loz; }
   const unsigned v32 = (unsigned)iz * s.nxy + (unsigned)iy * s.nx + (unsigned)ix;

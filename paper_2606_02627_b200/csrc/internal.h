@@ -12,6 +12,7 @@ struct streami_field_s {
   int dims[3];                       // global vertex counts
   int layout;
   bool bricked;
+  bool tame;                         // every stored value finite and <= 2^60 (monolithic; see sample_nb)
   streami::Store store;              // monolithic
   std::vector<streami::Store> bricks;  // host copies
   streami::Store* d_bricks;          // device table
@@ -22,7 +23,7 @@ struct streami_field_s {
 
 namespace streami {
 
-struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; int segment_steps; int vertex_staging; int prefetch; int max_blocks_per_sm; int brick_round_steps; };
+struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; int segment_steps; int vertex_staging; int prefetch; int max_blocks_per_sm; int brick_round_steps; int integer_accept; };
 Options& options();
 std::atomic<unsigned long long>& launch_counter();
 void set_cuda_error(cudaError_t e);

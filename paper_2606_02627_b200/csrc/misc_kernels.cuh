@@ -14,6 +14,15 @@ static __global__ void repack_float4_kernel(const float* __restrict__ src, float
     dst[v] = make_float4(src[3 * v], src[3 * v + 1], src[3 * v + 2], 0.0f);
 }
 
+// Tame scan: *flag |= 1 if any of the n floats is NaN, infinite or above 2^60 in magnitude.
+static __global__ void tame_scan_kernel(const float* __restrict__ src, unsigned long long n, unsigned* flag) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  bool bad = false;
+  for (; i < n; i += step) bad |= !(fabsf(src[i]) <= 1.152921504606846976e18f);
+  if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flag, 1u);
+}
+
 // XPAIR record v = {V[v].xyz, (V[v+1] - V[v]).xyz, 0, 0} (the difference is the x-lerp's own
 // subtraction, done once here in fp32; see LayoutTraits in field.cuh); the last vertex of a row
 // pairs with itself (its upper half is never used: i_x <= nx-2).

@@ -1,6 +1,7 @@
 """Schedule-only options must not change any result: segments with Morton re-sort of the survivors
 (`segment_steps`), the one-step-ahead cell prefetch (`prefetch`), the staged vertex writer
-(`vertex_staging`), the occupancy limit (`max_blocks_per_sm`).  Each combination is compared bit for
+(`vertex_staging`), the occupancy limit (`max_blocks_per_sm`), the integer domain test
+(`integer_accept`).  Each combination is compared bit for
 bit with the oracle (RK4 and DP5(4), every layout family), with capacities that are and are not a
 multiple of the 8-slot staging group, and with a stride that cuts groups at segment boundaries."""
 import numpy as np
@@ -97,3 +98,43 @@ def test_unaligned_vertex_array_uses_scalar_stores(S, torch, oracle, wl, turb48)
         torch.cuda.synchronize()
         assert np.array_equal(counts.cpu().numpy().astype(np.uint32), ref.counts)
         assert np.array_equal(verts.cpu().numpy().view(np.uint32), ref.vertices.view(np.uint32)), shift
+
+
+@pytest.mark.parametrize("layout", [1, 3, 5])
+@pytest.mark.parametrize("kind", ["tame", "nan", "inf", "huge", "big_tame"])
+def test_integer_accept_keeps_the_domain_test_exact(S, torch, oracle, wl, turb48, layout, kind):
+    """`integer_accept` decides "inside" from floor(g) when every field value is finite and <= 2^60;
+    a field with NaN, infinite or larger values must take the float test (the library finds out at
+    create time).  Seeds sit on the faces g = 0 and g = N-1 as well; a step of 1e30 sends stage
+    points to +-inf.  All of it is compared bit for bit with the oracle, option on and off."""
+    import dataclasses
+    data = turb48.data.copy()
+    rng = np.random.default_rng(5)
+    idx = rng.integers(0, 48, size=(400, 3))
+    if kind == "nan":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.nan
+    elif kind == "inf":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.where(idx[:, 1] % 2, np.inf, -np.inf)
+    elif kind == "huge":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.where(idx[:, 1] % 2, 3e38, -3e38)
+    elif kind == "big_tame":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.where(idx[:, 1] % 2, 1e18, -1e18)
+    fld = dataclasses.replace(turb48, data=data)
+    n = 6000
+    seeds = wl.seeds_uniform(21, n, [47.0] * 3)
+    seeds[:600] = np.round(seeds[:600])                     # on vertices, many on the faces 0 and 47
+    seeds[600:900, 0] = 47.0; seeds[900:1200, 1] = 0.0; seeds[1200:1500, 2] = 47.0
+    seeds[1500:1700] = idx[:200] + 0.5                      # next to the planted values
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing)
+    f = gpu_field(S, torch, fld, layout)
+    for kw in (dict(integrator=0, h=0.25, max_steps=80, vmin=1e-6, capacity=16, stride=5),
+               dict(integrator=0, h=1e30, max_steps=3, vmin=0.0, capacity=4, stride=1)):
+        ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
+        assert kw["h"] > 1.0 or len(set(ref.status.tolist())) >= 2
+        for on in (1, 0):
+            try:
+                S.streami_set_option("integer_accept", on)
+                out = gpu_streamlines(S, torch, f, seeds, **kw)
+            finally:
+                S.streami_set_option("integer_accept", 1)
+            assert_same(out, ref, "%s integer_accept=%d %s" % (kind, on, kw))
