@@ -23,7 +23,7 @@ static __global__ void tame_scan_kernel(const float* __restrict__ src, unsigned 
   if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flag, 1u);
 }
 
-// XPAIR record v = {V[v].xyz, (V[v+1] - V[v]).xyz, 0, 0} (the difference is the x-lerp's own
+// XPAIR record v = {Vx, Vy, Dx, Dy, Vz, Dz, 0, 0} with V = V[v], D = V[v+1] - V[v] (the difference is the x-lerp's own
 // subtraction, done once here in fp32; see LayoutTraits in field.cuh); the last vertex of a row
 // pairs with itself (its upper half is never used: i_x <= nx-2).
 static __global__ void repack_xpair_kernel(const float* __restrict__ src, float4* __restrict__ dst,
@@ -34,8 +34,8 @@ static __global__ void repack_xpair_kernel(const float* __restrict__ src, float4
     unsigned long long w = ((v % nx) == nx - 1) ? v : v + 1;
     float a0 = src[3 * v], a1 = src[3 * v + 1], a2 = src[3 * v + 2];
     float b0 = src[3 * w], b1 = src[3 * w + 1], b2 = src[3 * w + 2];
-    dst[2 * v] = make_float4(a0, a1, a2, b0 - a0);
-    dst[2 * v + 1] = make_float4(b1 - a1, b2 - a2, 0.0f, 0.0f);
+    dst[2 * v] = make_float4(a0, a1, b0 - a0, b1 - a1);
+    dst[2 * v + 1] = make_float4(a2, b2 - a2, 0.0f, 0.0f);
   }
 }
 
@@ -52,8 +52,8 @@ static __global__ void repack_xyquad_kernel(const float* __restrict__ src, float
     const unsigned long long w = (x == nx - 1) ? v : v + 1;
     const float a0 = src[3 * v], a1 = src[3 * v + 1], a2 = src[3 * v + 2];
     const float b0 = src[3 * w], b1 = src[3 * w + 1], b2 = src[3 * w + 2];
-    dst[2 * t] = make_float4(a0, a1, a2, b0 - a0);
-    dst[2 * t + 1] = make_float4(b1 - a1, b2 - a2, 0.0f, 0.0f);
+    dst[2 * t] = make_float4(a0, a1, b0 - a0, b1 - a1);
+    dst[2 * t + 1] = make_float4(a2, b2 - a2, 0.0f, 0.0f);
   }
 }
 
@@ -75,8 +75,8 @@ static __global__ void repack_cell_kernel(const float* __restrict__ src, float4*
     const unsigned ix = (unsigned)(c % cx), iy = (unsigned)((c / cx) % cy), iz = (unsigned)(c / ((unsigned long long)cx * cy));
     const unsigned long long v = (((unsigned long long)sl * nz + iz + (r >> 1)) * ny + iy + (r & 1u)) * nx + ix;
     const float* p = src + 3ull * v;
-    dst[2 * t] = make_float4(p[0], p[1], p[2], p[3] - p[0]);
-    dst[2 * t + 1] = make_float4(p[4] - p[1], p[5] - p[2], 0.0f, 0.0f);
+    dst[2 * t] = make_float4(p[0], p[1], p[3] - p[0], p[4] - p[1]);
+    dst[2 * t + 1] = make_float4(p[2], p[5] - p[2], 0.0f, 0.0f);
   }
 }
 
