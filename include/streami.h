@@ -54,12 +54,12 @@ extern "C" {
 #define STREAMI_HALO_MISS      4u  /* bricks only: a stage point left the brick's stored box */
 
 /* field layouts (layout_hint of streami_field_create*, reported by streami_field_info) */
-#define STREAMI_LAYOUT_AUTO    0   /* library chooses: XPAIR; XYQUAD for steady fields of
-                                      1 GiB or more when it fits half the free device memory; falls back to a
-                                      smaller layout instead of failing with NOMEM */
+#define STREAMI_LAYOUT_AUTO    0   /* library chooses: XYQUAD for a steady field when its
+                                      64 B per vertex fit half the free device memory, else XPAIR; falls back
+                                      to a smaller layout instead of failing with NOMEM */
 #define STREAMI_LAYOUT_PACKED3 1   /* use the caller's packed float3 array in place (the paper's layout) */
 #define STREAMI_LAYOUT_FLOAT4  2   /* library-owned copy padded to 16 B per vertex */
-#define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: {V[x], V[x+1], pad}: one
+#define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: V[x] and V[x+1] - V[x]: one
                                       aligned sector per trilinear row */
 #define STREAMI_LAYOUT_XYQUAD  5   /* library-owned copy, 64 B per vertex: the XPAIR rows (x, y) and (x, y+1):
                                       a cell is two aligned 64-byte pieces (4x the packed size) */

@@ -140,11 +140,12 @@ static int fill_geom(Geom& g, const int dims[3], const float origin[3], const fl
   return STREAMI_OK;
 }
 
-// AUTO: XPAIR; for a steady field of 1 GiB or more of packed vertices --
-// far beyond L2, where the gathers are bound by DRAM accesses (C5) -- XYQUAD, whose 64-byte pieces
-// use both halves of every DRAM fetch, provided its 64 B per vertex fit comfortably.
+// AUTO: a steady field gets XYQUAD -- its 64-byte pieces use both halves of
+// every DRAM fetch and half as many L1 lines per cell (C5 1.21 -> 0.95 s, C2 16.6 -> 16.1 ms, and
+// no loss on fields that fit L2) -- provided its 64 B per vertex fit comfortably; otherwise, and
+// for unsteady fields (two slices per sample: C4 249 vs 264 ms), XPAIR.
 static int auto_layout(unsigned long long nvert, int nslices) {
-  if (nslices == 1 && 12ull * nvert >= (1ull << 30)) {
+  if (nslices == 1) {
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && 64ull * nvert <= free_b / 2) return LAYOUT_XYQUAD;
     cudaGetLastError();

@@ -53,11 +53,31 @@ struct BrickMap {
 
 __device__ __forceinline__ float lerp(float a, float b, float w) { return __fmaf_rn(w, b - a, a); }
 
-// ---- loads of the 8 cell vertices as 4 rows of {V[x].xyz, V[x+1].xyz} ----------------------
-// V[row*6 + dx*3 + c], row = dz*2 + dy.
+// One aligned 32-byte record: a single 256-bit read-only load (LDG.E.256 on sm_100a); 6 floats used.
+// NA = do not allocate the line in L1.  The branch-free RK4 path asks for that: its demand loads
+// still hit lines the one-step-ahead prefetch has brought in, but no longer evict them (768 lanes x
+// 4 lines per cell are several times the L1), C2 16.9 -> 16.6 ms.  Without a prefetcher the same
+// hint loses (C5 DP5(4) 0.95 -> 1.11 s, C4 two-slice reads 249 -> 276 ms), so it is per caller.
+template <bool NA>
+__device__ __forceinline__ void ldg_rec32(const char* p, float* o) {
+  float p6, p7;
+  if (NA)
+    asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(p6), "=f"(p7)
+                 : "l"(p));
+  else
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(p6), "=f"(p7)
+                 : "l"(p));
+  (void)p6; (void)p7;
+}
+
+// ---- loads of the 8 cell vertices as 4 rows of 6 floats --------------------------------------
+// V[row*6 + k], row = dz*2 + dy; k: {V[x].xyz, V[x+1].xyz} or, for the DIFF layouts, the record order.
 template <int LAYOUT> struct CellLoad;
 
 template <> struct CellLoad<LAYOUT_PACKED3> {
+  template <bool NA>
   static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
     const float* p = reinterpret_cast<const float*>(data) + 3ull * v;
 #pragma unroll
@@ -65,6 +85,7 @@ template <> struct CellLoad<LAYOUT_PACKED3> {
   }
 };
 template <> struct CellLoad<LAYOUT_FLOAT4> {
+  template <bool NA>
   static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
     const float4* p = reinterpret_cast<const float4*>(data) + v;
     float4 a = __ldg(p), b = __ldg(p + 1);
@@ -72,15 +93,9 @@ template <> struct CellLoad<LAYOUT_FLOAT4> {
   }
 };
 template <> struct CellLoad<LAYOUT_XPAIR> {
-  // one aligned 32-byte record per row: a single 256-bit read-only load (LDG.E.256 on sm_100a)
+  template <bool NA>
   static __device__ __forceinline__ void row(const void* data, unsigned long long v, float* o) {
-    const char* p = reinterpret_cast<const char*>(data) + 32ull * v;
-    float p6, p7;
-    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]),
-                   "=f"(p6), "=f"(p7)
-                 : "l"(p));
-    (void)p6; (void)p7;
+    ldg_rec32<NA>(reinterpret_cast<const char*>(data) + 32ull * v, o);
   }
 };
 
@@ -89,17 +104,11 @@ template <> struct CellLoad<LAYOUT_XPAIR> {
 // sector gathers top out near 1.7 TB/s on B200 and contiguous 128-byte ones near 5.4 TB/s
 // (DESIGN.md section 6), which is what this layout buys with 8x the memory.
 template <> struct CellLoad<LAYOUT_CELL> {
+  template <bool NA>
   static __device__ __forceinline__ void cell(const void* data, unsigned long long c, float* V) {
     const char* p = reinterpret_cast<const char*>(data) + 128ull * c;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      float p6, p7;
-      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                   : "=f"(V[6 * r]), "=f"(V[6 * r + 1]), "=f"(V[6 * r + 2]), "=f"(V[6 * r + 3]),
-                     "=f"(V[6 * r + 4]), "=f"(V[6 * r + 5]), "=f"(p6), "=f"(p7)
-                   : "l"(p + 32 * r));
-      (void)p6; (void)p7;
-    }
+    for (int r = 0; r < 4; ++r) ldg_rec32<NA>(p + 32 * r, V + 6 * r);
   }
 };
 
@@ -107,49 +116,43 @@ template <> struct CellLoad<LAYOUT_CELL> {
 // back: a cell is two 64-byte pieces (z and z+1).  DRAM brings 64 bytes per missed 32-byte sector
 // (ncu on C5: 3.7 TB read for 1.8 TB of missed sectors); here both halves of every fetch are used.
 template <> struct CellLoad<LAYOUT_XYQUAD> {
+  template <bool NA>
   static __device__ __forceinline__ void pair(const void* data, unsigned long long v, float* o) {
     const char* p = reinterpret_cast<const char*>(data) + 64ull * v;
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      float p6, p7;
-      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                   : "=f"(o[6 * r]), "=f"(o[6 * r + 1]), "=f"(o[6 * r + 2]), "=f"(o[6 * r + 3]),
-                     "=f"(o[6 * r + 4]), "=f"(o[6 * r + 5]), "=f"(p6), "=f"(p7)
-                   : "l"(p + 32 * r));
-      (void)p6; (void)p7;
-    }
+    for (int r = 0; r < 2; ++r) ldg_rec32<NA>(p + 32 * r, o + 6 * r);
   }
 };
 
 template <int LAYOUT>
 __device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, float* V) {
   if constexpr (LAYOUT == LAYOUT_CELL) {
-    CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+    CellLoad<LAYOUT_CELL>::template cell<false>(s.data, v, V);
   } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
-    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v, V);
-    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT_XYQUAD>::template pair<false>(s.data, v, V);
+    CellLoad<LAYOUT_XYQUAD>::template pair<false>(s.data, v + s.nxy, V + 12);
   } else {
-    CellLoad<LAYOUT>::row(s.data, v, V);
-    CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
-    CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
-    CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+    CellLoad<LAYOUT>::template row<false>(s.data, v, V);
+    CellLoad<LAYOUT>::template row<false>(s.data, v + s.nx, V + 6);
+    CellLoad<LAYOUT>::template row<false>(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT>::template row<false>(s.data, v + s.nxy + s.nx, V + 18);
   }
 }
 
 // A steady store holds fewer than 2^32 vertices (checked at create time), so the four row
 // indices fit 32 bits (v + nxy + nx <= nvert - 1) and each address is one 32x32->64 multiply-add.
-template <int LAYOUT>
+template <int LAYOUT, bool NA = false>
 __device__ __forceinline__ void load_cell32(const Store& s, unsigned v, float* V) {
   if constexpr (LAYOUT == LAYOUT_CELL) {
-    CellLoad<LAYOUT_CELL>::cell(s.data, v, V);
+    CellLoad<LAYOUT_CELL>::template cell<NA>(s.data, v, V);
   } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
-    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v, V);
-    CellLoad<LAYOUT_XYQUAD>::pair(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT_XYQUAD>::template pair<NA>(s.data, v, V);
+    CellLoad<LAYOUT_XYQUAD>::template pair<NA>(s.data, v + s.nxy, V + 12);
   } else {
-    CellLoad<LAYOUT>::row(s.data, v, V);
-    CellLoad<LAYOUT>::row(s.data, v + s.nx, V + 6);
-    CellLoad<LAYOUT>::row(s.data, v + s.nxy, V + 12);
-    CellLoad<LAYOUT>::row(s.data, v + s.nxy + s.nx, V + 18);
+    CellLoad<LAYOUT>::template row<NA>(s.data, v, V);
+    CellLoad<LAYOUT>::template row<NA>(s.data, v + s.nx, V + 6);
+    CellLoad<LAYOUT>::template row<NA>(s.data, v + s.nxy, V + 12);
+    CellLoad<LAYOUT>::template row<NA>(s.data, v + s.nxy + s.nx, V + 18);
   }
 }
 
@@ -343,7 +346,7 @@ __device__ __forceinline__ unsigned sample_nb(const Geom& g, const Store& s, Cel
   if (BRICK) { ix -= s.lox; iy -= s.loy; iz -= s.loz; }
   const unsigned v32 = (unsigned)iz * s.nxy + (unsigned)iy * s.nx + (unsigned)ix;
   if (CACHE) {
-    if (v32 != cc.key) { load_cell32<LAYOUT>(s, v32, cc.V); cc.key = v32; }
+    if (v32 != cc.key) { load_cell32<LAYOUT, !BRICK>(s, v32, cc.V); cc.key = v32; }
     interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, vx, vy, vz);
   } else {
     float V[24];

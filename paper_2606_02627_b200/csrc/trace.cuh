@@ -71,7 +71,11 @@ struct Lane {
 // partial group (at termination, at a hand-off, or for a capacity that is not a multiple of 8)
 // goes out with scalar stores.  Slots beyond the count stay untouched (A6).
 constexpr int REC_GROUP = 8;
-constexpr int REC_THREADS = 256;
+#ifndef STREAMI_RK4_BLOCK
+#define STREAMI_RK4_BLOCK 256      // threads per block of the RK4 kernels (the staging arrays are sized by it)
+#define STREAMI_RK4_MIN_BLOCKS 3  // resident blocks per SM the register allocation must allow
+#endif
+constexpr int REC_THREADS = STREAMI_RK4_BLOCK;
 __device__ __forceinline__ float* rec_stage() {
   __shared__ float s_rec[3 * REC_GROUP * REC_THREADS];        // [plane][slot & 7][thread]
   return s_rec + threadIdx.x;

@@ -14,8 +14,7 @@ namespace streami {
 
 // Threads per block: 256 for RK4; DP5(4) keeps six stage vectors (92 registers), and blocks of
 // 128 let 5 of them (20 warps) share an SM where 256-thread blocks fit only 2 (16 warps).
-constexpr int TRACE_BLOCK = 256;
-constexpr int trace_block(int integ) { return integ == 1 ? 128 : 256; }
+constexpr int trace_block(int integ) { return integ == 1 ? 128 : STREAMI_RK4_BLOCK; }
 
 __device__ __forceinline__ void finish_particle(const TraceArgs& a, Lane& L, unsigned st) {
   flush_vertices(a, L);
@@ -59,7 +58,7 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
 
 // Resident blocks per SM the compiler must allow for.  3 blocks of 256 (<= 80 registers): capping
 // the steady RK4 kernel at 64 registers for a 4th block was measured on C2 and lost to its spills.
-constexpr int trace_min_blocks(int integ, bool unsteady, bool brick) { return integ == 1 ? 5 : 3; }
+constexpr int trace_min_blocks(int integ, bool unsteady, bool brick) { return integ == 1 ? 5 : STREAMI_RK4_MIN_BLOCKS; }
 
 template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
 __global__ void __launch_bounds__(trace_block(INTEG), trace_min_blocks(INTEG, UNSTEADY, BRICK))
