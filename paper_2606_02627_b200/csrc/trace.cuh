@@ -77,8 +77,9 @@ constexpr int REC_GROUP = 8;
 #endif
 constexpr int REC_THREADS = STREAMI_RK4_BLOCK;
 __device__ __forceinline__ float* rec_stage() {
-  __shared__ float s_rec[3 * REC_GROUP * REC_THREADS];        // [plane][slot & 7][thread]
-  return s_rec + threadIdx.x;
+  // [thread][plane][slot & 7]: a lane's group is 96 contiguous bytes, read back as 6 LDS.128
+  __shared__ __align__(16) float s_rec[3 * REC_GROUP * REC_THREADS];
+  return s_rec + 3 * REC_GROUP * threadIdx.x;
 }
 
 __device__ __forceinline__ float* rec_scratch() {              // never read: cp.async prefetch target
@@ -95,11 +96,10 @@ __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
     if (cnt == (unsigned)REC_GROUP && a.vec_ok) {               // stage0 is then a multiple of 8
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
-        const float* sc = s + c * REC_GROUP * REC_THREADS;
+        const float4 lo = *reinterpret_cast<const float4*>(s + c * REC_GROUP);
+        const float4 hi = *reinterpret_cast<const float4*>(s + c * REC_GROUP + 4);
         asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst + c * plane),
-                     "f"(sc[0]), "f"(sc[REC_THREADS]), "f"(sc[2 * REC_THREADS]), "f"(sc[3 * REC_THREADS]),
-                     "f"(sc[4 * REC_THREADS]), "f"(sc[5 * REC_THREADS]), "f"(sc[6 * REC_THREADS]),
-                     "f"(sc[7 * REC_THREADS])
+                     "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w)
                      : "memory");
       }
     } else {
@@ -107,34 +107,37 @@ __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
 #pragma unroll 1
       for (unsigned j = 0; j < cnt; ++j) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) dst[c * plane + j] = s[(c * REC_GROUP + j0 + j) * REC_THREADS];
+        for (int c = 0; c < 3; ++c) dst[c * plane + j] = s[c * REC_GROUP + j0 + j];
       }
     }
   }
   L.stage0 = L.slot;
 }
 
+// Called once per accepted step.  The staged path has no branch up to the flush: some lane of a warp
+// records in almost every iteration (27 lanes, stride 8, phases apart), so a branch around the
+// three shared-memory stores was taken -- and its whole body issued for 3 lanes -- nearly always.
+// Without an output array the stores still go to the staging words, which are then never read.
 template <bool REC = true>
 __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
   if (!REC) return;
-  if (--L.rec_cd == 0) {
+  if (a.staging) {
+    const bool due = --L.rec_cd == 0u;
+    L.rec_cd = due ? a.stride : L.rec_cd;
+    const bool rec = due && L.slot < a.cap;
+    float* s = rec_stage() + (L.slot & (REC_GROUP - 1));
+    if (rec) { s[0] = L.px; s[REC_GROUP] = L.py; s[2 * REC_GROUP] = L.pz; }
+    L.slot += rec ? 1u : 0u;
+    if (rec && (L.slot & (REC_GROUP - 1)) == 0u) flush_vertices(a, L);
+  } else if (--L.rec_cd == 0) {                  // option "vertex_staging" = 0 (for A/B measurement)
     L.rec_cd = a.stride;
     if (L.slot < a.cap) {
-      if (!a.staging) {                          // option "vertex_staging" = 0 (for A/B measurement)
-        if (a.verts) {
-          unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
-          unsigned long long plane = a.n * a.cap;
-          a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
-        }
-        L.slot++; L.stage0 = L.slot;
-      } else {
-        if (a.verts) {
-          float* s = rec_stage() + (L.slot & (REC_GROUP - 1)) * REC_THREADS;
-          s[0] = L.px; s[REC_GROUP * REC_THREADS] = L.py; s[2 * REC_GROUP * REC_THREADS] = L.pz;
-        }
-        L.slot++;
-        if ((L.slot & (REC_GROUP - 1)) == 0u) flush_vertices(a, L);
+      if (a.verts) {
+        unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
+        unsigned long long plane = a.n * a.cap;
+        a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
       }
+      L.slot++; L.stage0 = L.slot;
     }
   }
 }
