@@ -172,7 +172,12 @@ __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s,
     const float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
     const float nx = __fmaf_rn(a.h6, sx, L.px), ny = __fmaf_rn(a.h6, sy, L.py), nz = __fmaf_rn(a.h6, sz, L.pz);
     float gx, gy, gz;
-    const bool in5 = to_index<UNIT>(a.g, nx, ny, nz, gx, gy, gz);
+    index_pos<UNIT>(a.g, nx, ny, nz, gx, gy, gz);
+    // A5.5 with the integer accept of sample_nb (fast = 0 unless the field is tame): floor(g) inside
+    // the cell range decides; the faces g = N-1, the outside and +-inf take the float test.
+    bool in5 = ((unsigned)__float2int_rd(gx) < s.fastx) & ((unsigned)__float2int_rd(gy) < s.fasty) &
+               ((unsigned)__float2int_rd(gz) < s.fastz);
+    if (__builtin_expect(!in5, 0)) in5 = in_domain(a.g, gx, gy, gz);
     const bool stag = m < a.vmin2;
     if ((r1 | r2 | r3 | r4) != 0u || stag || !in5) {                            // rare: the particle ends
       if (r1) { done = 1; return r1; }
