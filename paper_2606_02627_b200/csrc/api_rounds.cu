@@ -70,7 +70,7 @@ int streami_streak_begin(streami_field f, const float* points, size_t m, unsigne
   STREAMI_TRY(cudaMallocAsync((void**)&state, (size_t)m * nsteps, st));
   streami_streak_s* h = new streami_streak_s();
   StreakArgs& a = h->a;
-  a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
+  a.g = f->g; a.g.time_mode = params->time_mode; a.s = launch_store(f);
   a.points = points; a.m = m; a.nsteps = nsteps;
   a.h = params->h; a.h2 = 0.5f * params->h; a.h6 = params->h / 6.0f;
   a.vmin2 = params->vmin * params->vmin; a.t0 = params->t0;

@@ -137,10 +137,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   }
 
   TraceArgs a{};
-  a.g = f->g; a.g.time_mode = params->time_mode; a.s = f->store;
-  if (f->tame && options().integer_accept) {
-    a.s.fastx = (unsigned)(a.s.cmx + 1); a.s.fasty = (unsigned)(a.s.cmy + 1); a.s.fastz = (unsigned)(a.s.cmz + 1);
-  }
+  a.g = f->g; a.g.time_mode = params->time_mode; a.s = launch_store(f);
   a.bricks = nullptr; a.nbricks = 0;
   a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr; a.next = next; a.round = 0;
   a.seg_budget = K;

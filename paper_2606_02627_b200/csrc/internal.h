@@ -48,6 +48,16 @@ inline int check(cudaError_t e) {
 
 int num_sms();
 
+// The monolithic store as a launch sees it: with the integer-accept ranges of sample_nb (field.cuh)
+// filled in when the field is tame and option "integer_accept" is on.
+inline Store launch_store(const streami_field_s* f) {
+  Store s = f->store;
+  if (f->tame && options().integer_accept) {
+    s.fastx = (unsigned)(s.cmx + 1); s.fasty = (unsigned)(s.cmy + 1); s.fastz = (unsigned)(s.cmz + 1);
+  }
+  return s;
+}
+
 // Optional device timing of the advection kernel alone (option "kernel_timing"): a pair of CUDA
 // events recorded on the launching stream around each advection launch, summed by
 // streami_kernel_time().  Off by default; bench.py's roofline leg turns it on.
