@@ -249,8 +249,12 @@ int streami_streak_lines(streami_streak s, unsigned long long* out_offsets, floa
  * out_offsets [n+1] u64 and out_points [max_points][3]; only the stored vertices cross the bus, not
  * the capacity-padded slot array.  params->capacity/stride select the vertices as usual; the
  * optional outputs in params are host pointers.  *out_total (host, may be NULL) = points of all
- * lines.  Synchronises cuda_stream (twice: the total sizes the device buffer).  Returns
- * STREAMI_E_TRUNCATED if total > max_points (the first max_points points are then delivered). */
+ * lines.  Large inputs run in up to 4 batches of seeds (option "host_batch"): the points of one batch
+ * are copied out on a second, library-owned stream while the next batch is traced; pinned host
+ * buffers are what lets that overlap happen, pageable ones work but serialise.  Synchronises
+ * cuda_stream (once per batch: the batch's total sizes its device buffer) and returns with all copies
+ * complete.  Returns STREAMI_E_TRUNCATED if total > max_points (the first max_points points are then
+ * delivered). */
 int streami_trace_streamlines_lines_host(streami_field f, const float* seeds, size_t n,
                                          const streami_params* params, unsigned long long* out_offsets,
                                          float* out_points, unsigned long long max_points,
@@ -283,6 +287,7 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
  *   "max_blocks_per_sm" B     limit resident blocks per SM (0 = as many as fit)
  *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0)
  *   "streak_window"     W     streaklines: global steps per launch (0 = automatic)
+ *   "host_batch"        S     streami_trace_streamlines_lines_host: seeds per batch (0 = automatic)
  *   "kernel_timing"     0/1   record a CUDA event pair around every advection-kernel launch
  * Returns INVALID for unknown names. */
 int streami_set_option(const char* name, int value);

@@ -67,6 +67,16 @@ static __global__ void add_bases_kernel(unsigned long long* __restrict__ offsets
   if (i < n) offsets[i] += tile_base[i / SCAN_TILE];
 }
 
+// batches of the host polyline call: out[i] = local[i] + base (i < count), totals += part
+static __global__ void rebase_offsets_kernel(const unsigned long long* __restrict__ local, unsigned long long base,
+                                             unsigned long long* __restrict__ out, unsigned long long count) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < count) out[i] = local[i] + base;
+}
+static __global__ void accumulate_totals_kernel(unsigned long long* __restrict__ dst, const unsigned long long* __restrict__ part) {
+  if (threadIdx.x < 4) dst[threadIdx.x] += part[threadIdx.x];
+}
+
 // streamlines: point (line id, slot k) -> out_points[offsets[id] + k]; consecutive threads read
 // consecutive slots of one particle (coalesced in each SoA plane).
 static __global__ void gather_streamlines_kernel(const float* __restrict__ verts, const unsigned* __restrict__ counts,

@@ -149,3 +149,51 @@ def test_streamlines_lines_host_on_bricks(S, torch, oracle, wl):
     assert not trunc and total == int(roff[-1])
     assert np.array_equal(off.numpy().astype(np.uint64), roff)
     assert np.array_equal(pts.numpy()[:total].view(np.uint32), rp.view(np.uint32))      # P9: bricks == monolithic
+
+
+@pytest.mark.parametrize("bricked", [False, True])
+@pytest.mark.parametrize("batch", [700, 1000, 5000])
+def test_streamlines_lines_host_in_batches(S, torch, oracle, wl, bricked, batch):
+    """`host_batch` splits the seeds into batches whose polylines are copied out while the next batch
+    is traced; offsets, points, every optional per-particle output, the totals and the truncation
+    rule must not depend on the split (3001 seeds in batches of 700 / 1000 / one batch)."""
+    from oracle import lines
+    N = 24
+    fld = wl.turb_field_cpu(N, 32, 1, 5)
+    n = 3001
+    seeds = wl.seeds_uniform(23, n, [N - 1.0] * 3)
+    seeds[5] = [N + 2.0, 1, 1]                                           # an empty line
+    kw = dict(integrator=0, h=0.25, max_steps=90, vmin=1e-6, capacity=16, stride=4)
+    ref = oracle.streamlines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), seeds, oracle.params(**kw), "f32")
+    roff, rp = lines.streamline_lines(ref.vertices, ref.counts)
+    if bricked:
+        nbk = (2, 1, 2)
+        f = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nbk, 1,
+                                           [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nbk, 1)])
+    else:
+        f = gpu_field(S, torch, fld)
+    h_seeds = torch.from_numpy(seeds.copy()).pin_memory()
+    off = torch.zeros(n + 1, dtype=torch.int64).pin_memory()
+    pts = torch.full((n * 16, 3), float("nan"), dtype=torch.float32).pin_memory()
+    h_status = torch.zeros(n, dtype=torch.int32); h_steps = torch.zeros(n, dtype=torch.int32)
+    h_final = torch.zeros((3, n), dtype=torch.float32); h_totals = torch.zeros(4, dtype=torch.int64)
+    prm = S.params(**kw)
+    prm.out_status = h_status.data_ptr(); prm.out_steps = h_steps.data_ptr()
+    prm.out_final = h_final.data_ptr(); prm.out_totals = h_totals.data_ptr()
+    try:
+        S.streami_set_option("host_batch", batch)
+        total, trunc = S.streami_trace_streamlines_lines_host(f, h_seeds, prm, off, pts)
+        small = torch.zeros((1234, 3), dtype=torch.float32)
+        total2, trunc2 = S.streami_trace_streamlines_lines_host(f, h_seeds, S.params(**kw), off.clone(), small)
+    finally:
+        S.streami_set_option("host_batch", 0)
+    assert not trunc and total == int(roff[-1])
+    assert np.array_equal(off.numpy().astype(np.uint64), roff)
+    assert np.array_equal(pts.numpy()[:total].view(np.uint32), rp.view(np.uint32))
+    assert np.isnan(pts.numpy()[total:]).all()
+    assert np.array_equal(h_status.numpy().astype(np.uint32), ref.status)
+    assert np.array_equal(h_steps.numpy().astype(np.uint32), ref.steps)
+    assert np.array_equal(h_final.numpy().view(np.uint32), ref.final.view(np.uint32))
+    assert np.array_equal(h_totals.numpy()[:3].astype(np.uint64), ref.totals[:3])
+    assert trunc2 and total2 == total
+    assert np.array_equal(small.numpy().view(np.uint32), rp[:1234].view(np.uint32))
