@@ -180,7 +180,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
  * experiment (a structured grid re-expressed as hexahedra).  Formula sheet U1-U4:
  * cell c has corners H[c][l], l = dx + 2 dy + 4 dz, at reference coordinates (dx, dy, dz); a point
  * is located through a uniform bin grid nb over the box lo..hi as the first (lowest-numbered) cell
- * listed in its bin whose inverse isoparametric map (6 Newton steps from the centre) converges to
+ * listed in its bin whose inverse isoparametric map (Newton from the centre, at most 6 steps) converges to
  * reference coordinates inside the unit cube (+- 2e-5); the value is the trilinear combination of
  * the corner values at those coordinates.
  * _create_hex: X [nv][3], V [nv][3], H [nc][8] are HOST arrays (consumed: the handle owns a device

@@ -16,13 +16,15 @@
 //     outside.  Hexahedron c is listed, in ascending c, in every bin between the bins of the
 //     componentwise min and max of its 8 vertices (both clamped into the box).
 //  U3 inverse map.  G(xi) = tri(X, xi) - p with tri = 3 nested lerps (x, then y, then z) per
-//     component.  Start xi = (1/2,1/2,1/2); NEWTON = 6 times: J columns
+//     component.  Start xi = (1/2,1/2,1/2); at most NEWTON = 6 times, stopping after the first
+//     update with |d_a| <= TOL for all a (the usual Newton termination; the paper does not specify
+//     the inverse map, it calls a library point query): J columns
 //       J_x = lerp(lerp(X1-X0, X3-X2, xi_y), lerp(X5-X4, X7-X6, xi_y), xi_z),
 //       J_y = lerp(lerp(X2-X0, X3-X1, xi_x), lerp(X6-X4, X7-X5, xi_x), xi_z),
 //       J_z = lerp(lerp(X4-X0, X5-X1, xi_x), lerp(X6-X2, X7-X3, xi_x), xi_y);
 //     cofactors c_ij with fma(a, b, -(c*d)); det = fma(J_x.z, c_xz, fma(J_x.y, c_xy, J_x.x * c_xx));
 //     r = 1/det; d_a = r * fma(G.z, ., fma(G.y, ., G.x * .)) (adjugate row a); xi = xi - d.
-//     p is in c iff the last update has |d_a| <= TOL (the iteration converged: a far cell's iterate may
+//     p is in c iff the last update has |d_a| <= TOL (the iteration stopped by convergence: a far cell's iterate may
 //     otherwise pass through the unit cube) and -TOL <= xi_a <= 1 + TOL for all a (TOL = 2e-5 in fp32,
 //     1e-11 in fp64: it only has to
 //     exceed the error of the inverse map so that no point falls between two cells; NaN -> no).
@@ -127,6 +129,8 @@ template <class T> bool hx_invert(const HexMesh<T>& m, size_t c, const T* p, T* 
     d[1] = r * std::fma(G[2], cyz, std::fma(G[1], cyy, G[0] * cyx));
     d[2] = r * std::fma(G[2], czz, std::fma(G[1], czy, G[0] * czx));
     xi[0] = xi[0] - d[0]; xi[1] = xi[1] - d[1]; xi[2] = xi[2] - d[2];
+    const T tt = HexMesh<T>::tol();
+    if (std::fabs(d[0]) <= tt && std::fabs(d[1]) <= tt && std::fabs(d[2]) <= tt) break;   // converged
   }
   const T t = HexMesh<T>::tol();
   const bool converged = std::fabs(d[0]) <= t && std::fabs(d[1]) <= t && std::fabs(d[2]) <= t;

@@ -17,7 +17,7 @@
 namespace streami {
 
 constexpr int MESH_REC = 56;            // floats per cell record
-constexpr int MESH_NEWTON = 6;          // U3
+constexpr int MESH_NEWTON = 6;          // U3: at most this many Newton steps
 constexpr float MESH_TOL = 2e-5f;       // U3
 
 struct MeshDev {
@@ -65,6 +65,7 @@ __device__ __forceinline__ bool hx_invert(const float* __restrict__ P, float px,
     dy = r * __fmaf_rn(G[2], cyz, __fmaf_rn(G[1], cyy, G[0] * cyx));
     dz = r * __fmaf_rn(G[2], czz, __fmaf_rn(G[1], czy, G[0] * czx));
     x = x - dx; y = y - dy; z = z - dz;
+    if (fabsf(dx) <= MESH_TOL && fabsf(dy) <= MESH_TOL && fabsf(dz) <= MESH_TOL) break;   // U3: converged
   }
   const float t = MESH_TOL;
   const bool converged = fabsf(dx) <= t && fabsf(dy) <= t && fabsf(dz) <= t;
@@ -75,30 +76,62 @@ __device__ __forceinline__ bool hx_invert(const float* __restrict__ P, float px,
 // The bounding-box pre-test only skips cells that cannot pass U3 (a converged xi inside the unit
 // cube +- TOL maps into the box +- TOL x its extent, and `margin` is 50 times that), so the located
 // cell is the same with and without it.
-__device__ __forceinline__ long long hx_locate(const MeshDev& m, float px, float py, float pz, float& x,
-                                               float& y, float& z) {
+__device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, float py, float pz, float& x,
+                                                    float& y, float& z) {
   if (!((px >= m.lox && px <= m.hix) && (py >= m.loy && py <= m.hiy) && (pz >= m.loz && pz <= m.hiz))) return -1;
   const int bx = min(__float2int_rd((px - m.lox) * m.sx), m.nbx - 1);
   const int by = min(__float2int_rd((py - m.loy) * m.sy), m.nby - 1);
   const int bz = min(__float2int_rd((pz - m.loz) * m.sz), m.nbz - 1);
   const unsigned id = ((unsigned)bz * m.nby + by) * m.nbx + bx;
-  const unsigned k1 = m.bin_start[id + 1];
-  for (unsigned k = m.bin_start[id]; k < k1; ++k) {
-    const unsigned c = m.bin_items[k];
-    const float* rec = m.cells + (size_t)c * MESH_REC;
-    const float g = m.margin;
-    if (px < rec[48] - g || px > rec[51] + g || py < rec[49] - g || py > rec[52] + g || pz < rec[50] - g ||
-        pz > rec[53] + g)
-      continue;
-    float P[24];
+  const unsigned k0 = m.bin_start[id], k1 = m.bin_start[id + 1];
+  const float g = m.margin;
+  // The list is walked in order, four candidates at a time: their ids, then their boxes, are
+  // fetched with independent loads (one memory round trip each instead of one per candidate: the
+  // walk is a chain of dependent L2 reads and the kernel is bound by their latency), the boxes are
+  // tested, and the survivors -- normally one -- go through U3 in list order.
+  for (unsigned kb = k0; kb < k1; kb += 4u) {
+    unsigned cand[4];
 #pragma unroll
-    for (int i = 0; i < 24; i += 4) {
-      const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
-      P[i] = q.x; P[i + 1] = q.y; P[i + 2] = q.z; P[i + 3] = q.w;
+    for (int j = 0; j < 4; ++j) cand[j] = kb + j < k1 ? __ldg(m.bin_items + kb + j) : 0xffffffffu;
+    float4 lo4[4], hi4[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const float* rec = m.cells + (size_t)(cand[j] == 0xffffffffu ? 0u : cand[j]) * MESH_REC;
+      lo4[j] = __ldg(reinterpret_cast<const float4*>(rec + 48));      // min.xyz, max.x
+      hi4[j] = __ldg(reinterpret_cast<const float4*>(rec + 52));      // max.yz, pad
     }
-    if (hx_invert(P, px, py, pz, x, y, z)) return (long long)c;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (cand[j] == 0xffffffffu) continue;
+      if (px < lo4[j].x - g || px > lo4[j].w + g || py < lo4[j].y - g || py > hi4[j].x + g || pz < lo4[j].z - g ||
+          pz > hi4[j].y + g)
+        continue;
+      const float* rec = m.cells + (size_t)cand[j] * MESH_REC;
+      float P[24];
+#pragma unroll
+      for (int i = 0; i < 24; i += 4) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
+        P[i] = q.x; P[i + 1] = q.y; P[i + 2] = q.z; P[i + 3] = q.w;
+      }
+      if (hx_invert(P, px, py, pz, x, y, z)) return (long long)cand[j];
+    }
   }
   return -1;
+}
+
+// One out-of-line copy serves the five call sites of the advection kernel (the inlined copies made
+// it spill at 128 registers); the result comes back in registers.
+struct HxHit { long long c; float x, y, z; };
+static __device__ __noinline__ HxHit hx_locate_call(const MeshDev& m, float px, float py, float pz) {
+  HxHit r; r.x = 0.f; r.y = 0.f; r.z = 0.f;
+  r.c = hx_locate_body(m, px, py, pz, r.x, r.y, r.z);
+  return r;
+}
+__device__ __forceinline__ long long hx_locate(const MeshDev& m, float px, float py, float pz, float& x,
+                                               float& y, float& z) {
+  const HxHit r = hx_locate_call(m, px, py, pz);
+  x = r.x; y = r.y; z = r.z;
+  return r.c;
 }
 
 // U4: value at reference coordinates xi of cell c.
@@ -120,7 +153,7 @@ static __global__ void mesh_sample_kernel(const MeshDev m, const float* __restri
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float x, y, z, vx = 0.f, vy = 0.f, vz = 0.f;
-  const long long c = hx_locate(m, pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], x, y, z);
+  const long long c = hx_locate_body(m, pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], x, y, z);
   if (c >= 0) hx_value(m, c, x, y, z, vx, vy, vz);
   out_v[3 * i] = vx; out_v[3 * i + 1] = vy; out_v[3 * i + 2] = vz;
   if (out_cell) out_cell[i] = c;
@@ -141,7 +174,7 @@ struct MeshTraceArgs {
 // Persistent grid, one lane per particle; a lane whose particle has ended takes the next work item
 // from a global counter, so that all lanes of a warp take one RK4 step per iteration.  The cell
 // and xi located for p_new are reused for the next step's k1 (the same point: the same result).
-static __global__ void __launch_bounds__(128) mesh_trace_kernel(const MeshTraceArgs a) {
+static __global__ void __launch_bounds__(128) mesh_trace_kernel(const __grid_constant__ MeshTraceArgs a) {
   __shared__ unsigned long long s_tot[3];
   if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
   __syncthreads();
