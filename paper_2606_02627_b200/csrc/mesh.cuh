@@ -76,8 +76,9 @@ __device__ __forceinline__ bool hx_invert(const float* __restrict__ P, float px,
 // The bounding-box pre-test only skips cells that cannot pass U3 (a converged xi inside the unit
 // cube +- TOL maps into the box +- TOL x its extent, and `margin` is 50 times that), so the located
 // cell is the same with and without it.
+template <bool VALUE>
 __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, float py, float pz, float& x,
-                                                    float& y, float& z) {
+                                                    float& y, float& z, float* v) {
   if (!((px >= m.lox && px <= m.hix) && (py >= m.loy && py <= m.hiy) && (pz >= m.loz && pz <= m.hiz))) return -1;
   const int bx = min(__float2int_rd((px - m.lox) * m.sx), m.nbx - 1);
   const int by = min(__float2int_rd((py - m.loy) * m.sy), m.nby - 1);
@@ -113,25 +114,32 @@ __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, 
         const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
         P[i] = q.x; P[i + 1] = q.y; P[i + 2] = q.z; P[i + 3] = q.w;
       }
-      if (hx_invert(P, px, py, pz, x, y, z)) return (long long)cand[j];
+      float Q[24];
+      if (VALUE) {             // U4's operands, requested together with U3's (one round trip, not two)
+#pragma unroll
+        for (int i = 0; i < 24; i += 4) {
+          const float4 q = __ldg(reinterpret_cast<const float4*>(rec + 24 + i));
+          Q[i] = q.x; Q[i + 1] = q.y; Q[i + 2] = q.z; Q[i + 3] = q.w;
+        }
+      }
+      if (hx_invert(P, px, py, pz, x, y, z)) {
+        if (VALUE) { v[0] = hx_tri(Q, x, y, z); v[1] = hx_tri(Q + 8, x, y, z); v[2] = hx_tri(Q + 16, x, y, z); }
+        return (long long)cand[j];
+      }
     }
   }
   return -1;
 }
 
-// One out-of-line copy serves the five call sites of the advection kernel (the inlined copies made
-// it spill at 128 registers); the result comes back in registers.
-struct HxHit { long long c; float x, y, z; };
-static __device__ __noinline__ HxHit hx_locate_call(const MeshDev& m, float px, float py, float pz) {
-  HxHit r; r.x = 0.f; r.y = 0.f; r.z = 0.f;
-  r.c = hx_locate_body(m, px, py, pz, r.x, r.y, r.z);
+// S(p) on a mesh: located cell (or -1) and value.  One out-of-line copy serves the five call sites
+// of the advection kernel (the inlined copies made it spill at 128 registers); the result comes back
+// in registers.
+struct HxSample { long long c; float vx, vy, vz; };
+static __device__ __noinline__ HxSample hx_sample_call(const MeshDev& m, float px, float py, float pz) {
+  HxSample r; float x, y, z, v[3] = {0.f, 0.f, 0.f};
+  r.c = hx_locate_body<true>(m, px, py, pz, x, y, z, v);
+  r.vx = v[0]; r.vy = v[1]; r.vz = v[2];
   return r;
-}
-__device__ __forceinline__ long long hx_locate(const MeshDev& m, float px, float py, float pz, float& x,
-                                               float& y, float& z) {
-  const HxHit r = hx_locate_call(m, px, py, pz);
-  x = r.x; y = r.y; z = r.z;
-  return r.c;
 }
 
 // U4: value at reference coordinates xi of cell c.
@@ -153,7 +161,7 @@ static __global__ void mesh_sample_kernel(const MeshDev m, const float* __restri
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float x, y, z, vx = 0.f, vy = 0.f, vz = 0.f;
-  const long long c = hx_locate_body(m, pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], x, y, z);
+  const long long c = hx_locate_body<false>(m, pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], x, y, z, nullptr);
   if (c >= 0) hx_value(m, c, x, y, z, vx, vy, vz);
   out_v[3 * i] = vx; out_v[3 * i + 1] = vy; out_v[3 * i + 2] = vz;
   if (out_cell) out_cell[i] = c;
@@ -172,16 +180,15 @@ struct MeshTraceArgs {
 
 // RK4 streamlines on a mesh (A4-A6 with S := the mesh sample, "inside" := a cell is located).
 // Persistent grid, one lane per particle; a lane whose particle has ended takes the next work item
-// from a global counter, so that all lanes of a warp take one RK4 step per iteration.  The cell
-// and xi located for p_new are reused for the next step's k1 (the same point: the same result).
+// from a global counter, so that all lanes of a warp take one RK4 step per iteration.  The sample
+// taken at p_new for the exit test (A5.5) is the next step's k1 (the same point: the same result).
 static __global__ void __launch_bounds__(128) mesh_trace_kernel(const __grid_constant__ MeshTraceArgs a) {
   __shared__ unsigned long long s_tot[3];
   if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
   __syncthreads();
   const unsigned long long plane = a.n * a.cap;
   unsigned long long id = 0;
-  float px = 0.f, py = 0.f, pz = 0.f, x = 0.f, y = 0.f, z = 0.f;
-  long long c = -1;
+  float px = 0.f, py = 0.f, pz = 0.f, k1x = 0.f, k1y = 0.f, k1z = 0.f;
   unsigned n = 0, slot = 0, samples = 0, attempts = 0;
   bool active = false, exhausted = false;
   auto record = [&](unsigned k) {
@@ -208,8 +215,9 @@ static __global__ void __launch_bounds__(128) mesh_trace_kernel(const __grid_con
         id = a.perm ? a.perm[w] : w;
         px = a.seeds[3 * id]; py = a.seeds[3 * id + 1]; pz = a.seeds[3 * id + 2];
         n = 0; slot = 0; samples = 0; attempts = 0; active = true;
-        c = hx_locate(a.m, px, py, pz, x, y, z);
-        if (c < 0) finish(ST_OUT);                                              // A5.1
+        const HxSample s0 = hx_sample_call(a.m, px, py, pz);
+        k1x = s0.vx; k1y = s0.vy; k1z = s0.vz;
+        if (s0.c < 0) finish(ST_OUT);                                           // A5.1
         else record(0u);
       }
     }
@@ -221,30 +229,26 @@ static __global__ void __launch_bounds__(128) mesh_trace_kernel(const __grid_con
       unsigned st = ST_ALIVE;
       do {
         if (n == a.max_steps) { st = ST_MAXSTEPS; break; }                      // A5.2
-        float k1x, k1y, k1z, k2x, k2y, k2z, k3x, k3y, k3z, k4x, k4y, k4z, qx, qy, qz;
-        hx_value(a.m, c, x, y, z, k1x, k1y, k1z); samples++;                    // A5.3
-        const float mm = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));
+        samples++;                                                              // k1 = S(p), carried
+        const float mm = __fmaf_rn(k1z, k1z, __fmaf_rn(k1y, k1y, k1x * k1x));   // A5.3
         if (mm < a.vmin2) { st = ST_STAGNANT; break; }
         attempts++;
-        qx = __fmaf_rn(a.h2, k1x, px); qy = __fmaf_rn(a.h2, k1y, py); qz = __fmaf_rn(a.h2, k1z, pz);
-        long long cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-        if (cq < 0) { st = ST_OUT; break; }
-        hx_value(a.m, cq, x, y, z, k2x, k2y, k2z);
-        qx = __fmaf_rn(a.h2, k2x, px); qy = __fmaf_rn(a.h2, k2y, py); qz = __fmaf_rn(a.h2, k2z, pz);
-        cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-        if (cq < 0) { st = ST_OUT; break; }
-        hx_value(a.m, cq, x, y, z, k3x, k3y, k3z);
-        qx = __fmaf_rn(a.h, k3x, px); qy = __fmaf_rn(a.h, k3y, py); qz = __fmaf_rn(a.h, k3z, pz);
-        cq = hx_locate(a.m, qx, qy, qz, x, y, z); samples++;
-        if (cq < 0) { st = ST_OUT; break; }
-        hx_value(a.m, cq, x, y, z, k4x, k4y, k4z);
-        const float sx = (k1x + k4x) + 2.0f * (k2x + k3x);
-        const float sy = (k1y + k4y) + 2.0f * (k2y + k3y);
-        const float sz = (k1z + k4z) + 2.0f * (k2z + k3z);
+        float qx = __fmaf_rn(a.h2, k1x, px), qy = __fmaf_rn(a.h2, k1y, py), qz = __fmaf_rn(a.h2, k1z, pz);
+        const HxSample s2 = hx_sample_call(a.m, qx, qy, qz); samples++;
+        if (s2.c < 0) { st = ST_OUT; break; }
+        qx = __fmaf_rn(a.h2, s2.vx, px); qy = __fmaf_rn(a.h2, s2.vy, py); qz = __fmaf_rn(a.h2, s2.vz, pz);
+        const HxSample s3 = hx_sample_call(a.m, qx, qy, qz); samples++;
+        if (s3.c < 0) { st = ST_OUT; break; }
+        qx = __fmaf_rn(a.h, s3.vx, px); qy = __fmaf_rn(a.h, s3.vy, py); qz = __fmaf_rn(a.h, s3.vz, pz);
+        const HxSample s4 = hx_sample_call(a.m, qx, qy, qz); samples++;
+        if (s4.c < 0) { st = ST_OUT; break; }
+        const float sx = (k1x + s4.vx) + 2.0f * (s2.vx + s3.vx);
+        const float sy = (k1y + s4.vy) + 2.0f * (s2.vy + s3.vy);
+        const float sz = (k1z + s4.vz) + 2.0f * (s2.vz + s3.vz);
         const float nx = __fmaf_rn(a.h6, sx, px), ny = __fmaf_rn(a.h6, sy, py), nz = __fmaf_rn(a.h6, sz, pz);
-        cq = hx_locate(a.m, nx, ny, nz, x, y, z);                               // A5.5
-        if (cq < 0) { st = ST_OUT; break; }
-        px = nx; py = ny; pz = nz; c = cq; n++;                                 // A5.6
+        const HxSample s5 = hx_sample_call(a.m, nx, ny, nz);                    // A5.5
+        if (s5.c < 0) { st = ST_OUT; break; }
+        px = nx; py = ny; pz = nz; k1x = s5.vx; k1y = s5.vy; k1z = s5.vz; n++;  // A5.6
         record(n);
       } while (false);
       if (st != ST_ALIVE) finish(st);
