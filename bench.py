@@ -265,7 +265,7 @@ class Job:
                           counts=pin(self.counts), steps=pin(self.steps_o), status=pin(self.status_o),
                           final=None if self.final_o is None else pin(self.final_o),
                           totals=t.zeros(4, dtype=t.int64).pin_memory())
-            if self.kind not in ("gyre", "mesh"):
+            if self.kind != "gyre":
                 # polyline buffers instead of the capacity-padded slot array
                 self.h["verts"] = None; self.h["counts"] = None
                 self.h["offsets"] = t.zeros(self.n + 1, dtype=t.int64).pin_memory()
@@ -285,7 +285,7 @@ class Job:
         nb = lambda x: 0 if x is None else x.numel() * x.element_size()
         bi = nb(h["seeds"])
         bo = sum(nb(h[k]) for k in ("verts", "counts", "steps", "status", "final", "totals"))
-        if self.kind not in ("gyre", "mesh"):          # offsets + the points actually delivered
+        if self.kind != "gyre":                        # offsets + the points actually delivered
             bo += nb(h["offsets"]) + 12 * int(self.e2e_points)
         return bi, bo
 
@@ -294,14 +294,8 @@ class Job:
         trace, D2H of every output, stream sync -- all inside the library."""
         h, S = self._pinned(), self.S
         if self.kind == "mesh":
-            # no host-buffer entry point for meshes yet: the same copies are issued here around the
-            # device call (pinned host -> device, device -> pinned host, stream sync)
-            self.seeds.copy_(h["seeds"], non_blocking=True)
-            self.step_device()
-            for k, d in (("verts", self.verts), ("counts", self.counts), ("steps", self.steps_o),
-                         ("status", self.status_o), ("final", self.final_o), ("totals", self.totals_o)):
-                h[k].copy_(d, non_blocking=True)
-            self.torch.cuda.current_stream().synchronize()
+            self.e2e_points, _ = S.streami_mesh_trace_streamlines_lines_host(self.field, h["seeds"], self.prm_h,
+                                                                             h["offsets"], h["points"])
         elif self.kind == "gyre":
             S.streami_trace_streaklines_host(self.field, h["seeds"], self.nsteps, self.prm_h, h["verts"], h["counts"])
         else:

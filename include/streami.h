@@ -197,6 +197,12 @@ int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* ou
                         void* cuda_stream);
 int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n, const streami_params* params,
                                    float* out_vertices, unsigned* out_counts, void* cuda_stream);
+/* As streami_trace_streamlines_lines_host (HOST seeds in, HOST polylines out, batched and overlapped
+ * in the same way), on a mesh. */
+int streami_mesh_trace_streamlines_lines_host(streami_mesh m, const float* seeds, size_t n,
+                                              const streami_params* params, unsigned long long* out_offsets,
+                                              float* out_points, unsigned long long max_points,
+                                              unsigned long long* out_total, void* cuda_stream);
 
 /* Seed generation on a control shape (the paper's convenience kernels: "uniformly distributed seed
  * points given simple control shapes such as planes or lines").  The shape is

@@ -62,6 +62,7 @@ def lib():
         L.streami_mesh_destroy.argtypes = [P]
         L.streami_mesh_sample.argtypes = [P, P, Z, P, P, P]
         L.streami_mesh_trace_streamlines.argtypes = [P, P, Z, P, P, P, P]
+        L.streami_mesh_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
         L.streami_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
         L.streami_streak_step.argtypes = [P, U, P]
         L.streami_streak_position.argtypes = [P, P]
@@ -283,19 +284,28 @@ def streami_seed_shape(origin, edge_u, edge_v=(0, 0, 0), edge_w=(0, 0, 0), nu=1,
     return out
 
 
-def streami_trace_streamlines_lines_host(field, seeds, prm_host, out_offsets, out_points, stream=None):
-    """Host seeds in, host polylines out (offsets int64 [n+1], points float32 [max_points, 3]).
-    Returns (total_points, truncated)."""
+def _lines_host(fn, handle, seeds, prm_host, out_offsets, out_points, stream):
     for t, nm in ((seeds, "seeds"), (out_offsets, "out_offsets"), (out_points, "out_points")):
         if t is not None and (t.is_cuda or not t.is_contiguous()):
             raise ValueError("%s: contiguous CPU tensor expected" % nm)
     total = ctypes.c_ulonglong(0)
-    rc = _check(lib().streami_trace_streamlines_lines_host(field.handle, _ptr(seeds), seeds.shape[0],
-                                                           ctypes.byref(prm_host), _ptr(out_offsets),
-                                                           _ptr(out_points), out_points.shape[0],
-                                                           ctypes.byref(total), _stream(stream)),
+    rc = _check(fn(handle, _ptr(seeds), seeds.shape[0], ctypes.byref(prm_host), _ptr(out_offsets),
+                   _ptr(out_points), out_points.shape[0], ctypes.byref(total), _stream(stream)),
                 allow=(E_TRUNCATED,))
     return total.value, rc == E_TRUNCATED
+
+
+def streami_trace_streamlines_lines_host(field, seeds, prm_host, out_offsets, out_points, stream=None):
+    """Host seeds in, host polylines out (offsets int64 [n+1], points float32 [max_points, 3]).
+    Returns (total_points, truncated)."""
+    return _lines_host(lib().streami_trace_streamlines_lines_host, field.handle, seeds, prm_host, out_offsets,
+                       out_points, stream)
+
+
+def streami_mesh_trace_streamlines_lines_host(mesh, seeds, prm_host, out_offsets, out_points, stream=None):
+    """The same on a hexahedral mesh."""
+    return _lines_host(lib().streami_mesh_trace_streamlines_lines_host, mesh.handle, seeds, prm_host, out_offsets,
+                       out_points, stream)
 
 
 def streami_probe_gather(span_bytes, piece_bytes, iters=2000, stream=None):

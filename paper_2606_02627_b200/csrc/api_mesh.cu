@@ -4,6 +4,7 @@
 #include <cmath>
 #include <vector>
 
+#include "host_lines.cuh"
 #include "internal.h"
 #include "mesh.cuh"
 #include "sorter.cuh"
@@ -73,27 +74,46 @@ int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V
   for (size_t c = 0; c < nc; ++c) for_bins(c, [&](size_t b) { start[b + 1]++; total++; });
   if (total > 0xffffffffull) return STREAMI_E_INVALID;
   for (size_t b = 0; b < nbins; ++b) start[b + 1] += start[b];
-  std::vector<unsigned> items(std::max<size_t>(total, 1)), fill(start.begin(), start.end() - 1);
-  for (size_t c = 0; c < nc; ++c) for_bins(c, [&](size_t b) { items[fill[b]++] = (unsigned)c; });
+  // list entries: cell id + the cell's box in the coordinates of the bin (MESH_BOX_SCALE in mesh.cuh)
+  const float margin = 50.0f * MESH_TOL * extent;
+  std::vector<uint4> items(std::max<size_t>(total, 1));
+  std::vector<unsigned> fill(start.begin(), start.end() - 1);
+  auto pack = [](double u_lo, double u_hi, unsigned& lo16, unsigned& hi16) {
+    const double a = std::floor((u_lo - MESH_BOX_SLACK) * (double)MESH_BOX_SCALE);
+    const double b = std::ceil((u_hi + MESH_BOX_SLACK) * (double)MESH_BOX_SCALE);
+    lo16 = (unsigned)(unsigned short)(short)std::min(std::max(a, -32768.0), 32767.0);
+    hi16 = (unsigned)(unsigned short)(short)std::min(std::max(b, -32768.0), 32767.0);
+  };
+  for (size_t c = 0; c < nc; ++c) {
+    const float* rec = cells.data() + c * MESH_REC;
+    for_bins(c, [&](size_t b) {
+      const int bi[3] = {(int)(b % nb[0]), (int)((b / nb[0]) % nb[1]), (int)(b / ((size_t)nb[0] * nb[1]))};
+      unsigned l16[3], h16[3];
+      for (int a = 0; a < 3; ++a)
+        pack(((double)rec[48 + a] - margin - lo[a]) * s[a] - bi[a], ((double)rec[51 + a] + margin - lo[a]) * s[a] - bi[a],
+             l16[a], h16[a]);
+      items[fill[b]++] = make_uint4((unsigned)c, l16[0] | (l16[1] << 16), l16[2] | (h16[0] << 16), h16[1] | (h16[2] << 16));
+    });
+  }
 
   streami_mesh_s* m = new streami_mesh_s();
   m->nc = nc; m->dev_cells = m->dev_start = m->dev_items = nullptr;
   cudaError_t e = cudaMalloc(&m->dev_cells, cells.size() * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&m->dev_start, start.size() * sizeof(unsigned));
-  if (e == cudaSuccess) e = cudaMalloc(&m->dev_items, items.size() * sizeof(unsigned));
+  if (e == cudaSuccess) e = cudaMalloc(&m->dev_items, items.size() * sizeof(uint4));
   if (e == cudaSuccess) e = cudaMemcpy(m->dev_cells, cells.data(), cells.size() * sizeof(float), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(m->dev_start, start.data(), start.size() * sizeof(unsigned), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(m->dev_items, items.data(), items.size() * sizeof(unsigned), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(m->dev_items, items.data(), items.size() * sizeof(uint4), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
     cudaFree(m->dev_cells); cudaFree(m->dev_start); cudaFree(m->dev_items);
     delete m;
     return check(e);
   }
   MeshDev& d = m->d;
-  d.cells = (const float*)m->dev_cells; d.bin_start = (const unsigned*)m->dev_start; d.bin_items = (const unsigned*)m->dev_items;
+  d.cells = (const float*)m->dev_cells; d.bin_start = (const unsigned*)m->dev_start; d.bin_items = (const uint4*)m->dev_items;
   d.lox = lo[0]; d.loy = lo[1]; d.loz = lo[2]; d.hix = hi[0]; d.hiy = hi[1]; d.hiz = hi[2];
   d.sx = s[0]; d.sy = s[1]; d.sz = s[2]; d.nbx = nb[0]; d.nby = nb[1]; d.nbz = nb[2];
-  d.margin = 50.0f * MESH_TOL * extent;
+  d.margin = margin;
   *out = m;
   return STREAMI_OK;
 }
@@ -162,6 +182,17 @@ int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n,
   if (perm) cudaFreeAsync(perm, st);
   if (have_sorter) sorter.release();
   return check(e);
+}
+
+int streami_mesh_trace_streamlines_lines_host(streami_mesh m, const float* seeds, size_t n,
+                                              const streami_params* params, unsigned long long* out_offsets,
+                                              float* out_points, unsigned long long max_points,
+                                              unsigned long long* out_total, void* cuda_stream) {
+  if (!m) return STREAMI_E_INVALID;
+  auto trace = [&](const float* d_seeds, size_t nb, const streami_params* dp, float* d_v, unsigned* d_c) {
+    return streami_mesh_trace_streamlines(m, d_seeds, nb, dp, d_v, d_c, cuda_stream);
+  };
+  return lines_host(trace, false, seeds, n, params, out_offsets, out_points, max_points, out_total, cuda_stream);
 }
 
 }  // extern "C"

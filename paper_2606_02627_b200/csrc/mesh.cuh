@@ -19,14 +19,25 @@ namespace streami {
 constexpr int MESH_REC = 56;            // floats per cell record
 constexpr int MESH_NEWTON = 6;          // U3: at most this many Newton steps
 constexpr float MESH_TOL = 2e-5f;       // U3
+// A list entry carries, next to the cell id, the cell's bounding box (grown by `margin` and a slack
+// of MESH_BOX_SLACK bin widths, rounded outwards) in the coordinates of ITS bin, 1/256 bin width per
+// unit, six int16: one 16-byte load per candidate decides whether the cell record is worth
+// fetching.  The box only filters (any superset of the cells that can pass U3 gives the same
+// located cell), so its own rounding does not matter as long as it errs outwards; the slack covers
+// the fp32 rounding of the point's bin coordinate (<= 2 nb 2^-24 bin widths).
+constexpr float MESH_BOX_SCALE = 256.0f;
+#ifndef MESH_WALK
+#define MESH_WALK 4                      // list entries fetched per round trip
+#endif
+constexpr double MESH_BOX_SLACK = 1.0 / 1024.0;
 
 struct MeshDev {
   const float* cells;                   // [nc][MESH_REC]
   const unsigned* bin_start;            // [nbins + 1]
-  const unsigned* bin_items;
+  const uint4* bin_items;               // {cell id, packed box}: see MESH_BOX_SCALE
   float lox, loy, loz, hix, hiy, hiz, sx, sy, sz;
   int nbx, nby, nbz;
-  float margin;                         // bounding-box pre-test margin (build's choice, see hx_locate)
+  float margin;                         // what the packed boxes were grown by (build's choice, see hx_locate)
 };
 
 __device__ __forceinline__ float hx_tri(const float* Q, float x, float y, float z) {
@@ -73,9 +84,9 @@ __device__ __forceinline__ bool hx_invert(const float* __restrict__ P, float px,
 }
 
 // U2 + U3.  Returns the located cell or -1; xi is valid when a cell is returned.
-// The bounding-box pre-test only skips cells that cannot pass U3 (a converged xi inside the unit
-// cube +- TOL maps into the box +- TOL x its extent, and `margin` is 50 times that), so the located
-// cell is the same with and without it.
+// The box pre-test only skips cells that cannot pass U3 (a converged xi inside the unit cube +- TOL
+// maps into the bounding box +- TOL x its extent; the packed boxes are grown by `margin` = 50 times
+// that, plus their own slack), so the located cell is the same with and without it.
 template <bool VALUE>
 __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, float py, float pz, float& x,
                                                     float& y, float& z, float* v) {
@@ -85,29 +96,26 @@ __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, 
   const int bz = min(__float2int_rd((pz - m.loz) * m.sz), m.nbz - 1);
   const unsigned id = ((unsigned)bz * m.nby + by) * m.nbx + bx;
   const unsigned k0 = m.bin_start[id], k1 = m.bin_start[id + 1];
-  const float g = m.margin;
-  // The list is walked in order, four candidates at a time: their ids, then their boxes, are
-  // fetched with independent loads (one memory round trip each instead of one per candidate: the
-  // walk is a chain of dependent L2 reads and the kernel is bound by their latency), the boxes are
-  // tested, and the survivors -- normally one -- go through U3 in list order.
-  for (unsigned kb = k0; kb < k1; kb += 4u) {
-    unsigned cand[4];
+  // the point in the coordinates of its bin, in box units (t - b is exact: both lie in [b, b+1])
+  const float ux = ((px - m.lox) * m.sx - (float)bx) * MESH_BOX_SCALE;
+  const float uy = ((py - m.loy) * m.sy - (float)by) * MESH_BOX_SCALE;
+  const float uz = ((pz - m.loz) * m.sz - (float)bz) * MESH_BOX_SCALE;
+  // The list is walked in order, MESH_WALK candidates at a time: the entries are fetched with independent
+  // loads (the walk is a chain of dependent L2 reads and the kernel is bound by their latency), the
+  // boxes are tested, and the survivors -- normally one -- go through U3 in list order.
+  for (unsigned kb = k0; kb < k1; kb += (unsigned)MESH_WALK) {
+    uint4 ent[MESH_WALK];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) cand[j] = kb + j < k1 ? __ldg(m.bin_items + kb + j) : 0xffffffffu;
-    float4 lo4[4], hi4[4];
+    for (int j = 0; j < MESH_WALK; ++j) ent[j] = kb + j < k1 ? __ldg(m.bin_items + kb + j) : make_uint4(0xffffffffu, 0u, 0u, 0u);
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const float* rec = m.cells + (size_t)(cand[j] == 0xffffffffu ? 0u : cand[j]) * MESH_REC;
-      lo4[j] = __ldg(reinterpret_cast<const float4*>(rec + 48));      // min.xyz, max.x
-      hi4[j] = __ldg(reinterpret_cast<const float4*>(rec + 52));      // max.yz, pad
-    }
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      if (cand[j] == 0xffffffffu) continue;
-      if (px < lo4[j].x - g || px > lo4[j].w + g || py < lo4[j].y - g || py > hi4[j].x + g || pz < lo4[j].z - g ||
-          pz > hi4[j].y + g)
-        continue;
-      const float* rec = m.cells + (size_t)cand[j] * MESH_REC;
+    for (int j = 0; j < MESH_WALK; ++j) {
+      const unsigned cand = ent[j].x;
+      if (cand == 0xffffffffu) continue;
+      const float lx = (float)(short)(ent[j].y & 0xffffu), ly = (float)(short)(ent[j].y >> 16);
+      const float lz = (float)(short)(ent[j].z & 0xffffu), hx = (float)(short)(ent[j].z >> 16);
+      const float hy = (float)(short)(ent[j].w & 0xffffu), hz = (float)(short)(ent[j].w >> 16);
+      if (ux < lx || ux > hx || uy < ly || uy > hy || uz < lz || uz > hz) continue;
+      const float* rec = m.cells + (size_t)cand * MESH_REC;
       float P[24];
 #pragma unroll
       for (int i = 0; i < 24; i += 4) {
@@ -124,7 +132,7 @@ __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, 
       }
       if (hx_invert(P, px, py, pz, x, y, z)) {
         if (VALUE) { v[0] = hx_tri(Q, x, y, z); v[1] = hx_tri(Q + 8, x, y, z); v[2] = hx_tri(Q + 16, x, y, z); }
-        return (long long)cand[j];
+        return (long long)cand;
       }
     }
   }
