@@ -51,7 +51,10 @@ int lines_host(Trace&& trace, bool one_batch, const float* seeds, size_t n, cons
   // most 4 batches of at least 262,144 seeds.  Results do not depend on the split (ids are local to
   // a batch only inside the library).
   size_t per = (size_t)options().host_batch;
-  if (per == 0) per = one_batch ? n : std::max<size_t>((n + 3) / 4, 262144);
+  // Points cost 12 B per `stride` steps on a ~50 GB/s bus against ~2e-11 s per RK4 step: only a dense
+  // recording (C2, stride 8: the copy takes 1.5x the trace) has a copy worth hiding; with a sparse one
+  // (C5, stride 128: 3 %) the extra kernel tails of the batches are all that is left (998 -> 1,077 ms).
+  if (per == 0) per = (one_batch || params->stride > 32u) ? n : std::max<size_t>((n + 3) / 4, 262144);
   per = std::min(per, n);
   const size_t nbatch = (n + per - 1) / per;
   static cudaStream_t copy_st = nullptr;

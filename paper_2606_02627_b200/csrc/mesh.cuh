@@ -40,6 +40,12 @@ struct MeshDev {
   float margin;                         // what the packed boxes were grown by (build's choice, see hx_locate)
 };
 
+__device__ __forceinline__ void ldg256(const float* p, float* o) {   // p 32-byte aligned
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(o[6]), "=f"(o[7])
+               : "l"(p));
+}
+
 __device__ __forceinline__ float hx_tri(const float* Q, float x, float y, float z) {
   const float c00 = lerp(Q[0], Q[1], x), c01 = lerp(Q[2], Q[3], x);
   const float c10 = lerp(Q[4], Q[5], x), c11 = lerp(Q[6], Q[7], x);
@@ -116,19 +122,13 @@ __device__ __forceinline__ long long hx_locate_body(const MeshDev& m, float px, 
       const float hy = (float)(short)(ent[j].w & 0xffffu), hz = (float)(short)(ent[j].w >> 16);
       if (ux < lx || ux > hx || uy < ly || uy > hy || uz < lz || uz > hz) continue;
       const float* rec = m.cells + (size_t)cand * MESH_REC;
-      float P[24];
+      float P[24];             // records are 224 = 7 x 32 bytes: one 256-bit load per sector
 #pragma unroll
-      for (int i = 0; i < 24; i += 4) {
-        const float4 q = __ldg(reinterpret_cast<const float4*>(rec + i));
-        P[i] = q.x; P[i + 1] = q.y; P[i + 2] = q.z; P[i + 3] = q.w;
-      }
+      for (int i = 0; i < 24; i += 8) ldg256(rec + i, P + i);
       float Q[24];
       if (VALUE) {             // U4's operands, requested together with U3's (one round trip, not two)
 #pragma unroll
-        for (int i = 0; i < 24; i += 4) {
-          const float4 q = __ldg(reinterpret_cast<const float4*>(rec + 24 + i));
-          Q[i] = q.x; Q[i + 1] = q.y; Q[i + 2] = q.z; Q[i + 3] = q.w;
-        }
+        for (int i = 0; i < 24; i += 8) ldg256(rec + 24 + i, Q + i);
       }
       if (hx_invert(P, px, py, pz, x, y, z)) {
         if (VALUE) { v[0] = hx_tri(Q, x, y, z); v[1] = hx_tri(Q + 8, x, y, z); v[2] = hx_tri(Q + 16, x, y, z); }
