@@ -33,6 +33,15 @@ int num_sms() {
   return n;
 }
 
+cudaStream_t copy_stream() {
+  static cudaStream_t s = [] {
+    cudaStream_t c = nullptr;
+    if (cudaStreamCreateWithFlags(&c, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c = nullptr; }
+    return c;
+  }();
+  return s;
+}
+
 static std::mutex g_time_mutex;
 static std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_time_pairs;   // recorded, not yet read
 static std::vector<cudaEvent_t> g_time_free;

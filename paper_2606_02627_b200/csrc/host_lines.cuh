@@ -57,9 +57,8 @@ int lines_host(Trace&& trace, bool one_batch, const float* seeds, size_t n, cons
   if (per == 0) per = (one_batch || params->stride > 32u) ? n : std::max<size_t>((n + 3) / 4, 262144);
   per = std::min(per, n);
   const size_t nbatch = (n + per - 1) / per;
-  static cudaStream_t copy_st = nullptr;
-  if (nbatch > 1 && !copy_st) STREAMI_TRY(cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking));
-  cudaStream_t cs = nbatch > 1 ? copy_st : st;
+  cudaStream_t cs = st;
+  if (nbatch > 1) { cs = copy_stream(); if (!cs) return STREAMI_E_CUDA; }
 
   int rc = STREAMI_OK;
   unsigned long long total = 0;

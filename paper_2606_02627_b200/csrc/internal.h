@@ -47,6 +47,7 @@ inline int check(cudaError_t e) {
   } while (0)
 
 int num_sms();
+cudaStream_t copy_stream();      // the library's own non-blocking stream for overlapped D2H copies (created once)
 
 // The monolithic store as a launch sees it: with the integer-accept ranges of sample_nb (field.cuh)
 // filled in when the field is tame and option "integer_accept" is on.
