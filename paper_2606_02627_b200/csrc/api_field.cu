@@ -162,6 +162,21 @@ static int auto_layout(unsigned long long nvert, int nslices) {
   return LAYOUT_XPAIR;
 }
 
+// Tame scan of n packed floats (sample_nb in field.cuh says what it licenses).
+static int scan_tame(const float* dev_ptr, unsigned long long n, bool* tame) {
+  unsigned* flag = nullptr; unsigned bad = 1u;
+  cudaError_t e = cudaMalloc((void**)&flag, sizeof(unsigned));
+  if (e == cudaSuccess) e = cudaMemset(flag, 0, sizeof(unsigned));
+  if (e == cudaSuccess) {
+    tame_scan_kernel<<<148 * 8, 256>>>(dev_ptr, n, flag);
+    launch_counter()++;
+    e = cudaMemcpy(&bad, flag, sizeof(unsigned), cudaMemcpyDeviceToHost);
+  }
+  cudaFree(flag);
+  *tame = bad == 0u;
+  return check(e);
+}
+
 static int pick_layout(int hint) {
   if (hint == STREAMI_LAYOUT_AUTO) return 0;              // decided per stored array (auto_layout)
   if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR ||
@@ -194,7 +209,7 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.hix = dims[0] - 1; s.hiy = dims[1] - 1; s.hiz = dims[2] - 1;
   s.topflagx = s.topflagy = s.topflagz = 1;
   s.cmx = s.hix - 1; s.cmy = s.hiy - 1; s.cmz = s.hiz - 1;
-  s.fastx = s.fasty = s.fastz = 0u;
+  s.fastx = s.fasty = s.fastz = 0u; s.self = nullptr;
   s.nx = (unsigned)dims[0]; s.nxy = (unsigned)dims[0] * (unsigned)dims[1];
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
@@ -212,18 +227,9 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   f->layout = layout;
   if (rc) { delete f; return rc; }
   f->tame = false;
-  if (nslices == 1) {                 // only the steady RK4 path asks (sample_nb)
-    unsigned* flag = nullptr; unsigned bad = 1u;
-    cudaError_t e = cudaMalloc((void**)&flag, sizeof(unsigned));
-    if (e == cudaSuccess) e = cudaMemset(flag, 0, sizeof(unsigned));
-    if (e == cudaSuccess) {
-      tame_scan_kernel<<<148 * 8, 256>>>(dev_ptr, 3ull * s.slice_stride, flag);
-      launch_counter()++;
-      e = cudaMemcpy(&bad, flag, sizeof(unsigned), cudaMemcpyDeviceToHost);
-    }
-    cudaFree(flag);
-    if (e != cudaSuccess) { if (bytes) cudaFree(data); delete f; return check(e); }
-    f->tame = bad == 0u;
+  if (nslices == 1) {                 // only the steady paths ask
+    rc = scan_tame(dev_ptr, 3ull * s.slice_stride, &f->tame);
+    if (rc) { if (bytes) cudaFree(data); delete f; return rc; }
   }
   if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
   s.data = data;
@@ -253,7 +259,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
   int rc = fill_geom(f->g, global_dims, origin, spacing, 1, 1.0f);
   if (rc) { delete f; return rc; }
   for (int a = 0; a < 3; ++a) f->dims[a] = global_dims[a];
-  f->layout = layout; f->bricked = true; f->d_bricks = nullptr; f->owned_bytes = 0;
+  f->layout = layout; f->bricked = true; f->d_bricks = nullptr; f->owned_bytes = 0; f->tame = true;
   BrickMap& m = f->bm;
   m.nbx = brick_grid[0]; m.nby = brick_grid[1]; m.nbz = brick_grid[2];
   m.Bx = global_dims[0] / m.nbx; m.By = global_dims[1] / m.nby; m.Bz = global_dims[2] / m.nbz;
@@ -294,7 +300,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
           }
           s.olox = ol[0]; s.oloy = ol[1]; s.oloz = ol[2]; s.ohix = oh[0]; s.ohiy = oh[1]; s.ohiz = oh[2];
         }
-        s.fastx = s.fasty = s.fastz = 0u;
+        s.fastx = s.fasty = s.fastz = 0u; s.self = nullptr;
         s.nx = (unsigned)(hi[0] - lo[0] + 1);
         s.nxy = s.nx * (unsigned)(hi[1] - lo[1] + 1);
         s.slice_stride = (unsigned long long)s.nxy * (unsigned)(hi[2] - lo[2] + 1);
@@ -306,11 +312,20 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
         if (layout == LAYOUT_CELL) cell_strides(s, bnx, bny, bnz);
         s.data = data;
         if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
+        bool brick_tame = false;
+        rc = scan_tame(src, 3ull * bnx * bny * bnz, &brick_tame);
+        if (rc) return fail(rc);
+        f->tame = f->tame && brick_tame;
         f->bricks.push_back(s);
       }
   void* tbl = nullptr;
   if (check(cudaMalloc(&tbl, sizeof(Store) * nb)) != STREAMI_OK) return fail(STREAMI_E_NOMEM);
   f->owned.push_back(tbl);
+  for (int i = 0; i < nb; ++i) {
+    Store& s = f->bricks[i];
+    s.self = (const Store*)tbl + i;
+    if (f->tame) { s.fastx = (unsigned)(s.hix - s.lox); s.fasty = (unsigned)(s.hiy - s.loy); s.fastz = (unsigned)(s.hiz - s.loz); }
+  }
   cudaError_t e = cudaMemcpy(tbl, f->bricks.data(), sizeof(Store) * nb, cudaMemcpyHostToDevice);
   if (e != cudaSuccess) return fail(check(e));
   f->d_bricks = (Store*)tbl;

@@ -235,6 +235,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
   a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = nb;
+  a.brick_fast = options().integer_accept;
   a.seeds = seeds; a.perm = nullptr; a.next = d_next; a.nwork_dev = nullptr;
   // the paper re-queues EVERY particle after every RK step (Listing 1 ends in
   // emitOutgoing; one forward per step).  brick_round_steps = 1

@@ -42,6 +42,10 @@ struct Store {
   // Monolithic steady stores: cells per axis if every stored value is tame (finite, |v| <= 2^60),
   // else 0.  See sample_nb: floor(g) < fast on all axes then decides "inside" with integers.
   unsigned fastx, fasty, fastz;
+  // Bricks: device address of this descriptor in the brick table.  The advection kernel keeps a copy
+  // of the descriptor in registers; the fields only the rare float tests need are read through
+  // `self` when wanted instead of staying live (the brick kernel is short of registers).
+  const Store* self;
   unsigned long long slice_stride;   // records per slice
 };
 
@@ -275,9 +279,24 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
                                            float& vz) {
   float gx, gy, gz;
   index_pos<UNIT>(g, px, py, pz, gx, gy, gz);
-  if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
   unsigned long long v; float fx, fy, fz;
-  if (!locate<BRICK>(s, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
+  if constexpr (BRICK && !UNSTEADY) {
+    // Integer accept (see sample_nb), brick form: lo <= floor(g) < hi on every axis <=> the brick
+    // serves g (A9) and g is inside the domain; no clamp is needed there.  fast = hi - lo if every
+    // brick is tame, else 0; the faces g = N-1, misses, the outside and +-inf take the float tests.
+    const int jx = __float2int_rd(gx), jy = __float2int_rd(gy), jz = __float2int_rd(gz);
+    const int lx = jx - s.lox, ly = jy - s.loy, lz = jz - s.loz;
+    if (((unsigned)lx < s.fastx) & ((unsigned)ly < s.fasty) & ((unsigned)lz < s.fastz)) {
+      fx = gx - (float)jx; fy = gy - (float)jy; fz = gz - (float)jz;
+      v = (unsigned long long)((unsigned)lz * s.nxy + (unsigned)ly * s.nx + (unsigned)lx);
+    } else {
+      if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
+      if (!locate<BRICK>(*s.self, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
+    }
+  } else {
+    if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
+    if (!locate<BRICK>(s, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
+  }
   if (UNSTEADY) {
     float a; bool two;
     int j = time_slice(g, t, a, two);
@@ -394,10 +413,10 @@ __device__ __forceinline__ void prefetch_cell32(const Store& s, unsigned v, unsi
 template <bool BRICK>
 __device__ __forceinline__ unsigned clamped_cell(const Store& s, float gx, float gy, float gz) {
   int ix, iy, iz;
-  if (BRICK) {
-    ix = max(min(__float2int_rz(gx), s.cmx), s.lox) - s.lox;
-    iy = max(min(__float2int_rz(gy), s.cmy), s.loy) - s.loy;
-    iz = max(min(__float2int_rz(gz), s.cmz), s.loz) - s.loz;
+  if (BRICK) {      // from lo and the integer-accept range only (fast = 0: every prediction maps to cell 0)
+    ix = max(min(__float2int_rz(gx) - s.lox, (int)s.fastx - 1), 0);
+    iy = max(min(__float2int_rz(gy) - s.loy, (int)s.fasty - 1), 0);
+    iz = max(min(__float2int_rz(gz) - s.loz, (int)s.fastz - 1), 0);
   } else {
     ix = max(min(__float2int_rz(gx), s.cmx), 0);
     iy = max(min(__float2int_rz(gy), s.cmy), 0);

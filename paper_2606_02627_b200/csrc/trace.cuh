@@ -42,6 +42,7 @@ struct TraceArgs {
   int vec_ok;                      // capacity % 8 == 0 and verts 32-byte aligned: full-sector vertex stores
   int prefetch;                    // 1 = one-step-ahead cell prefetch (field.cuh), 0 = off
   int staging;                     // 1 = stage vertices in shared memory (default), 0 = store each directly
+  int brick_fast;                  // 0 = clear the bricks' integer-accept ranges (option "integer_accept" = 0)
   unsigned* counts; unsigned* steps; unsigned* status; float* fin;
   unsigned long long* totals;      // [4]
   // brick outputs

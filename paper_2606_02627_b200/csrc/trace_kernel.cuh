@@ -124,7 +124,10 @@ trace_kernel(const TraceArgs a) {
             }
           }
           if (active) {
-            if (BRICK) { st = a.bricks[my_brick]; }
+            if (BRICK) {
+              st = a.bricks[my_brick];
+              if (!a.brick_fast) { st.fastx = 0u; st.fasty = 0u; st.fastz = 0u; }
+            }
             cc.invalidate();
             if (INTEG == 1) {
               // k1 of the first attempt.  For a continued particle this recomputes the FSAL value

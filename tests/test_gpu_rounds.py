@@ -302,3 +302,51 @@ def test_bricks_dp5(S, torch, oracle, wl, layout, budget):
     for key in ("status", "steps", "counts"):
         assert np.array_equal(out[key][ok], mono[key][ok]), key
     assert np.array_equal(out["final"].view(np.uint32)[:, ok], mono["final"].view(np.uint32)[:, ok])
+
+
+@pytest.mark.parametrize("kind", ["tame", "nan", "inf"])
+@pytest.mark.parametrize("integ", [0, 1])
+def test_bricks_integer_accept_and_untamed_fields(S, torch, oracle, wl, kind, integ):
+    """The brick kernels decide "served and inside" from floor(g) when every brick holds finite
+    values and fall back to the float tests (descriptor read through its table entry) otherwise:
+    fields with planted NaN / inf, the option on and off, thin ghosts (HALO_MISS), seeds on the
+    domain faces -- RK4 and DP5(4), all against the oracle bit for bit."""
+    import dataclasses
+    N, nb = 28, (2, 2, 2)
+    base = wl.turb_field_cpu(N, 32, 1, 5)
+    data = base.data.copy()
+    idx = np.random.default_rng(6).integers(0, N, size=(150, 3))
+    if kind == "nan":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.nan
+    elif kind == "inf":
+        data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.where(idx[:, 1] % 2, np.inf, -np.inf)
+    fld = dataclasses.replace(base, data=data)
+    n = 8000
+    seeds = wl.seeds_uniform(31, n, [N - 1.0] * 3)
+    seeds[:300] = np.round(seeds[:300]); seeds[300:500, 0] = N - 1.0; seeds[500:700, 2] = 0.0
+    seeds[700:850] = idx + 0.5
+    if integ == 0:
+        kw = dict(integrator=0, h=1.5, max_steps=12, vmin=1e-6, capacity=20, stride=1)      # long steps: halo misses
+    else:
+        kw = dict(integrator=1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-4, rtol=1e-4, max_steps=120, vmin=1e-6,
+                  capacity=20, stride=8)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    for on in (1, 0):
+        try:
+            S.streami_set_option("integer_accept", on)
+            out = gpu_bricks(S, torch, wl, fld, nb, seeds, **kw)
+        finally:
+            S.streami_set_option("integer_accept", 1)
+        for key in ("status", "steps", "counts"):
+            assert np.array_equal(out[key], getattr(ref, key)), (key, on)
+        assert np.array_equal(out["final"].view(np.uint32), ref.final.view(np.uint32)), on
+        assert np.array_equal(out["vertices"].view(np.uint32), ref.vertices.view(np.uint32)), on
+        assert np.array_equal(out["totals"], ref.totals), on
+        assert out["nrounds"] == ref.nrounds and np.array_equal(out["log"], ref.log)
+    hist = np.bincount(ref.status, minlength=5)
+    assert hist[1] > 50
+    if integ == 0:
+        assert hist[2] > 50 and hist[4] > 0, "the case must contain MAX_STEPS and HALO_MISS"
