@@ -293,6 +293,16 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
       if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
       if (!locate<BRICK>(*s.self, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;
     }
+  } else if constexpr (!BRICK && !UNSTEADY && !KNOWN) {
+    // the same accept for a monolithic steady store (DP5(4) stages; RK4 goes through sample_nb)
+    const int jx = __float2int_rd(gx), jy = __float2int_rd(gy), jz = __float2int_rd(gz);
+    if (((unsigned)jx < s.fastx) & ((unsigned)jy < s.fasty) & ((unsigned)jz < s.fastz)) {
+      fx = gx - (float)jx; fy = gy - (float)jy; fz = gz - (float)jz;
+      v = (unsigned long long)((unsigned)jz * s.nxy + (unsigned)jy * s.nx + (unsigned)jx);
+    } else {
+      if (!in_domain(g, gx, gy, gz)) return ST_OUT;
+      locate<false>(s, gx, gy, gz, v, fx, fy, fz);
+    }
   } else {
     if (!KNOWN) { if (!in_domain(g, gx, gy, gz)) return ST_OUT; }
     if (!locate<BRICK>(s, gx, gy, gz, v, fx, fy, fz)) return ST_HALO;

@@ -128,9 +128,11 @@ def test_integer_accept_keeps_the_domain_test_exact(S, torch, oracle, wl, turb48
     g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing)
     f = gpu_field(S, torch, fld, layout)
     for kw in (dict(integrator=0, h=0.25, max_steps=80, vmin=1e-6, capacity=16, stride=5),
-               dict(integrator=0, h=1e30, max_steps=3, vmin=0.0, capacity=4, stride=1)):
+               dict(integrator=0, h=1e30, max_steps=3, vmin=0.0, capacity=4, stride=1),
+               dict(integrator=1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-4, rtol=1e-4, max_steps=60, vmin=1e-6,
+                    capacity=16, stride=5)):
         ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
-        assert kw["h"] > 1.0 or len(set(ref.status.tolist())) >= 2
+        assert kw["h"] > 1.0 or len(set(ref.status.tolist())) >= 2       # (RK4, RK4 with stage points at +-inf, DP5(4))
         for on in (1, 0):
             try:
                 S.streami_set_option("integer_accept", on)
