@@ -20,13 +20,18 @@ int check_params(const streami_params* p, bool need_capacity);
 void fill_integrator(TraceArgs& a, const streami_params* p);
 
 typedef void (*StreakKernel)(const StreakArgs);
-static StreakKernel pick_streak(int layout, bool unsteady) {
+template <int LAYOUT>
+static StreakKernel pick_streak_l(bool unsteady, bool tcache) {
+  if (!unsteady) return streak_kernel<LAYOUT, false, false>;
+  return tcache ? streak_kernel<LAYOUT, true, true> : streak_kernel<LAYOUT, true, false>;
+}
+static StreakKernel pick_streak(int layout, bool unsteady, bool tcache) {
   switch (layout) {
-    case LAYOUT_PACKED3: return unsteady ? streak_kernel<LAYOUT_PACKED3, true> : streak_kernel<LAYOUT_PACKED3, false>;
-    case LAYOUT_FLOAT4: return unsteady ? streak_kernel<LAYOUT_FLOAT4, true> : streak_kernel<LAYOUT_FLOAT4, false>;
-    case LAYOUT_CELL: return unsteady ? streak_kernel<LAYOUT_CELL, true> : streak_kernel<LAYOUT_CELL, false>;
-    case LAYOUT_XYQUAD: return unsteady ? streak_kernel<LAYOUT_XYQUAD, true> : streak_kernel<LAYOUT_XYQUAD, false>;
-    default: return unsteady ? streak_kernel<LAYOUT_XPAIR, true> : streak_kernel<LAYOUT_XPAIR, false>;
+    case LAYOUT_PACKED3: return pick_streak_l<LAYOUT_PACKED3>(unsteady, tcache);
+    case LAYOUT_FLOAT4: return pick_streak_l<LAYOUT_FLOAT4>(unsteady, tcache);
+    case LAYOUT_CELL: return pick_streak_l<LAYOUT_CELL>(unsteady, tcache);
+    case LAYOUT_XYQUAD: return pick_streak_l<LAYOUT_XYQUAD>(unsteady, tcache);
+    default: return pick_streak_l<LAYOUT_XPAIR>(unsteady, tcache);
   }
 }
 }  // namespace streami
@@ -76,7 +81,7 @@ int streami_streak_begin(streami_field f, const float* points, size_t m, unsigne
   a.h = params->h; a.h2 = 0.5f * params->h; a.h6 = params->h / 6.0f;
   a.vmin2 = params->vmin * params->vmin; a.t0 = params->t0;
   a.verts = out_vertices; a.state = state; a.steps = params->out_steps; a.totals = params->out_totals;
-  h->k = pick_streak(f->layout, unsteady);
+  h->k = pick_streak(f->layout, unsteady, options().cell_cache != 0);
   h->done = 0; h->window = K; h->out_status = params->out_status;
   *out = h;
   return STREAMI_OK;

@@ -220,6 +220,19 @@ struct CellCache {
   __device__ __forceinline__ void invalidate() { key = 0xffffffffu; }   // never a low corner
 };
 
+// The same for an unsteady field read with linear interpolation in time (A3): the cell in slice j
+// and in slice j+1, keyed by the record index in slice j (which fixes j as well).  Stages 2 and 3 of
+// an RK4 step share their time and almost always their cell, and so do stage 4 and stage 1 of the
+// next step (t_n + h and t_{n+1} fall in the same slice interval, the points differ by O(h^2)): about
+// half of the two-slice gathers of a streakline step are repeats.
+struct CellCacheT {
+  unsigned long long key;
+  float V[48];
+  __device__ __forceinline__ void invalidate() { key = ~0ull; }
+};
+template <class CC> struct IsTimeCache { static constexpr bool value = false; };
+template <> struct IsTimeCache<CellCacheT> { static constexpr bool value = true; };
+
 // A2.1 + A2.2: index-space position and the closed-box test (NaN -> false).
 // UNIT = the grid is its own index space (origin 0, spacing 1, hence r = 1): (p - 0.0f) * 1.0f
 // returns p bit for bit, so the two operations are skipped.  C2, C3 and C5 are such grids.
@@ -273,8 +286,8 @@ __device__ __forceinline__ int time_slice(const Geom& g, float t, float& a, bool
 // Full sample S(p, t) (A2/A3, brick form A9).  Returns 0 ok, ST_OUT or ST_HALO.
 // KNOWN: the caller has already established that p is inside the domain (it passed the A5.5 test
 // at the end of the previous step, or the A5.1 test at the seed), so the test is not repeated.
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT = false, bool KNOWN = false>
-__device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCache& cc, float px,
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT = false, bool KNOWN = false, class CC = CellCache>
+__device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CC& cc, float px,
                                            float py, float pz, float t, float& vx, float& vy,
                                            float& vz) {
   float gx, gy, gz;
@@ -311,6 +324,20 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
     float a; bool two;
     int j = time_slice(g, t, a, two);
     unsigned long long vj = v + (unsigned long long)j * s.slice_stride;
+    if constexpr (CACHE && IsTimeCache<CC>::value) {
+      if (two) {
+        if (vj != cc.key) {
+          load_cell<LAYOUT>(s, vj, cc.V);
+          load_cell<LAYOUT>(s, vj + s.slice_stride, cc.V + 24);
+          cc.key = vj;
+        }
+        float ux, uy, uz, wx, wy, wz;
+        interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, ux, uy, uz);
+        interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V + 24, fx, fy, fz, wx, wy, wz);
+        vx = lerp(ux, wx, a); vy = lerp(uy, wy, a); vz = lerp(uz, wz, a);   // space first, time last
+        return 0;
+      }
+    }
     float V[24];
     load_cell<LAYOUT>(s, vj, V);
     float ux, uy, uz;
@@ -321,7 +348,7 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CellCa
       interp_cell<LayoutTraits<LAYOUT>::DIFF>(V, fx, fy, fz, wx, wy, wz);
       vx = lerp(ux, wx, a); vy = lerp(uy, wy, a); vz = lerp(uz, wz, a);   // space first, time last
     } else { vx = ux; vy = uy; vz = uz; }
-  } else if (CACHE) {
+  } else if constexpr (CACHE && !IsTimeCache<CC>::value) {
     const unsigned v32 = (unsigned)v;
     if (v32 != cc.key) { load_cell32<LAYOUT>(s, v32, cc.V); cc.key = v32; }
     interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, vx, vy, vz);

@@ -135,6 +135,9 @@ __global__ void sample_kernel(Geom g, Store s, const float* __restrict__ pts, un
 // One launch covers the global steps [s0, s1).  Particle id = j*m + i (release j, point i) is
 // born at point i at global step j.  Its state between launches is its output slot (the last
 // inside position is what the slot must hold anyway) plus one status byte.
+template <bool T> struct StreakCache { typedef CellCache type; };
+template <> struct StreakCache<true> { typedef CellCacheT type; };
+
 struct StreakArgs {
   Geom g; Store s;
   const float* points; unsigned long long m; unsigned nsteps, s0, s1;
@@ -145,7 +148,9 @@ struct StreakArgs {
   unsigned long long* totals;
 };
 
-template <int LAYOUT, bool UNSTEADY>
+// TCACHE (option "cell_cache", unsteady fields read linearly in time): the two-slice cell copy of
+// field.cuh stays in registers across the stages and steps of a window.
+template <int LAYOUT, bool UNSTEADY, bool TCACHE>
 __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
   __shared__ unsigned long long s_tot[3];
   if (threadIdx.x < 3) s_tot[threadIdx.x] = 0ull;
@@ -173,14 +178,14 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
       ta.g = a.g; ta.h = a.h; ta.h2 = a.h2; ta.h6 = a.h6; ta.vmin2 = a.vmin2;
       ta.max_steps = 0xffffffffu; ta.verts = nullptr; ta.cap = 0; ta.stride = 0xffffffffu;
       Lane L; L.px = px; L.py = py; L.pz = pz; L.id = 0; L.slot = 0; L.rec_cd = 0xffffffffu;
-      CellCache cc; cc.invalidate();
+      typename StreakCache<UNSTEADY && TCACHE>::type cc; cc.invalidate();
       unsigned n_samples = 0, n_attempts = 0;
       const unsigned s_first = s;
       for (; s < a.s1; ++s) {
         L.n = s;                                                 // t_s = t0 + (float)s*h, shared by all
         ta.t0 = a.t0;
         unsigned done;
-        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, false, false, false>(ta, a.s, cc, L, done);
+        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, UNSTEADY && TCACHE, false, false>(ta, a.s, cc, L, done);
         if (rc) { st = rc; n_attempts = done >= 2u ? 1u : 0u; n_samples = min(done, 4u); break; }
       }
       n_attempts += s - s_first; n_samples += 4u * (s - s_first);

@@ -149,8 +149,8 @@ __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
 // `done` samples and is an attempt iff done >= 2 or the new position left the domain (A5.3
 // comes before the attempt is counted).  The stage-1 sample does not repeat the domain test:
 // p passed it at the end of the previous step (A5.5) or at the seed (A5.1).
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool REC = true>
-__device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CellCache& cc,
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool REC = true, class CC = CellCache>
+__device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CC& cc,
                                              Lane& L, unsigned& done) {
   done = 0;
   if (L.n == a.max_steps) return ST_MAXSTEPS;                                   // A5.2

@@ -39,10 +39,12 @@ def gpu_streaklines(S, torch, field, pts, nsteps, **kw):
             totals.cpu().numpy().astype(np.uint64))
 
 
-@pytest.mark.parametrize("layout", [1, 2, 3, 4])
+@pytest.mark.parametrize("cache", [1, 0])
+@pytest.mark.parametrize("layout", [1, 2, 3, 4, 5])
 @pytest.mark.parametrize("window", [0, 1, 7])
-def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window):
-    """A scaled-down config 4: double gyre slices, rake + a few points that leave or start outside."""
+def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window, cache):
+    """A scaled-down config 4: double gyre slices, rake + a few points that leave or start outside.
+    cache = the two-slice register copy of the current cell (option "cell_cache"), on and off."""
     fld = wl.double_gyre_field(dims=(64, 32, 16), nslices=10, dt=0.25)
     pts = wl.rake_c4(16, 8)
     pts = np.concatenate([pts, np.array([[2.5, 0.5, 0.5], [1.999, 0.5, 0.999], [0.001, 0.999, 0.001]],
@@ -52,11 +54,13 @@ def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window):
     g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
     ref = oracle.streaklines(g, pts, nsteps, oracle.params(**kw), "f32")
     S.streami_set_option("streak_window", window)
+    S.streami_set_option("cell_cache", cache)
     try:
         v, counts, steps, status, totals = gpu_streaklines(S, torch, gpu_field(S, torch, fld, layout),
                                                            pts, nsteps, **kw)
     finally:
         S.streami_set_option("streak_window", 0)
+        S.streami_set_option("cell_cache", 1)
     assert np.array_equal(status, ref.status) and np.array_equal(steps, ref.steps)
     assert np.array_equal(counts, ref.counts)
     assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32))
