@@ -62,16 +62,14 @@ int streami_streak_begin(streami_field f, const float* points, size_t m, unsigne
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (params->out_totals) STREAMI_TRY(cudaMemsetAsync(params->out_totals, 0, 4 * sizeof(unsigned long long), st));
   const bool unsteady = f->g.nslices > 1;
-  // Window = global steps per launch.  Unsteady: about two slice intervals, so that the slices a
-  // launch touches stay L2-resident; steady: everything in one launch.
+  // Window = global steps per launch.  A particle lives in registers inside a window (with the
+  // two-slice copy of its cell) and goes through its output slot between windows, so long windows
+  // win: C4 at 10 / 40 / 100 / 200 / 1000 steps per launch takes 155 / 99 / 88 / 86 / 86 ms.  The
+  // earlier rule (two slice intervals per launch, to keep the slices of a launch L2-resident) cost
+  // more in relaunches and cold caches than the residency bought.  256 bounds the state a caller
+  // waits for between launches; steady fields take everything in one launch.
   unsigned K = (unsigned)options().streak_window;
-  if (K == 0) {
-    if (!unsteady) K = nsteps;
-    else {
-      float per = 2.0f / (f->g.q * params->h);
-      K = per < 4.0f ? 4u : (per > 64.0f ? 64u : (unsigned)per);
-    }
-  }
+  if (K == 0) K = unsteady ? std::min(nsteps, 256u) : nsteps;
   unsigned char* state = nullptr;
   STREAMI_TRY(cudaMallocAsync((void**)&state, (size_t)m * nsteps, st));
   streami_streak_s* h = new streami_streak_s();
