@@ -336,6 +336,11 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CC& cc
         interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V + 24, fx, fy, fz, wx, wy, wz);
         vx = lerp(ux, wx, a); vy = lerp(uy, wy, a); vz = lerp(uz, wz, a);   // space first, time last
         return 0;
+      } else {                                         // hold-floor-slice mode: one slice, the first half of the copy
+        const unsigned long long k1 = vj | (1ull << 63);
+        if (k1 != cc.key) { load_cell<LAYOUT>(s, vj, cc.V); cc.key = k1; }
+        interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, vx, vy, vz);
+        return 0;
       }
     }
     float V[24];

@@ -68,6 +68,33 @@ def test_streaklines_double_gyre(S, torch, oracle, wl, layout, window, cache):
     assert np.count_nonzero(ref.status == 1) >= nsteps       # the outside point, every release
 
 
+@pytest.mark.parametrize("cache", [1, 0])
+@pytest.mark.parametrize("layout", [3, 5])
+def test_streaklines_hold_floor_slice(S, torch, oracle, wl, layout, cache):
+    """The paper's own time handling (fields[(int)simTime]; time_mode = 1) through
+    the streakline kernel, with and without the register copy of the cell, two window lengths."""
+    fld = wl.double_gyre_field(dims=(64, 32, 16), nslices=10, dt=0.25)
+    pts = np.concatenate([wl.rake_c4(16, 8), np.array([[2.5, 0.5, 0.5], [1.999, 0.5, 0.999]], dtype=np.float32)])
+    nsteps = 70
+    kw = dict(integrator=0, h=0.05, vmin=0.0, t0=0.0)
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt, 1)
+    ref = oracle.streaklines(g, pts, nsteps, oracle.params(**kw), "f32")
+    kw["time_mode"] = 1
+    S.streami_set_option("cell_cache", cache)
+    try:
+        for window in (0, 9):
+            S.streami_set_option("streak_window", window)
+            v, counts, steps, status, totals = gpu_streaklines(S, torch, gpu_field(S, torch, fld, layout),
+                                                               pts, nsteps, **kw)
+            assert np.array_equal(status, ref.status) and np.array_equal(steps, ref.steps)
+            assert np.array_equal(counts, ref.counts)
+            assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32))
+            assert np.array_equal(totals[:3], ref.totals[:3])
+    finally:
+        S.streami_set_option("streak_window", 0)
+        S.streami_set_option("cell_cache", 1)
+
+
 def test_streaklines_steady_field_with_deaths(S, torch, oracle, wl):
     fld = wl.turb_field_cpu(32, 48, 1, 6)
     pts = wl.seeds_uniform(3, 300, [31.0] * 3)
