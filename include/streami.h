@@ -283,7 +283,7 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
 
 /* Tuning knobs (process-wide).  None changes any result: they select schedules and staging only,
  * and exist so that each design choice can be measured A/B in one process.  name is one of
- *   "cell_cache"        0/1   keep the 8 cell vertices in registers while samples stay in the cell
+ *   "cell_cache"        0/1   keep the 8 cell vertices (streaklines: of both slices) in registers while samples stay in the cell
  *   "presort"           0/1   process work items in Morton order of their 4^3-cell block
  *   "segment_steps"     K     streamlines: K step attempts per particle per launch, survivors are
  *                             re-sorted between launches (0 = one launch; DP5(4) then synchronises)
@@ -294,6 +294,9 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
  *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0)
  *   "streak_window"     W     streaklines: global steps per launch (0 = automatic)
  *   "host_batch"        S     streami_trace_streamlines_lines_host: seeds per batch (0 = automatic)
+ *   "queue_steps"       Q     steady RK4 streamlines: a particle passes through a device queue, consumed by
+ *                             the same launch, every Q steps, so that the launch runs breadth first and
+ *                             ends without a long tail (0 = off, the default)
  *   "kernel_timing"     0/1   record a CUDA event pair around every advection-kernel launch
  * Returns INVALID for unknown names. */
 int streami_set_option(const char* name, int value);

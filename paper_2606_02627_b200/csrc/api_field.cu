@@ -12,7 +12,7 @@
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0, 1, 0}; return o; }
+Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0, 1, 0, 0}; return o; }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -405,6 +405,7 @@ int streami_set_option(const char* name, int value) {
   else if (!strcmp(name, "prefetch")) o.prefetch = value < 0 ? 0 : (value > 2 ? 2 : value);
   else if (!strcmp(name, "integer_accept")) o.integer_accept = value != 0;
   else if (!strcmp(name, "host_batch")) o.host_batch = value < 0 ? 0 : value;
+  else if (!strcmp(name, "queue_steps")) o.queue_steps = value < 0 ? 0 : value;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }
@@ -423,6 +424,7 @@ int streami_get_option(const char* name, int* value) {
   else if (!strcmp(name, "prefetch")) *value = o.prefetch;
   else if (!strcmp(name, "integer_accept")) *value = o.integer_accept;
   else if (!strcmp(name, "host_batch")) *value = o.host_batch;
+  else if (!strcmp(name, "queue_steps")) *value = o.queue_steps;
   else return STREAMI_E_INVALID;
   return STREAMI_OK;
 }

@@ -36,6 +36,21 @@ TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, 
   }
 }
 
+// Steady monolithic RK4 with the cell cache and the in-kernel continuation queue (trace_kernel.cuh, INQ).
+template <int L>
+static TraceKernel pick_inq_l(bool unit) {
+  return unit ? trace_kernel<L, 0, false, false, true, true, true> : trace_kernel<L, 0, false, false, true, false, true>;
+}
+static TraceKernel pick_trace_kernel_inq(int layout, bool unit) {
+  switch (layout) {
+    case LAYOUT_PACKED3: return pick_inq_l<LAYOUT_PACKED3>(unit);
+    case LAYOUT_FLOAT4: return pick_inq_l<LAYOUT_FLOAT4>(unit);
+    case LAYOUT_CELL: return pick_inq_l<LAYOUT_CELL>(unit);
+    case LAYOUT_XYQUAD: return pick_inq_l<LAYOUT_XYQUAD>(unit);
+    default: return pick_inq_l<LAYOUT_XPAIR>(unit);
+  }
+}
+
 bool unit_geometry(const Geom& g) {
   return g.ox == 0.0f && g.oy == 0.0f && g.oz == 0.0f && g.rx == 1.0f && g.ry == 1.0f && g.rz == 1.0f;
 }
@@ -97,10 +112,6 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   const bool unsteady = f->g.nslices > 1;
   const bool cache = options().cell_cache && !unsteady;
   TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache, unit_geometry(f->g));
-  int grid = 0;
-  const int block = trace_block(params->integrator);
-  rc = trace_grid(k, n, block, &grid);
-  if (rc) return rc;
 
   // Segments: K step attempts per particle per launch, Morton re-sort of the survivors between
   // launches (trace_kernel.cuh).  K = 0, or a trace too short or too small to need it: one launch.
@@ -109,21 +120,54 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   if (!sorting || K >= params->max_steps) K = 0;
   const bool dp5 = params->integrator == 1;
 
-  // scratch: [0] work counter u64, [8] queue counts u32 x 2
+  // In-kernel continuation queue (trace_kernel.cuh, INQ): steady RK4 with the cell cache, one launch.
+  // Option "queue_steps" = Q > 0: steps per particle between two passes through the queue (0 = off, the
+  // default: on C2 the shorter tail does not pay for the passes).  A particle
+  // is queued at most floor(max_steps / Q) times, which sizes the queue; if that does not fit, the
+  // launch runs without.
+  unsigned Q = 0;
+  if (!dp5 && !unsteady && cache && K == 0 && options().queue_steps > 0) {
+    Q = (unsigned)options().queue_steps;
+    if (Q >= params->max_steps) Q = 0;
+  }
+  unsigned long long qcap = Q ? (unsigned long long)n * (params->max_steps / Q) : 0ull;
+  if (qcap >= 0xffffffffull) { Q = 0; qcap = 0; }
+  QRec* cq = nullptr;
+  if (Q) {
+    cudaError_t qe = cudaMallocAsync((void**)&cq, sizeof(QRec) * qcap, st);
+    if (qe == cudaSuccess) qe = cudaMemsetAsync(cq, 0, sizeof(QRec) * qcap, st);   // all-zero = not written yet
+    if (qe != cudaSuccess) {
+      cudaGetLastError();
+      if (cq) cudaFreeAsync(cq, st);
+      cq = nullptr; Q = 0;
+    } else {
+      k = pick_trace_kernel_inq(f->layout, unit_geometry(f->g));
+    }
+  }
+  int grid = 0;
+  const int block = trace_block(params->integrator);
+  rc = trace_grid(k, n, block, &grid);
+  if (rc) { if (cq) cudaFreeAsync(cq, st); return rc; }
+
+  // scratch: [0] work counter u64, [8] queue counts u32 x 2 (INQ: tail, head), [16] INQ: particles terminated
   char* ctr = nullptr;
-  STREAMI_TRY(cudaMallocAsync((void**)&ctr, 16, st));
+  {
+    cudaError_t ce = cudaMallocAsync((void**)&ctr, 32, st);
+    if (ce != cudaSuccess) { if (cq) cudaFreeAsync(cq, st); return check(ce); }
+  }
   unsigned long long* next = (unsigned long long*)ctr;
   unsigned* qcount = (unsigned*)(ctr + 8);
   unsigned* perm = nullptr; QRec* q[2] = {nullptr, nullptr};
   MortonSorter sorter{}; bool have_sorter = false;
   auto cleanup = [&]() {
     cudaFreeAsync(ctr, st);
+    if (cq) cudaFreeAsync(cq, st);
     if (perm) cudaFreeAsync(perm, st);
     if (q[0]) cudaFreeAsync(q[0], st);
     if (q[1]) cudaFreeAsync(q[1], st);
     if (have_sorter) sorter.release();
   };
-  cudaError_t e = cudaMemsetAsync(ctr, 0, 16, st);
+  cudaError_t e = cudaMemsetAsync(ctr, 0, 32, st);
   if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
   if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
   if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
@@ -145,6 +189,10 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
   a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
+  if (Q) {
+    a.seg_budget = Q; a.qout = cq; a.qout_count = qcount; a.cq_head = qcount + 1;
+    a.cq_done = (unsigned*)(ctr + 16); a.cq_cap = (unsigned)qcap;
+  }
   timing_begin(st);
   k<<<grid, block, 0, st>>>(a);
   timing_end(st);

@@ -23,7 +23,7 @@ struct streami_field_s {
 
 namespace streami {
 
-struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; int segment_steps; int vertex_staging; int prefetch; int max_blocks_per_sm; int brick_round_steps; int integer_accept; int host_batch; };
+struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; int segment_steps; int vertex_staging; int prefetch; int max_blocks_per_sm; int brick_round_steps; int integer_accept; int host_batch; int queue_steps; };
 Options& options();
 std::atomic<unsigned long long>& launch_counter();
 void set_cuda_error(cudaError_t e);

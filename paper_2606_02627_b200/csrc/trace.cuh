@@ -47,6 +47,10 @@ struct TraceArgs {
   unsigned long long* totals;      // [4]
   // brick outputs
   QRec* qout; unsigned* qout_count;
+  // in-kernel continuation queue (trace_kernel.cuh, INQ): qout, zero-initialised, is consumed by the same launch
+  unsigned* cq_head;               // next index to claim
+  unsigned* cq_done;               // particles terminated so far
+  unsigned cq_cap;
   unsigned* rc_this;               // round_counts row of this round (round 0 only), or NULL
   unsigned* rc_next;               // round_counts row of the next round, or NULL
   unsigned long long* log; unsigned long long log_cap; unsigned long long* log_count;

@@ -1,7 +1,7 @@
 """Schedule-only options must not change any result: segments with Morton re-sort of the survivors
 (`segment_steps`), the one-step-ahead cell prefetch (`prefetch`), the staged vertex writer
 (`vertex_staging`), the occupancy limit (`max_blocks_per_sm`), the integer domain test
-(`integer_accept`).  Each combination is compared bit for
+(`integer_accept`), the continuation queue consumed by the same launch (`queue_steps`).  Each combination is compared bit for
 bit with the oracle (RK4 and DP5(4), every layout family), with capacities that are and are not a
 multiple of the 8-slot staging group, and with a stride that cuts groups at segment boundaries."""
 import numpy as np
@@ -32,7 +32,7 @@ def turb48(wl):
     return wl.turb_field_cpu(48, 64, 1, 12)
 
 
-DEFAULTS = dict(segment_steps=0, prefetch=1, vertex_staging=1, max_blocks_per_sm=0, presort=1)
+DEFAULTS = dict(segment_steps=0, prefetch=1, vertex_staging=1, max_blocks_per_sm=0, presort=1, queue_steps=0)
 
 
 def _with(S, opts, fn):
@@ -45,10 +45,12 @@ def _with(S, opts, fn):
             S.streami_set_option(k, v)
 
 
-@pytest.mark.parametrize("layout", [1, 3, 4])
+@pytest.mark.parametrize("layout", [1, 3, 4, 5])
 @pytest.mark.parametrize("opts", [dict(segment_steps=16), dict(segment_steps=37, prefetch=0),
                                   dict(vertex_staging=0), dict(prefetch=2, max_blocks_per_sm=1),
-                                  dict(segment_steps=5, vertex_staging=0, presort=1)])
+                                  dict(segment_steps=5, vertex_staging=0, presort=1),
+                                  dict(queue_steps=16), dict(queue_steps=7, vertex_staging=0),
+                                  dict(queue_steps=50, prefetch=0, max_blocks_per_sm=1)])
 def test_rk4_schedule_options(S, torch, oracle, wl, turb48, layout, opts):
     n = 70001                                      # >= 65536: sorting and segments are active
     seeds = wl.seeds_uniform(11, n, [47.0] * 3)
@@ -59,6 +61,21 @@ def test_rk4_schedule_options(S, torch, oracle, wl, turb48, layout, opts):
         ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
         out = _with(S, opts, lambda: gpu_streamlines(S, torch, f, seeds, **kw))
         assert_same(out, ref, "rk4 %s %s" % (opts, kw))
+
+
+@pytest.mark.parametrize("n", [1, 37, 5000])
+@pytest.mark.parametrize("q", [1, 10, 64])
+def test_continuation_queue_small_launches(S, torch, oracle, wl, turb48, n, q):
+    """`queue_steps` with fewer particles than lanes (most warps only ever poll), seeds outside the
+    domain (terminated before their first step) and particles that are queued at step max_steps."""
+    seeds = wl.seeds_uniform(13, n, [47.0] * 3)
+    seeds[::5, 0] += 60.0                           # every fifth seed starts outside
+    g = oracle.grid(turb48.data, turb48.dims, turb48.origin, turb48.spacing)
+    f = gpu_field(S, torch, turb48, 5)
+    kw = dict(integrator=0, h=0.25, max_steps=128, vmin=1e-6, capacity=40, stride=4)
+    ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
+    out = _with(S, dict(queue_steps=q), lambda: gpu_streamlines(S, torch, f, seeds, **kw))
+    assert_same(out, ref, "queue n=%d q=%d" % (n, q))
 
 
 @pytest.mark.parametrize("layout", [3, 4])
