@@ -574,6 +574,12 @@ def main():
                     roofline["traffic_source"] = row["source"]
                     roofline["ncu"] = {k: float(v) for k, v in row.items()
                                        if k not in ("workload", "source", "dram_bytes_per_launch")}
+                    # the same kernel against the same peak, but with the DRAM bytes ncu counted for one launch
+                    # (the profiled launch; C4's launches differ in work, see profiles/traffic.md) instead of the
+                    # algorithmic bytes: how far the memory system, not the method's request stream, is loaded
+                    if kms > 0:
+                        roofline["dram_gbs_from_traffic"] = roofline["traffic"] / (kms * 1e-3) / 1e9
+                        roofline["dram_frac_from_traffic"] = roofline["dram_gbs_from_traffic"] / peak
 
     cpu = None
     if world == 1 and not args.no_cpu and job.host_field is not None:

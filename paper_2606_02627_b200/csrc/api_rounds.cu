@@ -22,7 +22,7 @@ void fill_integrator(TraceArgs& a, const streami_params* p);
 typedef void (*StreakKernel)(const StreakArgs);
 template <int LAYOUT>
 static StreakKernel pick_streak_l(bool unsteady, bool tcache) {
-  if (!unsteady) return streak_kernel<LAYOUT, false, false>;
+  if (!unsteady) return tcache ? streak_kernel<LAYOUT, false, true> : streak_kernel<LAYOUT, false, false>;
   return tcache ? streak_kernel<LAYOUT, true, true> : streak_kernel<LAYOUT, true, false>;
 }
 static StreakKernel pick_streak(int layout, bool unsteady, bool tcache) {

@@ -148,8 +148,8 @@ struct StreakArgs {
   unsigned long long* totals;
 };
 
-// TCACHE (option "cell_cache", unsteady fields read linearly in time): the two-slice cell copy of
-// field.cuh stays in registers across the stages and steps of a window.
+// TCACHE (option "cell_cache"): the copy of the current cell (field.cuh; both slices of it for an
+// unsteady field) stays in registers across the stages and steps of a window.
 template <int LAYOUT, bool UNSTEADY, bool TCACHE>
 __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
   __shared__ unsigned long long s_tot[3];
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
     if (run) {
       TraceArgs ta;                                              // only the fields rk4_step reads
       ta.g = a.g; ta.h = a.h; ta.h2 = a.h2; ta.h6 = a.h6; ta.vmin2 = a.vmin2;
-      ta.max_steps = 0xffffffffu; ta.verts = nullptr; ta.cap = 0; ta.stride = 0xffffffffu;
+      ta.max_steps = 0xffffffffu; ta.verts = nullptr; ta.cap = 0; ta.stride = 0xffffffffu; ta.prefetch = 0;
       Lane L; L.px = px; L.py = py; L.pz = pz; L.id = 0; L.slot = 0; L.rec_cd = 0xffffffffu;
       typename StreakCache<UNSTEADY && TCACHE>::type cc; cc.invalidate();
       unsigned n_samples = 0, n_attempts = 0;
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(256) streak_kernel(const StreakArgs a) {
         L.n = s;                                                 // t_s = t0 + (float)s*h, shared by all
         ta.t0 = a.t0;
         unsigned done;
-        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, UNSTEADY && TCACHE, false, false>(ta, a.s, cc, L, done);
+        unsigned rc = rk4_step<LAYOUT, UNSTEADY, false, TCACHE, false, false>(ta, a.s, cc, L, done);
         if (rc) { st = rc; n_attempts = done >= 2u ? 1u : 0u; n_samples = min(done, 4u); break; }
       }
       n_attempts += s - s_first; n_samples += 4u * (s - s_first);

@@ -102,13 +102,15 @@ def test_streaklines_steady_field_with_deaths(S, torch, oracle, wl):
     kw = dict(integrator=0, h=0.25, vmin=1e-6, t0=0.0)
     ref = oracle.streaklines(oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing), pts, nsteps,
                              oracle.params(**kw), "f32")
-    for window in (0, 16):
+    for window, cache in ((0, 1), (16, 1), (0, 0), (16, 0)):
         S.streami_set_option("streak_window", window)
+        S.streami_set_option("cell_cache", cache)
         try:
             v, counts, steps, status, totals = gpu_streaklines(S, torch, gpu_field(S, torch, fld), pts,
                                                                nsteps, **kw)
         finally:
             S.streami_set_option("streak_window", 0)
+            S.streami_set_option("cell_cache", 1)
         assert np.array_equal(status, ref.status) and np.array_equal(steps, ref.steps)
         assert np.array_equal(counts, ref.counts)
         assert np.array_equal(v.view(np.uint32), ref.vertices.view(np.uint32))
