@@ -21,6 +21,7 @@ static TraceKernel pick_lu(int integ, bool brick, bool cache) {      // steady
 
 template <int L>
 static TraceKernel pick_l(int integ, bool unsteady, bool brick, bool cache, bool unit) {
+  if (unsteady && cache) return integ ? trace_kernel<L, 1, true, false, true, false> : trace_kernel<L, 0, true, false, true, false>;
   if (unsteady) return integ ? trace_kernel<L, 1, true, false, false, false> : trace_kernel<L, 0, true, false, false, false>;
   return unit ? pick_lu<L, true>(integ, brick, cache) : pick_lu<L, false>(integ, brick, cache);
 }
@@ -110,7 +111,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   if (n == 0) return STREAMI_OK;
 
   const bool unsteady = f->g.nslices > 1;
-  const bool cache = options().cell_cache && !unsteady;
+  const bool cache = options().cell_cache != 0;     // unsteady fields: the two-slice copy (CellCacheT)
   TraceKernel k = pick_trace_kernel(f->layout, params->integrator, unsteady, false, cache, unit_geometry(f->g));
 
   // Segments: K step attempts per particle per launch, Morton re-sort of the survivors between

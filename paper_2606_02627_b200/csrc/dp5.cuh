@@ -58,8 +58,8 @@ __device__ __forceinline__ float rp10(float x) {
   if (rc) return rc;
 
 // One DP5(4) attempt.  L.k1 holds k1 (FSAL).  Returns 0 to continue, else the final status.
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT>
-__device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store& s, CellCache& cc,
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, class CC = CellCache>
+__device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store& s, CC& cc,
                                                 Lane& L, unsigned& n_samples, unsigned& n_attempts) {
   if (L.n == a.max_steps) return ST_MAXSTEPS;
   const float k1x = L.k1x, k1y = L.k1y, k1z = L.k1z;

@@ -70,7 +70,12 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
 
 // Resident blocks per SM the compiler must allow for.  3 blocks of 256 (<= 80 registers): capping
 // the steady RK4 kernel at 64 registers for a 4th block was measured on C2 and lost to its spills.
-constexpr int trace_min_blocks(int integ, bool unsteady, bool brick) { return integ == 1 ? 5 : STREAMI_RK4_MIN_BLOCKS; }
+// Pathlines with the two-slice cell copy (48 more registers): 2 blocks of 256 (RK4), 3 of 128 (DP5(4)).
+constexpr int trace_min_blocks(int integ, bool unsteady, bool brick, bool cache) {
+  return (unsteady && cache) ? (integ == 1 ? 3 : 2) : (integ == 1 ? 5 : STREAMI_RK4_MIN_BLOCKS);
+}
+template <bool T> struct TraceCache { typedef CellCache type; };
+template <> struct TraceCache<true> { typedef CellCacheT type; };
 
 // INQ (build's choice; results unchanged): the continuation queue is consumed by the SAME launch.
 // A particle that has spent its step budget is appended to the queue as above; a lane that finds
@@ -95,7 +100,7 @@ __device__ __forceinline__ uint4 ld_volatile_v4(const uint4* p) {
 }
 
 template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool INQ = false>
-__global__ void __launch_bounds__(trace_block(INTEG), trace_min_blocks(INTEG, UNSTEADY, BRICK))
+__global__ void __launch_bounds__(trace_block(INTEG), trace_min_blocks(INTEG, UNSTEADY, BRICK, CACHE))
 trace_kernel(const TraceArgs a) {
   __shared__ unsigned long long s_tot[4];
   if (threadIdx.x < 4) s_tot[threadIdx.x] = 0ull;
@@ -105,7 +110,7 @@ trace_kernel(const TraceArgs a) {
   const unsigned FULL = 0xffffffffu;
   const unsigned long long nwork = a.nwork_dev ? (unsigned long long)*a.nwork_dev : a.nwork;
   Lane L; L.rejected = false; L.pf = 0xffffffffu;
-  CellCache cc; cc.invalidate();
+  typename TraceCache<UNSTEADY && CACHE>::type cc; cc.invalidate();
   Store st = a.s;                 // brick mode: replaced per particle
   int my_brick = 0;
   bool active = false, exhausted = false;

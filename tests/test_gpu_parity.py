@@ -154,9 +154,11 @@ def test_dp5_forced_floor_and_tight_tolerance(S, torch, oracle, wl, turb48):
 
 
 # ---- unsteady streamlines (pathlines through slices) -----------------------------------------
+@pytest.mark.parametrize("cache", [1, 0])
 @pytest.mark.parametrize("layout", LAYOUTS)
 @pytest.mark.parametrize("integrator", [0, 1])
-def test_unsteady_pathlines(S, torch, oracle, wl, layout, integrator):
+def test_unsteady_pathlines(S, torch, oracle, wl, layout, integrator, cache):
+    """cache = the two-slice register copy of the current cell (option "cell_cache"), on and off."""
     fld = wl.double_gyre_field(dims=(64, 32, 16), nslices=12, dt=0.25)
     seeds = wl.seeds_uniform(5, 4099, [2.0, 1.0, 1.0])
     kw = dict(integrator=integrator, h=0.05, h_min=0.001, h_max=0.5, atol=1e-6, rtol=1e-6,
@@ -165,9 +167,13 @@ def test_unsteady_pathlines(S, torch, oracle, wl, layout, integrator):
         g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt,
                         time_mode)
         ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
-        out = gpu_streamlines(S, torch, gpu_field(S, torch, fld, layout), seeds, time_mode=time_mode,
-                              **kw)
-        assert_same(out, ref, "unsteady tm=%d" % time_mode)
+        S.streami_set_option("cell_cache", cache)
+        try:
+            out = gpu_streamlines(S, torch, gpu_field(S, torch, fld, layout), seeds, time_mode=time_mode,
+                                  **kw)
+        finally:
+            S.streami_set_option("cell_cache", 1)
+        assert_same(out, ref, "unsteady tm=%d cache=%d" % (time_mode, cache))
 
 
 # ---- edge cases ------------------------------------------------------------------------------
