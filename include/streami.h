@@ -291,7 +291,8 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
  *   "integer_accept"    0/1   steady RK4 on a field of finite values: decide "inside" from floor(g)
  *   "vertex_staging"    0/1   stage vertices in shared memory and store full 32-byte sectors
  *   "max_blocks_per_sm" B     limit resident blocks per SM (0 = as many as fit)
- *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0)
+ *   "brick_round_steps" k     brick rounds, see streami_brick_advect (-1, 0 = automatic, k > 0; -2 = one launch,
+ *                             hand-offs through a device ring consumed by the same launch, if rounds are not observed)
  *   "streak_window"     W     streaklines: global steps per launch (0 = automatic)
  *   "host_batch"        S     streami_trace_streamlines_lines_host: seeds per batch (0 = automatic)
  *   "queue_steps"       Q     steady RK4 streamlines: a particle passes through a device queue, consumed by

@@ -400,7 +400,7 @@ int streami_set_option(const char* name, int value) {
   else if (!strcmp(name, "kernel_timing")) o.kernel_timing = value != 0;
   else if (!strcmp(name, "segment_steps")) o.segment_steps = value < 0 ? 0 : value;
   else if (!strcmp(name, "vertex_staging")) o.vertex_staging = value != 0;
-  else if (!strcmp(name, "brick_round_steps")) o.brick_round_steps = value < -1 ? -1 : value;
+  else if (!strcmp(name, "brick_round_steps")) o.brick_round_steps = value < -2 ? -2 : value;
   else if (!strcmp(name, "max_blocks_per_sm")) o.max_blocks_per_sm = value < 0 ? 0 : value;
   else if (!strcmp(name, "prefetch")) o.prefetch = value < 0 ? 0 : (value > 2 ? 2 : value);
   else if (!strcmp(name, "integer_accept")) o.integer_accept = value != 0;

@@ -14,6 +14,7 @@
 namespace streami {
 typedef void (*TraceKernel)(const TraceArgs);
 TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, bool cache, bool unit);
+TraceKernel pick_trace_kernel_inq(int layout, bool unit, bool brick);
 bool unit_geometry(const Geom& g);
 int trace_grid(TraceKernel k, unsigned long long nwork, int block, int* grid);
 int check_params(const streami_params* p, bool need_capacity);
@@ -37,6 +38,77 @@ static StreakKernel pick_streak(int layout, bool unsteady, bool tcache) {
 }  // namespace streami
 
 using namespace streami;
+
+// Brick advection in ONE launch (trace_kernel.cuh, INQ): a particle that leaves its brick, or has
+// spent its step budget, is appended to a device ring that the lanes of the same launch consume once
+// the seeds are gone.  The hand-off itself is unchanged (32-byte record into the queue, one atomic
+// per warp, picked up with the destination brick's descriptor); what goes away is
+// the round structure: one sort, launch, count readback and tail per round (C3: 37 rounds).  Used
+// only on request (option "brick_round_steps" = -2) and when the caller does not observe A9's rounds
+// (no round table, no hand-off log).  The ring holds 2^shift >= 2n records: at most n are queued at any time (a
+// particle is in at most one), and a slot is overwritten only after 2^shift later records.
+static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const streami_params* params,
+                            float* out_vertices, unsigned* out_counts, unsigned* out_nrounds, cudaStream_t st) {
+  TraceKernel k = pick_trace_kernel_inq(f->layout, unit_geometry(f->g), true);
+  const int block = trace_block(0);
+  unsigned shift = 10;
+  while ((1ull << shift) < 2ull * n) ++shift;
+  if (shift > 31) return STREAMI_E_INVALID;
+  const size_t cap = (size_t)1 << shift;
+  char* ctr = nullptr; QRec* cq = nullptr; unsigned* perm = nullptr;
+  MortonSorter sorter{}; bool have_sorter = false;
+  const bool sorting = options().presort && n >= 65536;
+  auto cleanup = [&]() {
+    if (ctr) cudaFreeAsync(ctr, st);
+    if (cq) cudaFreeAsync(cq, st);
+    if (perm) cudaFreeAsync(perm, st);
+    if (have_sorter) sorter.release();
+  };
+  // scratch: [0] work counter u64, [8] ring tail u32, [12] ring head u32, [16] particles done u32, [20] error u32
+  cudaError_t e = cudaMallocAsync((void**)&ctr, 32, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ctr, 0, 32, st);
+  if (e == cudaSuccess) e = cudaMallocAsync((void**)&cq, sizeof(QRec) * cap, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(cq, 0, sizeof(QRec) * cap, st);
+  if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+  if (e != cudaSuccess) { cleanup(); return check(e); }
+  int rc = STREAMI_OK;
+  if (sorting) {
+    rc = sorter.init(f, n, st);
+    if (rc) { cleanup(); return rc; }
+    have_sorter = true;
+    rc = sorter.sort(f->g, seeds, 3, n, nullptr, perm);
+    if (rc) { cleanup(); return rc; }
+  }
+  TraceArgs a{};
+  a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
+  a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = (int)f->bricks.size();
+  a.brick_fast = options().integer_accept;
+  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr;
+  a.next = (unsigned long long*)ctr; a.round = 0;
+  a.seg_budget = options().queue_steps > 0 ? (unsigned)options().queue_steps : 0u;   // 0 = until the particle leaves its brick
+  fill_integrator(a, params);
+  a.verts = out_vertices; a.n = n; a.counts = out_counts;
+  a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
+  a.qout = cq; a.qout_count = (unsigned*)(ctr + 8); a.cq_head = (unsigned*)(ctr + 12);
+  a.cq_done = (unsigned*)(ctr + 16); a.cq_error = (unsigned*)(ctr + 20);
+  a.cq_mask = (unsigned)(cap - 1); a.cq_shift = shift;
+  int grid = 0;
+  rc = trace_grid(k, n, block, &grid);
+  if (rc) { cleanup(); return rc; }
+  timing_begin(st);
+  k<<<grid, block, 0, st>>>(a);
+  timing_end(st);
+  launch_counter()++;
+  e = cudaGetLastError();
+  unsigned err = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&err, ctr + 20, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  cleanup();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // streami_brick_advect synchronises its stream (streami.h)
+  if (e != cudaSuccess) return check(e);
+  if (err) return STREAMI_E_CUDA;
+  if (out_nrounds) *out_nrounds = 1;
+  return STREAMI_OK;
+}
 
 extern "C" {
 
@@ -210,6 +282,10 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   if (n == 0) return check(cudaStreamSynchronize(st));
 
   const bool cache = options().cell_cache != 0;
+  // brick_round_steps = -2: one launch with the in-kernel ring instead of rounds (measured on C3: 158 ms
+  // against 157 ms for sorted rounds -- the Morton sort of every round is worth what the rounds cost)
+  if (options().brick_round_steps == -2 && !out_round_counts && !out_handoff_log && params->integrator == 0 && cache)
+    return brick_advect_inq(f, seeds, n, params, out_vertices, out_counts, out_nrounds, st);
   TraceKernel k = pick_trace_kernel(f->layout, params->integrator, false, true, cache, unit_geometry(f->g));
   const int block = trace_block(params->integrator);
 
@@ -250,7 +326,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   {
     const int o = options().brick_round_steps;
     const bool observed = out_round_counts || out_handoff_log;
-    a.seg_budget = o > 0 ? (unsigned)o : ((o == 0 && !observed) ? 256u : 0u);
+    a.seg_budget = o > 0 ? (unsigned)o : ((o == 0 && !observed) ? 256u : 0u);   // o < 0: A9's rounds
   }
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;

@@ -39,16 +39,17 @@ TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, 
 
 // Steady monolithic RK4 with the cell cache and the in-kernel continuation queue (trace_kernel.cuh, INQ).
 template <int L>
-static TraceKernel pick_inq_l(bool unit) {
+static TraceKernel pick_inq_l(bool unit, bool brick) {
+  if (brick) return unit ? trace_kernel<L, 0, false, true, true, true, true> : trace_kernel<L, 0, false, true, true, false, true>;
   return unit ? trace_kernel<L, 0, false, false, true, true, true> : trace_kernel<L, 0, false, false, true, false, true>;
 }
-static TraceKernel pick_trace_kernel_inq(int layout, bool unit) {
+TraceKernel pick_trace_kernel_inq(int layout, bool unit, bool brick) {
   switch (layout) {
-    case LAYOUT_PACKED3: return pick_inq_l<LAYOUT_PACKED3>(unit);
-    case LAYOUT_FLOAT4: return pick_inq_l<LAYOUT_FLOAT4>(unit);
-    case LAYOUT_CELL: return pick_inq_l<LAYOUT_CELL>(unit);
-    case LAYOUT_XYQUAD: return pick_inq_l<LAYOUT_XYQUAD>(unit);
-    default: return pick_inq_l<LAYOUT_XPAIR>(unit);
+    case LAYOUT_PACKED3: return pick_inq_l<LAYOUT_PACKED3>(unit, brick);
+    case LAYOUT_FLOAT4: return pick_inq_l<LAYOUT_FLOAT4>(unit, brick);
+    case LAYOUT_CELL: return pick_inq_l<LAYOUT_CELL>(unit, brick);
+    case LAYOUT_XYQUAD: return pick_inq_l<LAYOUT_XYQUAD>(unit, brick);
+    default: return pick_inq_l<LAYOUT_XPAIR>(unit, brick);
   }
 }
 
@@ -131,8 +132,14 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
     Q = (unsigned)options().queue_steps;
     if (Q >= params->max_steps) Q = 0;
   }
-  unsigned long long qcap = Q ? (unsigned long long)n * (params->max_steps / Q) : 0ull;
-  if (qcap >= 0xffffffffull) { Q = 0; qcap = 0; }
+  // ring of 2^shift records >= the passes of all particles: a slot is written once, its tag is always 1
+  unsigned long long qcap = 0; unsigned qshift = 0;
+  if (Q) {
+    const unsigned long long need = (unsigned long long)n * (params->max_steps / Q);
+    while ((1ull << qshift) < need) ++qshift;
+    qcap = 1ull << qshift;
+    if (qshift > 31) { Q = 0; qcap = 0; }
+  }
   QRec* cq = nullptr;
   if (Q) {
     cudaError_t qe = cudaMallocAsync((void**)&cq, sizeof(QRec) * qcap, st);
@@ -142,7 +149,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
       if (cq) cudaFreeAsync(cq, st);
       cq = nullptr; Q = 0;
     } else {
-      k = pick_trace_kernel_inq(f->layout, unit_geometry(f->g));
+      k = pick_trace_kernel_inq(f->layout, unit_geometry(f->g), false);
     }
   }
   int grid = 0;
@@ -192,7 +199,8 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
   if (Q) {
     a.seg_budget = Q; a.qout = cq; a.qout_count = qcount; a.cq_head = qcount + 1;
-    a.cq_done = (unsigned*)(ctr + 16); a.cq_cap = (unsigned)qcap;
+    a.cq_done = (unsigned*)(ctr + 16); a.cq_error = (unsigned*)(ctr + 20);
+    a.cq_mask = (unsigned)(qcap - 1ull); a.cq_shift = qshift;
   }
   timing_begin(st);
   k<<<grid, block, 0, st>>>(a);

@@ -50,7 +50,8 @@ struct TraceArgs {
   // in-kernel continuation queue (trace_kernel.cuh, INQ): qout, zero-initialised, is consumed by the same launch
   unsigned* cq_head;               // next index to claim
   unsigned* cq_done;               // particles terminated so far
-  unsigned cq_cap;
+  unsigned* cq_error;              // set if a warp gave up waiting (never, unless a record was lost)
+  unsigned cq_mask, cq_shift;      // ring of 2^cq_shift records
   unsigned* rc_this;               // round_counts row of this round (round 0 only), or NULL
   unsigned* rc_next;               // round_counts row of the next round, or NULL
   unsigned long long* log; unsigned long long log_cap; unsigned long long* log_count;

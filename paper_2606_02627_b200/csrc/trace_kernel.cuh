@@ -43,15 +43,17 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
   r.pad0 = 0; r.pad1 = 0;
   if (INTEG == 1) { r.pad0 = __float_as_uint(L.t); r.pad1 = __float_as_uint(L.h); }
   if (INQ) {
-    // Self-validating halves, each ONE aligned 16-byte store into zero-initialised memory: ~id != 0
-    // (ids stay below 2^32 - 1) and n + 1 != 0 mark a half as written.  No fence: a gpu-scope fence
-    // invalidates the SM's L1 and with it the lines the cell prefetcher has just brought in
-    // (measured: L1 hit rate 47 -> 12 %, C2 15.7 -> 18.8 ms with __threadfence + a flag word).
-    uint4* q = reinterpret_cast<uint4*>(a.qout + pos);
+    // Ring slot pos & mask, two self-validating halves, each ONE aligned 16-byte store: both carry
+    // the tag (pos >> shift) + 1 of this pass through the ring (the memory starts zeroed, tags start
+    // at 1).  No fence: a gpu-scope fence invalidates the SM's L1 and with it the lines the cell
+    // prefetcher has just brought in (measured: L1 hit rate 47 -> 12 %, C2 15.7 -> 18.8 ms with
+    // __threadfence + a flag word).
+    uint4* q = reinterpret_cast<uint4*>(a.qout + (pos & a.cq_mask));
+    const unsigned tag = (pos >> a.cq_shift) + 1u;
     asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(q), "r"(__float_as_uint(r.px)),
-                 "r"(__float_as_uint(r.py)), "r"(__float_as_uint(r.pz)), "r"(~r.id) : "memory");
-    asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(q + 1), "r"(r.n + 1u), "r"(r.brick),
-                 "r"(r.pad0), "r"(r.pad1) : "memory");
+                 "r"(__float_as_uint(r.py)), "r"(__float_as_uint(r.pz)), "r"(tag) : "memory");
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(q + 1), "r"(r.id), "r"(r.n), "r"(r.brick),
+                 "r"(tag) : "memory");
   } else {
     a.qout[pos] = r;
   }
@@ -117,6 +119,7 @@ trace_kernel(const TraceArgs a) {
   unsigned n_samples = 0, n_attempts = 0, n_start = 0, budget = 0;
   unsigned pend = 0xffffffffu;    // INQ: claimed queue index whose record is not published yet
   bool term = false;              // INQ: this lane's particle terminated since the last count
+  unsigned spins = 0;             // INQ: polls of a warp with nothing to do
 
   for (;;) {
     if (INQ) {
@@ -197,20 +200,26 @@ trace_kernel(const TraceArgs a) {
         if (!active && exhausted && pend == 0xffffffffu) pend = base + __popc(want & ((1u << lane) - 1u));
       }
       uint4 r0 = make_uint4(0u, 0u, 0u, 0u), r1 = r0;
-      if (!active && pend < a.cq_cap) {                // (the "no claim" value is above every capacity)
-        r0 = ld_volatile_v4(reinterpret_cast<const uint4*>(a.qout + pend));
-        r1 = ld_volatile_v4(reinterpret_cast<const uint4*>(a.qout + pend) + 1);
+      const bool look = !active && pend != 0xffffffffu;
+      if (look) {
+        const uint4* q = reinterpret_cast<const uint4*>(a.qout + (pend & a.cq_mask));
+        r0 = ld_volatile_v4(q);
+        r1 = ld_volatile_v4(q + 1);
       }
-      if (r0.w != 0u && r1.x != 0u) {                  // both halves written (see emit_outgoing)
-        L.px = __uint_as_float(r0.x); L.py = __uint_as_float(r0.y); L.pz = __uint_as_float(r0.z); L.id = ~r0.w;
-        L.n = r1.x - 1u; my_brick = (int)r1.y;
-        if (INTEG == 1) { L.t = __uint_as_float(r1.z); L.h = __uint_as_float(r1.w); L.rejected = false; }
+      const unsigned tag = (pend >> a.cq_shift) + 1u;
+      if (look && r0.w == tag && r1.w == tag) {        // both halves written in this pass of the ring
+        L.px = __uint_as_float(r0.x); L.py = __uint_as_float(r0.y); L.pz = __uint_as_float(r0.z);
+        L.id = r1.x; L.n = r1.y; my_brick = (int)r1.z;
+        if (BRICK) {
+          st = a.bricks[my_brick];
+          if (!a.brick_fast) { st.fastx = 0u; st.fasty = 0u; st.fastz = 0u; }
+        }
         L.slot = min(a.cap, L.n / a.stride + 1u);
         L.rec_cd = a.stride - L.n % a.stride;
         L.stage0 = L.slot;
         n_samples = 0; n_attempts = 0; n_start = L.n; budget = a.seg_budget;
         cc.invalidate(); L.pf = 0xffffffffu;
-        pend = 0xffffffffu; active = true;
+        pend = 0xffffffffu; active = true; spins = 0;
       }
     }
     if (__all_sync(FULL, !active)) {
@@ -220,6 +229,10 @@ trace_kernel(const TraceArgs a) {
         if (lane == 0) dn = ld_volatile_u32(a.cq_done);
         dn = __shfl_sync(FULL, dn, 0);
         if (dn >= (unsigned)a.n && !__any_sync(FULL, term)) break;
+        // A warp that has nothing to do polls ~5 times per microsecond; 2^27 polls (half a minute) without the launch
+        // ending means a record was lost (it cannot be, see the ring's size in the host code): give
+        // up loudly instead of hanging the device.
+        if (++spins > (1u << 27)) { if (lane == 0) atomicExch(a.cq_error, 1u); break; }
         __nanosleep(200);
       }
       continue;

@@ -100,7 +100,7 @@ def test_argument_validation_without_a_gpu():
     assert L.streami_seed_shape(f3, f3, f3, f3, 0, 2, 2, 0, 0, NULL, NULL) == S.OK                  # no seeds: nothing to do
     assert L.streami_set_option(b"no_such_option", 1) == S.E_INVALID
     for name, v in (("segment_steps", 17), ("prefetch", 2), ("vertex_staging", 0), ("max_blocks_per_sm", 2),
-                    ("brick_round_steps", -1), ("presort", 0), ("cell_cache", 0), ("queue_steps", 96),
+                    ("brick_round_steps", -2), ("presort", 0), ("cell_cache", 0), ("queue_steps", 96),
                     ("streak_window", 12)):
         old = S.streami_get_option(name)
         S.streami_set_option(name, v)

@@ -201,6 +201,48 @@ def test_bricks_halo_miss_and_truncation(S, torch, oracle, wl):
     assert out["nrounds"] == 0 and list(out["status"]) == [1] * 5 and out["nlog"] == 0
 
 
+@pytest.mark.parametrize("nb,N,layout,q", [((2, 2, 2), 32, 5, 0), ((3, 2, 1), 31, 3, 0), ((2, 2, 2), 32, 5, 9),
+                                           ((1, 1, 1), 24, 5, 0), ((2, 2, 2), 32, 1, 40)])
+def test_bricks_one_launch_ring(S, torch, oracle, wl, nb, N, layout, q):
+    """Option brick_round_steps = -2: hand-offs (and, with queue_steps = q > 0, step budgets) go through
+    a device ring consumed by the same launch; no rounds.  Per-particle results and the number of
+    hand-offs equal the oracle's (A9: they do not depend on the round structure)."""
+    fld = wl.turb_field_cpu(N, 48, 1, 6)
+    n = 30011
+    seeds = wl.seeds_uniform(42, n, [N - 1.0] * 3)
+    seeds[3] = [-1, 2, 2]; seeds[4] = [N - 1.0] * 3
+    kw = dict(integrator=0, h=0.25, max_steps=400, vmin=1e-6, capacity=101, stride=4)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    arrays = [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nb, 1)]
+    f = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, 1, arrays, layout)
+    d_seeds = torch.from_numpy(seeds).cuda()
+    verts = torch.full((3, n, 101), float("nan"), dtype=torch.float32, device="cuda")
+    counts = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    steps = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    status = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    final = torch.zeros((3, n), dtype=torch.float32, device="cuda")
+    totals = torch.zeros(4, dtype=torch.int64, device="cuda")
+    prm = S.params(out_steps=steps, out_status=status, out_final=final, out_totals=totals, **kw)
+    S.streami_set_option("brick_round_steps", -2)
+    S.streami_set_option("queue_steps", q)
+    try:
+        nrounds, truncated = S.streami_brick_advect(f, d_seeds, prm, verts, counts)
+        torch.cuda.synchronize()
+    finally:
+        S.streami_set_option("brick_round_steps", 0)
+        S.streami_set_option("queue_steps", 0)
+    assert nrounds == 1 and not truncated
+    assert np.array_equal(status.cpu().numpy().astype(np.uint32), ref.status)
+    assert np.array_equal(steps.cpu().numpy().astype(np.uint32), ref.steps)
+    assert np.array_equal(counts.cpu().numpy().astype(np.uint32), ref.counts)
+    assert np.array_equal(final.cpu().numpy().view(np.uint32), ref.final.view(np.uint32))
+    assert np.array_equal(verts.cpu().numpy().view(np.uint32), ref.vertices.view(np.uint32))
+    assert np.array_equal(totals.cpu().numpy().astype(np.uint64), ref.totals)
+
+
 @pytest.mark.parametrize("k", [1, 7])
 def test_bricks_paper_step_rounds(S, torch, oracle, wl, k):
     """the paper's schedule (every particle re-queued after every RK step,
