@@ -52,6 +52,10 @@ WORKLOADS = {
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
                stride=128)),
+    # pathlines ("easy to implement within the framework"): streamlines through C4's time-sliced
+    # field, 1 Mi seeds uniform in the domain (never the reported headline)
+    "p4": dict(kind="path", n=1 << 20, prm=dict(integrator=0, h=0.05, max_steps=1000, vmin=1e-7, t0=0.0,
+               capacity=64, stride=16)),
     # the paper's other field type: a 128^3 turbulence grid re-expressed as 127^3 hexahedra
     # (PAPER.md:159), bins 127^3, RK4 (never the reported headline)
     "u1": dict(kind="mesh", N=128, M=128, kmax=32, n=1 << 18, nbins=(127, 127, 127), prm=dict(integrator=0, h=0.25,
@@ -72,6 +76,7 @@ DESCR = {
     "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
     "c4p": "C4 with the paper's hold-floor-slice time handling (comparison only)",
     "c2s": "C2 with an L2-resident 64^3 field (profiling aid only)",
+    "p4": "P4 pathlines through C4's double gyre (64 slices), 1,048,576 seeds, RK4 h=0.05, max 1,000",
     "u1": "U1 hexahedral mesh: 128^3 turbulence grid as 2,048,383 hexahedra, 262,144 seeds, RK4 h=0.25, max 500",
     "tiny": "tiny turbulence 48^3 (script self-check only)",
 }
@@ -159,6 +164,8 @@ def host_inputs(name, rank, need_field=True):
         return wl.abc_field(w["N"]), wl.seeds_uniform(shard_seed(rank), w["n"], [2 * np.pi] * 3)
     if w["kind"] == "gyre":
         return wl.double_gyre_field(), wl.rake_c4()
+    if w["kind"] == "path":
+        return wl.double_gyre_field(), wl.seeds_uniform(shard_seed(rank), w["n"], [2.0, 1.0, 1.0])
     seeds = wl.seeds_uniform(shard_seed(rank), w["n"], [w["N"] - 1.0] * 3)
     fld = None
     if need_field:
@@ -195,6 +202,12 @@ class Job:
             self.field = S.streami_field_create(fld.dims, fld.origin, fld.spacing, fld.nslices,
                                                 fld.slice_dt, self.data, layout)
             self.seeds_h = wl.rake_c4()
+        elif self.kind == "path":
+            fld = self.host_field = wl.double_gyre_field()
+            self.data = torch.from_numpy(fld.data).cuda()
+            self.field = S.streami_field_create(fld.dims, fld.origin, fld.spacing, fld.nslices,
+                                                fld.slice_dt, self.data, layout)
+            self.seeds_h = wl.seeds_uniform(shard_seed(rank), w["n"], [2.0, 1.0, 1.0])
         elif self.kind == "mesh":
             N = w["N"]
             fld, dev = wl.turb_field_cuda(N, w["M"], 1.0, w["kmax"], host=True)
@@ -314,7 +327,7 @@ class Job:
     def algorithmic_bytes(self, samples, stored):
         """useful gather bytes (8 vertices x 12 B per sample and slice) +
         12 B per stored vertex + per-particle fetch (12 B) and results (24 B)."""
-        per_sample = 192 if (self.kind == "gyre" and not self.w["prm"].get("time_mode")) else 96
+        per_sample = 192 if (self.kind in ("gyre", "path") and not self.w["prm"].get("time_mode")) else 96
         return samples * per_sample + stored * 12 + self.npart * 36
 
 
