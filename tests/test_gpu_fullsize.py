@@ -85,6 +85,20 @@ def test_c2_full_size_sampled(torch, bench, oracle):
           (st.mean().item(), st.median().item(), (job.steps_o == 2000).float().mean().item()))
 
 
+def test_p4_pathlines_full_size_sampled(torch, bench, oracle):
+    """P4 (bench.py --workload p4): 1,048,576 RK4 pathlines through C4's 64-slice double gyre with the
+    two-slice register copy of the cell; oracle on every 128th seed."""
+    job = bench.Job("p4", 0, 0)
+    fld = job.host_field
+    ids = np.arange(0, job.n, 128)
+    gpu = _gpu_outputs(job, torch, ids)
+    st = job.status_o
+    assert int(st.min()) >= 1 and int(st.max()) <= 3 and int(job.steps_o.max()) <= 1000
+    g = oracle.grid(fld.data, fld.dims, fld.origin, fld.spacing, fld.nslices, fld.slice_dt)
+    ref = oracle.streamlines(g, job.seeds_h[ids], oracle.params(**job.w["prm"]), "f32")
+    _compare(gpu, ref, "p4")
+
+
 def test_c2_parity_recording_first_200_vertices(torch, bench, oracle, wl):
     """C2 with the parity-run recording (capacity 201, stride 1): every one of the first 200
     vertices of every 256th particle, bit for bit, plus north_star's tolerance form."""
