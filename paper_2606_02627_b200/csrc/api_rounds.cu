@@ -55,11 +55,12 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
   while ((1ull << shift) < 2ull * n) ++shift;
   if (shift > 31) return STREAMI_E_INVALID;
   const size_t cap = (size_t)1 << shift;
-  char* ctr = nullptr; QRec* cq = nullptr; unsigned* perm = nullptr;
+  char* ctr = nullptr; QRec* cq = nullptr; unsigned* perm = nullptr; float4* seeds4 = nullptr;
   MortonSorter sorter{}; bool have_sorter = false;
   const bool sorting = options().presort && n >= 65536;
   auto cleanup = [&]() {
     if (ctr) cudaFreeAsync(ctr, st);
+    if (seeds4) cudaFreeAsync(seeds4, st);
     if (cq) cudaFreeAsync(cq, st);
     if (perm) cudaFreeAsync(perm, st);
     if (have_sorter) sorter.release();
@@ -78,12 +79,16 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
     have_sorter = true;
     rc = sorter.sort(f->g, seeds, 3, n, nullptr, perm);
     if (rc) { cleanup(); return rc; }
+    e = cudaMallocAsync((void**)&seeds4, sizeof(float4) * n, st);
+    if (e != cudaSuccess) { cleanup(); return check(e); }
+    rc = sorter.gather_seeds(seeds, perm, n, seeds4);
+    if (rc) { cleanup(); return rc; }
   }
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = 0; a.s = f->bricks[0];
   a.bricks = f->d_bricks; a.bm = f->bm; a.nbricks = (int)f->bricks.size();
   a.brick_fast = options().integer_accept;
-  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr;
+  a.seeds = seeds; a.seeds4 = seeds4; a.perm = seeds4 ? nullptr : perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr;
   a.next = (unsigned long long*)ctr; a.round = 0;
   a.seg_budget = options().queue_steps > 0 ? (unsigned)options().queue_steps : 0u;   // 0 = until the particle leaves its brick
   fill_integrator(a, params);
@@ -296,13 +301,16 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   cudaError_t e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
   if (e == cudaSuccess) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
   unsigned* perm = nullptr; MortonSorter sorter{}; bool have_sorter = false;
+  QRec* qs = nullptr;               // the round's work items in processing order (round 0: seeds as float4)
   const bool sorting = options().presort && n >= 65536;
   auto cleanup = [&]() {
     cudaFreeAsync(ctr, st); if (q[0]) cudaFreeAsync(q[0], st); if (q[1]) cudaFreeAsync(q[1], st);
+    if (qs) cudaFreeAsync(qs, st);
     if (perm) cudaFreeAsync(perm, st);
     if (have_sorter) sorter.release();
   };
   if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
+  if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&qs, sizeof(QRec) * n, st);
   if (e != cudaSuccess) { if (e != cudaSuccess && !q[0]) q[0] = nullptr; cleanup(); return check(e); }
   unsigned long long* d_next = (unsigned long long*)ctr;
   unsigned long long* d_logc = out_log_count ? out_log_count : (unsigned long long*)(ctr + 8);
@@ -346,12 +354,15 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   for (;;) {
     a.round = (int)round; a.nwork = nwork;
     a.qin = round ? q[round & 1] : nullptr; a.qout = q[(round + 1) & 1];
-    a.perm = nullptr;
+    a.perm = nullptr; a.seeds4 = nullptr;
     if (sorting && nwork >= 65536) {
+      // the round's work in processing order: sort, then gather the items themselves (sorter.cuh)
       rc = round ? sorter.sort(f->g, (const float*)q[round & 1], 8, nwork, nullptr, perm)
                  : sorter.sort(f->g, seeds, 3, nwork, nullptr, perm);
+      if (rc == STREAMI_OK)
+        rc = round ? sorter.gather_rec32(q[round & 1], perm, nwork, qs) : sorter.gather_seeds(seeds, perm, nwork, (float4*)qs);
       if (rc) { cleanup(); return rc; }
-      a.perm = perm;
+      if (round) a.qin = qs; else a.seeds4 = (const float4*)qs;
     }
     a.rc_this = nullptr; a.rc_next = nullptr;
     if (round == 0) {

@@ -165,10 +165,11 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   }
   unsigned long long* next = (unsigned long long*)ctr;
   unsigned* qcount = (unsigned*)(ctr + 8);
-  unsigned* perm = nullptr; QRec* q[2] = {nullptr, nullptr};
+  unsigned* perm = nullptr; QRec* q[2] = {nullptr, nullptr}; float4* seeds4 = nullptr;
   MortonSorter sorter{}; bool have_sorter = false;
   auto cleanup = [&]() {
     cudaFreeAsync(ctr, st);
+    if (seeds4) cudaFreeAsync(seeds4, st);
     if (cq) cudaFreeAsync(cq, st);
     if (perm) cudaFreeAsync(perm, st);
     if (q[0]) cudaFreeAsync(q[0], st);
@@ -186,12 +187,16 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
     have_sorter = true;
     rc = sorter.sort(f->g, seeds, 3, n, nullptr, perm);
     if (rc) { cleanup(); return rc; }
+    e = cudaMallocAsync((void**)&seeds4, sizeof(float4) * n, st);
+    if (e != cudaSuccess) { cleanup(); return check(e); }
+    rc = sorter.gather_seeds(seeds, perm, n, seeds4);
+    if (rc) { cleanup(); return rc; }
   }
 
   TraceArgs a{};
   a.g = f->g; a.g.time_mode = params->time_mode; a.s = launch_store(f);
   a.bricks = nullptr; a.nbricks = 0;
-  a.seeds = seeds; a.perm = perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr; a.next = next; a.round = 0;
+  a.seeds = seeds; a.seeds4 = seeds4; a.perm = seeds4 ? nullptr : perm; a.qin = nullptr; a.nwork = n; a.nwork_dev = nullptr; a.next = next; a.round = 0;
   a.seg_budget = K;
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
@@ -228,7 +233,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
       if (e != cudaSuccess) break;
       rc = sorter.sort(f->g, (const float*)q[in], 8, 0, qcount + in, perm);
       if (rc) { cleanup(); return rc; }
-      a.seeds = nullptr; a.qin = q[in]; a.nwork_dev = qcount + in; a.qout = q[out]; a.qout_count = qcount + out;
+      a.seeds = nullptr; a.seeds4 = nullptr; a.perm = perm; a.qin = q[in]; a.nwork_dev = qcount + in; a.qout = q[out]; a.qout_count = qcount + out;
       a.round = (int)r;
       timing_begin(st);
       k<<<grid, block, 0, st>>>(a);

@@ -110,4 +110,27 @@ static __global__ void presort_scatter_kernel(const unsigned* __restrict__ keys,
   }
 }
 
+// The work items in processing order, so that a refilling lane reads ONE record at its work index
+// instead of perm[w] and then the item (one dependent L2 round trip less per refill, with the whole
+// warp waiting).  Seeds become {x, y, z, id}; 32-byte queue records are copied as they are.
+static __global__ void gather_seeds_kernel(const float* __restrict__ seeds, const unsigned* __restrict__ perm,
+                                           unsigned long long n, float4* __restrict__ out) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; i < n; i += step) {
+    const unsigned id = perm[i];
+    out[i] = make_float4(seeds[3ull * id], seeds[3ull * id + 1], seeds[3ull * id + 2], __uint_as_float(id));
+  }
+}
+
+static __global__ void gather_rec32_kernel(const uint4* __restrict__ in, const unsigned* __restrict__ perm,
+                                           unsigned long long n, uint4* __restrict__ out) {
+  unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; i < n; i += step) {
+    const unsigned long long src = perm[i];
+    out[2 * i] = in[2 * src]; out[2 * i + 1] = in[2 * src + 1];
+  }
+}
+
 }  // namespace streami

@@ -45,6 +45,20 @@ struct MortonSorter {
     launch_counter() += 4;
     return check(cudaGetLastError());
   }
+
+  // out[i] = {seed perm[i], perm[i]} / the 32-byte record perm[i]: the work items in processing order
+  int gather_seeds(const float* seeds, const unsigned* perm, size_t n, float4* out) {
+    unsigned blocks = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)num_sms() * 16);
+    gather_seeds_kernel<<<blocks ? blocks : 1, 256, 0, st>>>(seeds, perm, n, out);
+    launch_counter()++;
+    return check(cudaGetLastError());
+  }
+  int gather_rec32(const void* in, const unsigned* perm, size_t n, void* out) {
+    unsigned blocks = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)num_sms() * 16);
+    gather_rec32_kernel<<<blocks ? blocks : 1, 256, 0, st>>>((const uint4*)in, perm, n, (uint4*)out);
+    launch_counter()++;
+    return check(cudaGetLastError());
+  }
 };
 
 }  // namespace streami

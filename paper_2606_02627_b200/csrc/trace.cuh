@@ -27,6 +27,7 @@ struct TraceArgs {
   const Store* bricks; BrickMap bm; int nbricks;   // brick mode
   // work
   const float* seeds;              // [n][3]
+  const float4* seeds4;            // optional: the seeds in processing order as {x, y, z, id}; perm is then unused
   const unsigned* perm;            // optional processing order of the work items (Morton sort), or NULL
   const QRec* qin;                 // work = queue records (brick rounds >= 1, segments >= 1), else seeds
   unsigned long long nwork;

@@ -151,8 +151,13 @@ trace_kernel(const TraceArgs a) {
             L.stage0 = L.slot;
             fresh = false;
           } else {
-            L.id = src;
-            L.px = a.seeds[3ull * L.id]; L.py = a.seeds[3ull * L.id + 1]; L.pz = a.seeds[3ull * L.id + 2];
+            if (a.seeds4) {
+              const float4 s4 = __ldg(a.seeds4 + w);
+              L.id = __float_as_uint(s4.w); L.px = s4.x; L.py = s4.y; L.pz = s4.z;
+            } else {
+              L.id = src;
+              L.px = a.seeds[3ull * L.id]; L.py = a.seeds[3ull * L.id + 1]; L.pz = a.seeds[3ull * L.id + 2];
+            }
             L.n = 0; L.slot = 0; L.rec_cd = 1; L.stage0 = 0;
             if (INTEG == 1) { L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false; }
           }
