@@ -42,6 +42,7 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
   QRec r; r.px = L.px; r.py = L.py; r.pz = L.pz; r.id = L.id; r.n = L.n; r.brick = (unsigned)dest;
   r.pad0 = 0; r.pad1 = 0;
   if (INTEG == 1) { r.pad0 = __float_as_uint(L.t); r.pad1 = __float_as_uint(L.h); }
+  else { r.pad0 = L.slot; r.pad1 = L.rec_cd; }     // RK4: the writer's position, so that the pick-up needs no division
   if (INQ) {
     // Ring slot pos & mask, two self-validating halves, each ONE aligned 16-byte store: both carry
     // the tag (pos >> shift) + 1 of this pass through the ring (the memory starts zeroed, tags start
@@ -145,9 +146,13 @@ trace_kernel(const TraceArgs a) {
           if (a.qin) {                                        // a continued or handed-over particle
             const QRec r = a.qin[src];
             L.px = r.px; L.py = r.py; L.pz = r.pz; L.id = r.id; L.n = r.n; my_brick = (int)r.brick;
-            if (INTEG == 1) { L.t = __uint_as_float(r.pad0); L.h = __uint_as_float(r.pad1); L.rejected = false; }
-            L.slot = min(a.cap, L.n / a.stride + 1u);
-            L.rec_cd = a.stride - L.n % a.stride;
+            if (INTEG == 1) {
+              L.t = __uint_as_float(r.pad0); L.h = __uint_as_float(r.pad1); L.rejected = false;
+              L.slot = min(a.cap, L.n / a.stride + 1u);
+              L.rec_cd = a.stride - L.n % a.stride;
+            } else {                               // = min(cap, n / stride + 1) and stride - n % stride
+              L.slot = r.pad0; L.rec_cd = r.pad1;
+            }
             L.stage0 = L.slot;
             fresh = false;
           } else {
