@@ -95,7 +95,7 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
   a.qout = cq; a.qout_count = (unsigned*)(ctr + 8); a.cq_head = (unsigned*)(ctr + 12);
-  a.cq_done = (unsigned*)(ctr + 16); a.cq_error = (unsigned*)(ctr + 20);
+  a.cq_done = (unsigned*)(ctr + 16); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 20);
   a.cq_mask = (unsigned)(cap - 1); a.cq_shift = shift;
   int grid = 0;
   rc = trace_grid(k, n, block, &grid);
@@ -351,9 +351,52 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   unsigned round = 0;
   unsigned long long nwork = n;
   std::vector<unsigned> h_buf(1 + nb);
+  // Automatic rounds only (nobody observes A9's round structure): once a round has less than n/16 particles
+  // left, the rest -- on C3 some twenty rounds of stragglers that changed brick often, each a launch that
+  // waits for its slowest particle -- is finished by ONE launch that consumes its own hand-off ring
+  // (trace_kernel.cuh, INQ).
+  const bool ring_finish = options().brick_round_steps == 0 && !out_round_counts && !out_handoff_log &&
+                           params->integrator == 0 && cache;
   for (;;) {
     a.round = (int)round; a.nwork = nwork;
     a.qin = round ? q[round & 1] : nullptr; a.qout = q[(round + 1) & 1];
+    if (ring_finish && round > 0 && nwork * 16ull <= (unsigned long long)n) {
+      unsigned shift = 10;
+      while ((1ull << shift) < 2ull * nwork) ++shift;
+      const size_t cap = (size_t)1 << shift;
+      char* rctr = nullptr; QRec* ring = nullptr;       // [0] ring tail, [4] head, [8] done, [12] error
+      e = cudaMallocAsync((void**)&rctr, 16, st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(rctr, 0, 16, st);
+      if (e == cudaSuccess) e = cudaMallocAsync((void**)&ring, sizeof(QRec) * cap, st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(ring, 0, sizeof(QRec) * cap, st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(d_next, 0, sizeof(unsigned long long), st);
+      unsigned err = 0;
+      if (e == cudaSuccess) {
+        TraceKernel kr = pick_trace_kernel_inq(f->layout, unit_geometry(f->g), true);
+        a.perm = nullptr; a.seeds4 = nullptr; a.rc_this = nullptr; a.rc_next = nullptr;
+        a.seg_budget = 0;                               // until the particle leaves its brick
+        a.qout = ring; a.qout_count = (unsigned*)rctr; a.cq_head = (unsigned*)(rctr + 4);
+        a.cq_done = (unsigned*)(rctr + 8); a.cq_error = (unsigned*)(rctr + 12); a.cq_total = (unsigned)nwork;
+        a.cq_mask = (unsigned)(cap - 1); a.cq_shift = shift;
+        int grid = 0;
+        rc = trace_grid(kr, nwork, block, &grid);
+        if (rc == STREAMI_OK) {
+          timing_begin(st);
+          kr<<<grid, block, 0, st>>>(a);
+          timing_end(st);
+          launch_counter()++;
+          e = cudaGetLastError();
+          if (e == cudaSuccess) e = cudaMemcpyAsync(&err, rctr + 12, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+          if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        }
+      }
+      if (rctr) cudaFreeAsync(rctr, st);
+      if (ring) cudaFreeAsync(ring, st);
+      if (rc) { cleanup(); return rc; }
+      if (e == cudaSuccess && err) { cleanup(); return STREAMI_E_CUDA; }
+      round++;
+      break;
+    }
     a.perm = nullptr; a.seeds4 = nullptr;
     if (sorting && nwork >= 65536) {
       // the round's work in processing order: sort, then gather the items themselves (sorter.cuh)

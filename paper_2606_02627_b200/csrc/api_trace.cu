@@ -204,7 +204,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
   if (Q) {
     a.seg_budget = Q; a.qout = cq; a.qout_count = qcount; a.cq_head = qcount + 1;
-    a.cq_done = (unsigned*)(ctr + 16); a.cq_error = (unsigned*)(ctr + 20);
+    a.cq_done = (unsigned*)(ctr + 16); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 20);
     a.cq_mask = (unsigned)(qcap - 1ull); a.cq_shift = qshift;
   }
   timing_begin(st);

@@ -51,6 +51,7 @@ struct TraceArgs {
   // in-kernel continuation queue (trace_kernel.cuh, INQ): qout, zero-initialised, is consumed by the same launch
   unsigned* cq_head;               // next index to claim
   unsigned* cq_done;               // particles terminated so far
+  unsigned cq_total;               // the launch ends when cq_done reaches this (the particles it was given)
   unsigned* cq_error;              // set if a warp gave up waiting (never, unless a record was lost)
   unsigned cq_mask, cq_shift;      // ring of 2^cq_shift records
   unsigned* rc_this;               // round_counts row of this round (round 0 only), or NULL

@@ -90,7 +90,7 @@ template <> struct TraceCache<true> { typedef CellCacheT type; };
 // dry keeps its SM waiting ~2,000 latency-bound steps (C2: 2.6 of 15.6 ms).  A claim never blocks:
 // the lane keeps its index and looks again in the next iteration, so a warp whose other lanes hold
 // particles (one of which may be the producer) keeps stepping.  The launch ends when every
-// particle has terminated (`cq_done` == n).
+// particle has terminated (`cq_done` == `cq_total`).
 __device__ __forceinline__ unsigned ld_volatile_u32(const unsigned* p) {
   unsigned v;
   asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -238,7 +238,7 @@ trace_kernel(const TraceArgs a) {
         unsigned dn = 0;
         if (lane == 0) dn = ld_volatile_u32(a.cq_done);
         dn = __shfl_sync(FULL, dn, 0);
-        if (dn >= (unsigned)a.n && !__any_sync(FULL, term)) break;
+        if (dn >= a.cq_total && !__any_sync(FULL, term)) break;
         // A warp that has nothing to do polls ~5 times per microsecond; 2^27 polls (half a minute) without the launch
         // ending means a record was lost (it cannot be, see the ring's size in the host code): give
         // up loudly instead of hanging the device.
