@@ -253,6 +253,15 @@ def test_p6_linear_in_time_exact(oracle, precision):
     prm = oracle.params(0, h=0.25, max_steps=8, vmin=0.0, t0=20.0)
     r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
     assert list(r.final[:, 0]) == [2 * (a[c] + 16 * b[c]) for c in range(3)]
+    # before the first slice (t < 0) the field is frozen at slice 0 (A3: s = max(t q, 0)): t0 = -3,
+    # 8 steps of 0.25 end at t = -1, so every stage sees v = a exactly
+    prm = oracle.params(0, h=0.25, max_steps=8, vmin=0.0, t0=-3.0)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
+    assert list(r.final[:, 0]) == [2 * a[c] for c in range(3)]
+    # ... and a trace that crosses t = 0 integrates a for t < 0 and a + b t after: t0 = -1, 16 steps
+    prm = oracle.params(0, h=0.25, max_steps=16, vmin=0.0, t0=-1.0)
+    r = oracle.streamlines(g, np.zeros((1, 3)), prm, precision)
+    assert list(r.final[:, 0]) == [a[c] * 4 + b[c] * 3 * 3 / 2 for c in range(3)]
 
 
 def test_p6_hold_floor_slice_mode(oracle):
@@ -449,24 +458,48 @@ def test_p8_controller_paths(oracle):
 # ------------------------------------------------------------------------------------------
 # P9 + P10: bricks (A9) == monolithic, bit for bit; queue invariants.
 # ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("integrator", [0, 1])
 @pytest.mark.parametrize("nb,N", [((2, 2, 2), 32), ((3, 2, 1), 31)])
-def test_p9_bricks_equal_monolithic(oracle, wl, nb, N):
+def test_p9_bricks_equal_monolithic(oracle, wl, nb, N, integrator):
+    """A9: a brick serves a sample bit for bit like the undivided field, so the brick-wise trace must
+    equal the monolithic one for RK4 AND for DP5(4), whose hand-off carries t and h and recomputes
+    the FSAL k1 in the receiving brick (this was pinned only through the GPU)."""
     f = wl.turb_field_cpu(N, 48, 1, 6, seed=2606)
     n = 3000
     seeds = wl.seeds_uniform(42, n, [N - 1] * 3)
-    prm = oracle.params(0, h=0.25, max_steps=400, vmin=1e-6, capacity=401)
+    if integrator == 0:
+        prm = oracle.params(0, h=0.25, max_steps=400, vmin=1e-6, capacity=401)
+    else:
+        prm = oracle.params(1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=400,
+                            vmin=1e-6, capacity=401)
     mono = oracle.streamlines(oracle.grid(f.data, f.dims, f.origin, f.spacing), seeds, prm, "f32")
     boxes = wl.brick_boxes(f.dims, nb, 1)
     arrays = wl.cut_bricks(f, nb, 1)
     bricks = [oracle.grid(a, None, f.origin, f.spacing, gdims=f.dims, lo=lo, hi=hi)
               for a, (lo, hi) in zip(arrays, boxes)]
     br = oracle.brick_advect(bricks, nb, seeds, prm, "f32")
-    assert np.count_nonzero(br.status == oracle.HALO_MISS) == 0
-    assert np.array_equal(br.status, mono.status) and np.array_equal(br.steps, mono.steps)
-    assert np.array_equal(br.counts, mono.counts)
-    assert np.array_equal(br.vertices, mono.vertices, equal_nan=True)
-    assert np.array_equal(br.final, mono.final)
-    assert np.array_equal(br.totals[:3], mono.totals[:3])
+    # P9 compares every particle whose status is not HALO_MISS.  RK4 at h = 0.25 never leaves the
+    # 1-cell halo (asserted); DP5(4) with h up to 1 does for a few fast particles (a stage point more
+    # than one cell beyond an ownership face), which is A9's defined behaviour, not an error.
+    ok = br.status != oracle.HALO_MISS
+    if integrator == 0:
+        assert ok.all()
+    else:
+        assert ok.mean() > 0.9 and not ok.all()
+    assert np.array_equal(br.status[ok], mono.status[ok]) and np.array_equal(br.steps[ok], mono.steps[ok])
+    assert np.array_equal(br.counts[ok], mono.counts[ok])
+    assert np.array_equal(br.vertices[:, ok], mono.vertices[:, ok], equal_nan=True)
+    assert np.array_equal(br.final[:, ok], mono.final[:, ok])
+    if ok.all():
+        assert np.array_equal(br.totals[:3], mono.totals[:3])
+    if integrator == 1:
+        assert mono.totals[0] > mono.totals[1]              # rejections occurred: the carried h / flag matter
+        assert br.totals[3] > 1000                          # and many DP5(4) particles did change brick
+        # a HALO_MISS particle followed the monolithic trajectory up to the step it was dropped at
+        bad = np.flatnonzero(~ok)
+        for i in bad[:20]:
+            k = int(br.counts[i])
+            assert k >= 1 and np.array_equal(br.vertices[:, i, :k], mono.vertices[:, i, :k])
     # P10 invariants
     assert br.nrounds >= 2 and br.totals[3] == br.nlog == len(br.log)
     B = [N // nb[a] for a in range(3)]
