@@ -1,7 +1,10 @@
-"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+"""Parity at BASELINE.json's FULL sizes.
 
-The CUDA path runs the whole workload (bench.Job: same field generator, seeds, parameters, layout
-and options as the timed run); the oracle runs a strided sample of the particles one by one on
+C2, C4, C5, P4 and `test_c3_full_size_bench_config` run exactly the call bench.py times
+(`bench.Job.step_device`: same field generator, seeds, parameters, layout and options).
+`test_c3_full_size_sampled` additionally asks for the round table and the hand-off log, which
+switches streami_brick_advect to A9's observable rounds (no step budget, no ring finish): it checks
+the queue outputs, not the timed configuration.  The oracle runs a strided sample of the particles one by one on
 the SAME field bytes (copied from the device) and every per-particle output of those ids is
 compared bit for bit.  Properties that hold at any size (P10 invariants) are checked on all ids.
 Tolerance: the formula sheet makes both sides execute the same IEEE operations, so the bar here is
@@ -164,6 +167,44 @@ def test_c3_full_size_sampled(torch, bench, oracle, wl):
     assert rc[0].sum() == n, "Q_0 holds every (inside) seed once"
     assert rc[1:nrounds + 1].sum() == nlog, "total hand-offs = sum of later queue sizes"
     assert int(job.totals_o[3].item()) == nlog
+
+
+def test_c3_full_size_bench_config(torch, bench, oracle, wl):
+    """C3 exactly as bench.py times it: `Job.step_device`, i.e. no round table and
+    no log, so the library runs its automatic schedule -- 256-step budget per round, Morton sort +
+    gather of every round's work (n >= 65,536), and the stragglers finished through the in-kernel
+    hand-off ring.  Every per-particle output of every 256th id is compared with the oracle's brick
+    rounds (A9) bit for bit; totals[0:3] and the hand-off count are schedule-independent and are
+    compared with `test_c3_full_size_sampled`'s observable-rounds run of the same seeds."""
+    import paper_2606_02627_b200 as S
+    job = bench.Job("c3", 0, 0)
+    fld = job.host_field
+    n = job.n
+    ids = np.arange(0, n, 256)
+    gpu = _gpu_outputs(job, torch, ids)                  # = job.step_device(): the timed call
+    tot_auto = job.totals_o.cpu().numpy().copy()
+    _invariants(job, torch, 4000, 256, 512)
+    assert int((job.status_o == 4).sum().item()) == 0, "HALO_MISS must not occur in C3 (Q14)"
+    boxes = wl.brick_boxes(fld.dims, (2, 2, 2), 1)
+    cut = wl.cut_bricks(fld, (2, 2, 2), 1)
+    bricks = [oracle.grid(c, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for c, (lo, hi) in zip(cut, boxes)]
+    ref = oracle.brick_advect(bricks, (2, 2, 2), job.seeds_h[ids], oracle.params(**job.w["prm"]), "f32")
+    _compare(gpu, ref, "c3 bench config")
+    # all particles: the automatic schedule and A9's rounds give the same per-particle results and totals
+    auto = dict(counts=job.counts.clone(), steps=job.steps_o.clone(), status=job.status_o.clone(),
+                final=job.final_o.clone())
+    logc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    rcounts = torch.zeros((256, 8), dtype=torch.int32, device="cuda")
+    job.counts.zero_(); job.steps_o.zero_(); job.status_o.zero_(); job.final_o.zero_()
+    S.streami_brick_advect(job.field, job.seeds, job.prm, job.verts, job.counts, rcounts, None, logc)
+    torch.cuda.synchronize()
+    for k, t in (("counts", job.counts), ("steps", job.steps_o), ("status", job.status_o)):
+        assert bool((auto[k] == t).all()), "c3 automatic vs A9 rounds: " + k
+    assert bool((auto["final"].view(torch.int32) == job.final_o.view(torch.int32)).all())
+    tot_a9 = job.totals_o.cpu().numpy()
+    assert np.array_equal(tot_auto[:3], tot_a9[:3]), "attempts / accepted / samples"
+    assert int(tot_auto[3]) == int(tot_a9[3]) == int(logc.item()), "hand-off count"
 
 
 def test_c4_full_size_sampled(torch, bench, oracle):
