@@ -51,7 +51,10 @@ WORKLOADS = {
     "c4p": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6, time_mode=1)),
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
-               stride=128)),
+               stride=128),
+               # 137 GB of CELL records: more than the half of the free memory AUTO allows itself, so the
+               # caller asks for it (streami.h: STREAMI_LAYOUT_CELL)
+               layout=4),
     # pathlines ("easy to implement within the framework"): streamlines through C4's time-sliced
     # field, 1 Mi seeds uniform in the domain (never the reported headline)
     "p4": dict(kind="path", n=1 << 20, prm=dict(integrator=0, h=0.05, max_steps=1000, vmin=1e-7, t0=0.0,
@@ -189,6 +192,8 @@ class Job:
         import paper_2606_02627_b200 as S
         self.S, self.torch, self.np, self.name = S, torch, np, name
         w = self.w = WORKLOADS[name]
+        if layout == 0:
+            layout = w.get("layout", 0)
         self.kind = w["kind"]
         self.host_field = None
         if self.kind == "abc":

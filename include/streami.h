@@ -54,9 +54,14 @@ extern "C" {
 #define STREAMI_HALO_MISS      4u  /* bricks only: a stage point left the brick's stored box */
 
 /* field layouts (layout_hint of streami_field_create*, reported by streami_field_info) */
-#define STREAMI_LAYOUT_AUTO    0   /* library chooses: XYQUAD for a steady field when its
-                                      64 B per vertex fit half the free device memory, else XPAIR; falls back
-                                      to a smaller layout instead of failing with NOMEM */
+#define STREAMI_LAYOUT_AUTO    0   /* library chooses the FASTEST layout whose library-owned copy fits HALF of the
+                                      device memory that is free at create time: steady
+                                      fields CELL (10.7x the packed size), else XYQUAD (5.3x), else XPAIR (2.7x);
+                                      unsteady fields XPAIR; falls back to the next smaller layout, in the end to
+                                      the caller's array in place, instead of failing with NOMEM.  The copy is
+                                      the price of speed: streami_field_info reports the layout chosen and the
+                                      bytes it took.  A caller that cannot spare the memory passes PACKED3 (no
+                                      copy at all) or FLOAT4 (1.3x) explicitly. */
 #define STREAMI_LAYOUT_PACKED3 1   /* use the caller's packed float3 array in place (the paper's layout) */
 #define STREAMI_LAYOUT_FLOAT4  2   /* library-owned copy padded to 16 B per vertex */
 #define STREAMI_LAYOUT_XPAIR   3   /* library-owned copy, 32 B per vertex: V[x] and V[x+1] - V[x]: one
@@ -64,7 +69,7 @@ extern "C" {
 #define STREAMI_LAYOUT_XYQUAD  5   /* library-owned copy, 64 B per vertex: the XPAIR rows (x, y) and (x, y+1):
                                       a cell is two aligned 64-byte pieces (4x the packed size) */
 #define STREAMI_LAYOUT_CELL    4   /* library-owned copy, 128 B per CELL: its 8 corner vertices in one
-                                      aligned L2 line (8x the packed size) */
+                                      aligned L2 line (10.7x the packed size) */
 
 typedef struct streami_field_s* streami_field;   /* opaque host-side handle (D2/D3) */
 

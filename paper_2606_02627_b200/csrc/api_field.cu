@@ -149,14 +149,18 @@ static int fill_geom(Geom& g, const int dims[3], const float origin[3], const fl
   return STREAMI_OK;
 }
 
-// AUTO: a steady field gets XYQUAD -- its 64-byte pieces use both halves of
-// every DRAM fetch and half as many L1 lines per cell (C5 1.21 -> 0.95 s, C2 16.6 -> 16.1 ms, and
-// no loss on fields that fit L2) -- provided its 64 B per vertex fit comfortably; otherwise, and
-// for unsteady fields (two slices per sample: C4 249 vs 264 ms), XPAIR.
-static int auto_layout(unsigned long long nvert, int nslices) {
+// AUTO: the fastest layout whose library-owned copy fits HALF of the free device
+// memory (the caller still has outputs to allocate).  Steady fields: CELL (128 B per cell, one L2 line
+// per cell: C2 15.6 -> 15.2 ms, C3 149.6 -> 139.3 ms, C5 939 -> 741 ms against XYQUAD), else XYQUAD
+// (64 B per vertex), else XPAIR (32 B per vertex).  Unsteady fields (two slices per sample: C4 249 vs
+// 264 ms on XYQUAD): XPAIR.  A caller that cannot spare the memory passes PACKED3 (no copy) or FLOAT4.
+static int auto_layout(unsigned long long nvert, unsigned long long ncell, int nslices) {
   if (nslices == 1) {
     size_t free_b = 0, total_b = 0;
-    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && 64ull * nvert <= free_b / 2) return LAYOUT_XYQUAD;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+      if (128ull * ncell <= free_b / 2) return LAYOUT_CELL;
+      if (64ull * nvert <= free_b / 2) return LAYOUT_XYQUAD;
+    }
     cudaGetLastError();
   }
   return LAYOUT_XPAIR;
@@ -214,9 +218,13 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   s.slice_stride = (unsigned long long)dims[0] * dims[1] * dims[2];
   void* data = nullptr; size_t bytes = 0;
   const bool automatic = layout == 0;
-  if (automatic) layout = auto_layout(s.slice_stride, nslices);
+  if (automatic) layout = auto_layout(s.slice_stride, (unsigned long long)(dims[0] - 1) * (dims[1] - 1) * (dims[2] - 1), nslices);
   rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
-  if (rc == STREAMI_E_NOMEM && automatic && layout != LAYOUT_XPAIR) {     // AUTO never fails for its own ambition
+  if (rc == STREAMI_E_NOMEM && automatic && layout == LAYOUT_CELL) {      // AUTO never fails for its own ambition
+    layout = LAYOUT_XYQUAD;
+    rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
+  }
+  if (rc == STREAMI_E_NOMEM && automatic && layout != LAYOUT_XPAIR) {
     layout = LAYOUT_XPAIR;
     rc = repack(dev_ptr, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2], (unsigned)nslices, layout, &data, &bytes);
   }
@@ -248,7 +256,8 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
   int layout = pick_layout(layout_hint);
   if (layout < 0 || ghost_cells < 1) return STREAMI_E_INVALID;
   if (layout == 0) {       // one layout for all bricks (one kernel serves them): decided on the whole grid
-    layout = auto_layout((unsigned long long)global_dims[0] * global_dims[1] * global_dims[2], 1);
+    const unsigned long long nv = (unsigned long long)global_dims[0] * global_dims[1] * global_dims[2];
+    layout = auto_layout(nv, nv, 1);     // the bricks' cells (ghost layers included) are about as many as the vertices
   }
   for (int a = 0; a < 3; ++a)
     if (brick_grid[a] < 1 || brick_grid[a] > global_dims[a] - 1) return STREAMI_E_INVALID;

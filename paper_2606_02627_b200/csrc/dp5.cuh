@@ -113,7 +113,7 @@ __device__ __forceinline__ unsigned dp5_attempt(const TraceArgs& a, const Store&
   if (accept) {
     L.px = nx; L.py = ny; L.pz = nz; L.k1x = k7x; L.k1y = k7y; L.k1z = k7z;   // FSAL
     L.t = t + h; L.n++;
-    record_vertex(a, L);
+    record_vertex<true, DP5_THREADS>(a, L);
     if (L.rejected) fac = fminf(fac, 1.0f);
     L.h = fminf(fmaxf(h * fac, a.hmin), a.hmax);
     L.rejected = false;

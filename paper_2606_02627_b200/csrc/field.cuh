@@ -76,6 +76,19 @@ __device__ __forceinline__ void ldg_rec32(const char* p, float* o) {
   (void)p6; (void)p7;
 }
 
+// The same load keeping all 8 floats (LAYOUT_CELL: 24 consecutive floats = 3 loads).
+template <bool NA>
+__device__ __forceinline__ void ldg8(const char* p, float* o) {
+  if (NA)
+    asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(o[6]), "=f"(o[7])
+                 : "l"(p));
+  else
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(o[6]), "=f"(o[7])
+                 : "l"(p));
+}
+
 // ---- loads of the 8 cell vertices as 4 rows of 6 floats --------------------------------------
 // V[row*6 + k], row = dz*2 + dy; k: {V[x].xyz, V[x+1].xyz} or, for the DIFF layouts, the record order.
 template <int LAYOUT> struct CellLoad;
@@ -103,16 +116,16 @@ template <> struct CellLoad<LAYOUT_XPAIR> {
   }
 };
 
-// LAYOUT_CELL: one aligned 128-byte record per CELL = the four XPAIR rows of that cell back to
-// back, i.e. all 8 corner vertices in ONE L2 line / one contiguous DRAM access.  Random 32-byte
-// sector gathers top out near 1.7 TB/s on B200 and contiguous 128-byte ones near 5.4 TB/s
-// (DESIGN.md section 6), which is what this layout buys with 8x the memory.
+// LAYOUT_CELL: one aligned 128-byte record per CELL: the four DIFF rows {Vx, Vy, Dx, Dy, Vz, Dz} of
+// that cell (row = dz*2 + dy) as 24 consecutive floats, then 32 bytes of padding.  All 8 corner
+// vertices sit in ONE 128-byte L2 line: three 256-bit loads whose misses the L1 merges into ~1.4 L2
+// requests per cell (ncu on C5), where XYQUAD's two 64-byte pieces make 4.
 template <> struct CellLoad<LAYOUT_CELL> {
   template <bool NA>
   static __device__ __forceinline__ void cell(const void* data, unsigned long long c, float* V) {
     const char* p = reinterpret_cast<const char*>(data) + 128ull * c;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) ldg_rec32<NA>(p + 32 * r, V + 6 * r);
+    for (int r = 0; r < 3; ++r) ldg8<NA>(p + 32 * r, V + 8 * r);
   }
 };
 
@@ -433,7 +446,7 @@ __device__ __forceinline__ void prefetch_cell32(const Store& s, unsigned v, unsi
   if constexpr (LAYOUT == LAYOUT_CELL) {
     const char* p = reinterpret_cast<const char*>(s.data) + 128ull * v;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) prefetch_sector(p + 32 * r, smem_addr);
+    for (int r = 0; r < 3; ++r) prefetch_sector(p + 32 * r, smem_addr);
   } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
     const char* p = reinterpret_cast<const char*>(s.data);
     prefetch_sector(p + 64ull * v, smem_addr);

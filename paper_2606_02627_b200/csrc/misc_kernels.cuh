@@ -57,9 +57,8 @@ static __global__ void repack_xyquad_kernel(const float* __restrict__ src, float
   }
 }
 
-// CELL record c = the four XPAIR rows (dz*2+dy) of cell c back to back: 128 bytes, 8 corners.
-// One thread per (cell, row): 6 source floats in, 32 bytes out; consecutive threads write
-// consecutive 32-byte pieces.
+// CELL record c = the four DIFF rows (dz*2+dy) of cell c as 24 consecutive floats {Vx, Vy, Dx, Dy, Vz, Dz} x 4,
+// then 32 bytes of zero padding: 128 bytes, 8 corners, one L2 line (field.cuh).  One thread per (cell, row).
 static __global__ void repack_cell_kernel(const float* __restrict__ src, float4* __restrict__ dst,
                                           unsigned nx, unsigned ny, unsigned nz, unsigned nslices) {
   const unsigned cx = nx - 1, cy = ny - 1, cz = nz - 1;
@@ -67,16 +66,21 @@ static __global__ void repack_cell_kernel(const float* __restrict__ src, float4*
   const unsigned long long total = 4ull * per_slice * nslices;
   unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  float2* out = reinterpret_cast<float2*>(dst);
   for (; t < total; t += step) {
     const unsigned r = (unsigned)(t & 3ull);
     unsigned long long c = t >> 2;
+    const unsigned long long rec = c;
     const unsigned sl = (unsigned)(c / per_slice);
     c -= (unsigned long long)sl * per_slice;
     const unsigned ix = (unsigned)(c % cx), iy = (unsigned)((c / cx) % cy), iz = (unsigned)(c / ((unsigned long long)cx * cy));
     const unsigned long long v = (((unsigned long long)sl * nz + iz + (r >> 1)) * ny + iy + (r & 1u)) * nx + ix;
     const float* p = src + 3ull * v;
-    dst[2 * t] = make_float4(p[0], p[1], p[3] - p[0], p[4] - p[1]);
-    dst[2 * t + 1] = make_float4(p[2], p[5] - p[2], 0.0f, 0.0f);
+    float2* o = out + 16ull * rec + 3u * r;
+    o[0] = make_float2(p[0], p[1]);
+    o[1] = make_float2(p[3] - p[0], p[4] - p[1]);
+    o[2] = make_float2(p[2], p[5] - p[2]);
+    if (r == 3u) { dst[8ull * rec + 6] = make_float4(0.f, 0.f, 0.f, 0.f); dst[8ull * rec + 7] = make_float4(0.f, 0.f, 0.f, 0.f); }
   }
 }
 

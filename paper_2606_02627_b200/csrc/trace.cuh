@@ -84,9 +84,11 @@ constexpr int REC_GROUP = 8;
 #define STREAMI_RK4_MIN_BLOCKS 3  // resident blocks per SM the register allocation must allow
 #endif
 constexpr int REC_THREADS = STREAMI_RK4_BLOCK;
+constexpr int DP5_THREADS = 128;   // threads per block of the DP5(4) kernels (trace_block in trace_kernel.cuh)
+template <int BT>
 __device__ __forceinline__ float* rec_stage() {
   // [thread][plane][slot & 7]: a lane's group is 96 contiguous bytes, read back as 6 LDS.128
-  __shared__ __align__(16) float s_rec[3 * REC_GROUP * REC_THREADS];
+  __shared__ __align__(16) float s_rec[3 * REC_GROUP * BT];
   return s_rec + 3 * REC_GROUP * threadIdx.x;
 }
 
@@ -95,10 +97,11 @@ __device__ __forceinline__ float* rec_scratch() {              // never read: cp
   return s_scr + threadIdx.x;
 }
 
+template <int BT = REC_THREADS>
 __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
   const unsigned cnt = L.slot - L.stage0;
   if (cnt != 0u && a.verts) {
-    const float* s = rec_stage();
+    const float* s = rec_stage<BT>();
     const unsigned long long plane = a.n * a.cap;
     float* dst = a.verts + (unsigned long long)L.id * a.cap + L.stage0;
     if (cnt == (unsigned)REC_GROUP && a.vec_ok) {               // stage0 is then a multiple of 8
@@ -126,17 +129,17 @@ __device__ __forceinline__ void flush_vertices(const TraceArgs& a, Lane& L) {
 // records in almost every iteration (27 lanes, stride 8, phases apart), so a branch around the
 // three shared-memory stores was taken -- and its whole body issued for 3 lanes -- nearly always.
 // Without an output array the stores still go to the staging words, which are then never read.
-template <bool REC = true>
+template <bool REC = true, int BT = REC_THREADS>
 __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
   if (!REC) return;
   if (a.staging) {
     const bool due = --L.rec_cd == 0u;
     L.rec_cd = due ? a.stride : L.rec_cd;
     const bool rec = due && L.slot < a.cap;
-    float* s = rec_stage() + (L.slot & (REC_GROUP - 1));
+    float* s = rec_stage<BT>() + (L.slot & (REC_GROUP - 1));
     if (rec) { s[0] = L.px; s[REC_GROUP] = L.py; s[2 * REC_GROUP] = L.pz; }
     L.slot += rec ? 1u : 0u;
-    if (rec && (L.slot & (REC_GROUP - 1)) == 0u) flush_vertices(a, L);
+    if (rec && (L.slot & (REC_GROUP - 1)) == 0u) flush_vertices<BT>(a, L);
   } else if (--L.rec_cd == 0) {                  // option "vertex_staging" = 0 (for A/B measurement)
     L.rec_cd = a.stride;
     if (L.slot < a.cap) {

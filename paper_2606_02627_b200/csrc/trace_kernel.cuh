@@ -12,12 +12,13 @@
 
 namespace streami {
 
-// Threads per block: 256 for RK4; DP5(4) keeps six stage vectors (92 registers), and blocks of
-// 128 let 5 of them (20 warps) share an SM where 256-thread blocks fit only 2 (16 warps).
-constexpr int trace_block(int integ) { return integ == 1 ? 128 : STREAMI_RK4_BLOCK; }
+// Threads per block: 256 for RK4; DP5(4) keeps six stage vectors, and blocks of 128 give the
+// register allocator a finer occupancy grid (6 to 8 blocks = 24 to 32 warps, see trace_min_blocks).
+__host__ __device__ constexpr int trace_block(int integ) { return integ == 1 ? DP5_THREADS : STREAMI_RK4_BLOCK; }
 
+template <int BT>
 __device__ __forceinline__ void finish_particle(const TraceArgs& a, Lane& L, unsigned st) {
-  flush_vertices(a, L);
+  flush_vertices<BT>(a, L);
   if (a.counts) a.counts[L.id] = L.slot;
   if (a.steps) a.steps[L.id] = L.n;
   if (a.status) a.status[L.id] = st;
@@ -32,7 +33,7 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
                                               bool handoff) {
   unsigned mask = __ballot_sync(__activemask(), emit);
   if (!emit) return;
-  flush_vertices(a, L);
+  flush_vertices<trace_block(INTEG)>(a, L);
   int lane = threadIdx.x & 31;
   int leader = __ffs(mask) - 1;
   unsigned base = 0;
@@ -74,8 +75,15 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
 // Resident blocks per SM the compiler must allow for.  3 blocks of 256 (<= 80 registers): capping
 // the steady RK4 kernel at 64 registers for a 4th block was measured on C2 and lost to its spills.
 // Pathlines with the two-slice cell copy (48 more registers): 2 blocks of 256 (RK4), 3 of 128 (DP5(4)).
-constexpr int trace_min_blocks(int integ, bool unsteady, bool brick, bool cache) {
-  return (unsteady && cache) ? (integ == 1 ? 3 : 2) : (integ == 1 ? 5 : STREAMI_RK4_MIN_BLOCKS);
+// Steady DP5(4) is latency-bound -- every stage of an attempt waits for the slowest lane's DRAM round
+// trip -- and scales with resident warps as long as the memory system takes the requests: on
+// LAYOUT_CELL (a cell = 3 loads from ONE line, ~1.4 L2 requests) C5 takes 933 / 774 / 746 / 741 ms
+// at 5 / 6 / 7 / 8 blocks of 128 (64 registers, 64 bytes of stack at 8); on XYQUAD (4 requests per cell)
+// 956 / 885 / 1194 / 1214 ms: past 6 blocks its requests saturate the L2 miss path.  The brick form
+// (descriptor live, spills at 80 registers already) stays at 5.
+constexpr int trace_min_blocks(int layout, int integ, bool unsteady, bool brick, bool cache) {
+  return (unsteady && cache) ? (integ == 1 ? 3 : 2)
+                             : (integ == 1 ? (brick ? 5 : (layout == LAYOUT_CELL ? 8 : 6)) : STREAMI_RK4_MIN_BLOCKS);
 }
 template <bool T> struct TraceCache { typedef CellCache type; };
 template <> struct TraceCache<true> { typedef CellCacheT type; };
@@ -103,7 +111,7 @@ __device__ __forceinline__ uint4 ld_volatile_v4(const uint4* p) {
 }
 
 template <int LAYOUT, int INTEG, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool INQ = false>
-__global__ void __launch_bounds__(trace_block(INTEG), trace_min_blocks(INTEG, UNSTEADY, BRICK, CACHE))
+__global__ void __launch_bounds__(trace_block(INTEG), trace_min_blocks(LAYOUT, INTEG, UNSTEADY, BRICK, CACHE))
 trace_kernel(const TraceArgs a) {
   __shared__ unsigned long long s_tot[4];
   if (threadIdx.x < 4) s_tot[threadIdx.x] = 0ull;
@@ -171,10 +179,10 @@ trace_kernel(const TraceArgs a) {
           if (fresh) {
             float gx, gy, gz;
             if (!to_index<UNIT>(a.g, L.px, L.py, L.pz, gx, gy, gz)) {           // A5.1
-              finish_particle(a, L, ST_OUT);
+              finish_particle<trace_block(INTEG)>(a, L, ST_OUT);
               active = false; term = true;
             } else {
-              record_vertex(a, L);                                              // vertex 0 = seed
+              record_vertex<true, trace_block(INTEG)>(a, L);                    // vertex 0 = seed
               if (BRICK) {
                 my_brick = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
                 if (a.rc_this) atomicAdd(a.rc_this + my_brick, 1u);
@@ -193,7 +201,7 @@ trace_kernel(const TraceArgs a) {
               unsigned rc = sample<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT, true>(a.g, st, cc, L.px, L.py, L.pz, L.t,
                                                                                L.k1x, L.k1y, L.k1z);
               if (fresh) n_samples++;
-              if (rc) { finish_particle(a, L, rc); active = false; term = true; atomicAdd(&s_tot[2], 1ull); }
+              if (rc) { finish_particle<trace_block(INTEG)>(a, L, rc); active = false; term = true; atomicAdd(&s_tot[2], 1ull); }
             }
           }
         }
@@ -264,7 +272,7 @@ trace_kernel(const TraceArgs a) {
       }
       if (rc) {
         active = false;
-        if (rc == RC_HANDOFF) emit = true; else { finish_particle(a, L, rc); term = true; }
+        if (rc == RC_HANDOFF) emit = true; else { finish_particle<trace_block(INTEG)>(a, L, rc); term = true; }
         if (INTEG == 0) {                       // RK4 counters are derived (see rk4_step)
           n_attempts = (L.n - n_start) + (done >= 2u ? 1u : 0u);
           n_samples = 4u * (L.n - n_start) + min(done, 4u);
