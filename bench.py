@@ -6,17 +6,32 @@
 A "step" is one pass of the whole hot path over one batch of
 synthetic input: one C-ABI trace call over all seeds of the workload -- Morton presort, the
 persistent advection kernel (fetch, cell location, trilinear gather, RK stages, termination,
-vertex record, refill) until every particle has terminated.  Default workload = BASELINE.json
-configs[1] (C2): 256^3 turbulence, 1,048,576 seeds, RK4 h = 0.25, max 2,000 steps, throughput
-recording (capacity 256, stride 8).
+vertex record, refill) until every particle has terminated.  Default workload = the LARGEST
+single-GPU configuration, BASELINE.json configs[4] (C5): 1024^3 turbulence (12.9 GB), 16,777,216
+seeds, DP5(4) tol 1e-5, max 8,000 steps, throughput recording (capacity 64, stride 128; SURVEY.md
+8(d) table) -- it stands in for the paper's only benchmark volume (1K^3 voxels).
+The same JSON line carries BASELINE.json configs[1] (C2: 256^3, 1,048,576 seeds, RK4 h = 0.25,
+max 2,000, capacity 256 stride 8) under "also": {"c2": {...}} with the same fields.
 
 metric  = RK particle-steps per second (step ATTEMPTS), whole job over all ranks.
 value   = device-resident inputs, CUDA events on the launching stream around each step.
 e2e     = the same through the C-ABI *_host calls with pinned HOST buffers (streamlines: seeds in,
           assembled polylines out -- streami_trace_streamlines_lines_host)
           (H2D of the seeds and D2H of every output inside the timed region).
-roofline= the advection kernel alone (event pair recorded by the library around its launch):
-          algorithmic bytes / its duration, against MEASURED_PEAKS.json.
+roofline= the advection kernel alone (event pair recorded by the library around its launch), against
+          MEASURED_PEAKS.json hbm_gbs:
+          achieved / frac    ALGORITHMIC bytes = SURVEY.md 8(d)'s compulsory row (what the method must move
+                             with perfect caching: 18 / 36 / 72 B per RK4-steady / RK4-unsteady / DP5(4) step
+                             attempt + 12 B per stored vertex + 36 B per particle) / live kernel time
+                             (= compulsory_frac)
+          traffic            dram__bytes_read + write per launch, ncu (profiles/traffic.csv, stamped with the
+                             commit and kernel time it was captured at; flagged when stale)
+          dram_gbs/dram_frac that measured traffic / LIVE kernel time: what the memory system carries
+          wasted_traffic     traffic / algorithmic bytes
+          useful_request_gbs bytes the samples ask for (8 vertices x 12 B per sample and slice), a RATE only:
+                             the register cell cache answers most of them without any memory access
+          l2                 lts__t_sectors_op_read x 32 B per launch (ncu) / live kernel time against the
+                             L2-resident gather ceiling measured on this chip
 cpu_baseline = the fp32 oracle, as it stands, on the host cores, on a bounded strided sample.
 
 Multi-GPU (torchrun): the field is replicated, every rank traces its own 1,048,576 seeds
@@ -47,8 +62,6 @@ WORKLOADS = {
     "c3": dict(kind="bricks", N=512, M=512, kmax=64, n=1 << 22, nb=(2, 2, 2), prm=dict(integrator=0,
                h=0.25, max_steps=4000, vmin=1e-6, capacity=256, stride=16)),
     "c4": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6)),
-    # C4 with the paper's own time handling, fields[(int)simTime]: one slice per sample
-    "c4p": dict(kind="gyre", m=4096, nsteps=1000, prm=dict(integrator=0, h=0.05, vmin=1e-6, time_mode=1)),
     "c5": dict(kind="turb", N=1024, M=1024, kmax=256, n=1 << 24, prm=dict(integrator=1, h=0.25,
                h_min=0.01, h_max=1.0, atol=1e-5, rtol=1e-5, max_steps=8000, vmin=1e-6, capacity=64,
                stride=128),
@@ -63,13 +76,6 @@ WORKLOADS = {
     # (PAPER.md:159), bins 127^3, RK4 (never the reported headline)
     "u1": dict(kind="mesh", N=128, M=128, kmax=32, n=1 << 18, nbins=(127, 127, 127), prm=dict(integrator=0, h=0.25,
                max_steps=500, vmin=1e-6, capacity=64, stride=8)),
-    # L2-resident variant of C2 (same step size and seed count, 64^3 field): isolates the instruction
-    # stream from the DRAM gathers when reading profiles (never a reported number)
-    "c2s": dict(kind="turb", N=64, M=64, kmax=16, n=1 << 20, prm=dict(integrator=0, h=0.25,
-                max_steps=2000, vmin=1e-6, capacity=256, stride=8)),
-    # reduced sizes for quick checks of this script itself (never a reported number)
-    "tiny": dict(kind="turb", N=48, M=32, kmax=8, n=4096, prm=dict(integrator=0, h=0.25,
-                 max_steps=500, vmin=1e-6, capacity=64, stride=8)),
 }
 DESCR = {
     "c1": "C1 ABC 32^3, 1,024 seeds, RK4 h=0.01, max 1,000",
@@ -77,11 +83,8 @@ DESCR = {
     "c3": "C3 turbulence 512^3 in 2x2x2 bricks (ghost 1), 4,194,304 seeds, RK4 h=0.25, max 4,000",
     "c4": "C4 double gyre 256x128x64 x 64 slices, 4,096-point rake, 1,000 steps, streaklines",
     "c5": "C5 turbulence 1024^3 (1,024 modes), 16,777,216 seeds, DP5(4) tol 1e-5, max 8,000",
-    "c4p": "C4 with the paper's hold-floor-slice time handling (comparison only)",
-    "c2s": "C2 with an L2-resident 64^3 field (profiling aid only)",
     "p4": "P4 pathlines through C4's double gyre (64 slices), 1,048,576 seeds, RK4 h=0.05, max 1,000",
     "u1": "U1 hexahedral mesh: 128^3 turbulence grid as 2,048,383 hexahedra, 262,144 seeds, RK4 h=0.25, max 500",
-    "tiny": "tiny turbulence 48^3 (script self-check only)",
 }
 
 
@@ -143,10 +146,10 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default=None, choices=sorted(WORKLOADS),
+                    help="default: c5 (the largest single-GPU config) with c2 carried under \"also\"")
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 packed3, 2 float4, 3 xpair, 4 cell, 5 xyquad")
     ap.add_argument("--opt", action="append", default=[], help="library option name=value")
-    ap.add_argument("--probe", action="store_true", help="print the gather ceilings (L2 / DRAM, 32-128 B pieces) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -322,18 +325,33 @@ class Job:
             self.e2e_points, _ = S.streami_trace_streamlines_lines_host(self.field, h["seeds"], self.prm_h,
                                                                         h["offsets"], h["points"])
 
+    def host_field_lazy(self):
+        """The field on the host for the oracle legs.  The 1024^3 field (12.9 GB) is copied back only when
+        asked for: the same bytes the CUDA path traced."""
+        if self.host_field is None and self.kind == "turb" and self.data is not None:
+            import workloads as wl
+            N = self.w["N"]
+            self.host_field = wl.Field((N, N, N), (0.0, 0.0, 0.0), (1.0, 1.0, 1.0), self.data.cpu().numpy())
+        return self.host_field
+
+    def release_pinned(self):
+        self.h = None
+
+    def close(self):
+        """Free the field handle and every device buffer of this job (the next workload needs the memory)."""
+        if self.kind != "mesh":
+            self.field.destroy()
+        else:
+            self.field.destroy()
+        for k in ("data", "seeds", "verts", "counts", "steps_o", "status_o", "final_o", "totals_o", "prm", "h", "host_field"):
+            setattr(self, k, None)
+
     def work(self):
         """(attempted steps, accepted steps, field samples, hand-offs, stored vertices) of the
         last device step."""
         tot = [int(x) for x in self.totals_o.cpu().tolist()]
         stored = self.npart if self.kind == "gyre" else int(self.counts.to(self.torch.int64).sum().item())
         return tot[0], tot[1], tot[2], tot[3], stored
-
-    def algorithmic_bytes(self, samples, stored):
-        """useful gather bytes (8 vertices x 12 B per sample and slice) +
-        12 B per stored vertex + per-particle fetch (12 B) and results (24 B)."""
-        per_sample = 192 if (self.kind in ("gyre", "path") and not self.w["prm"].get("time_mode")) else 96
-        return samples * per_sample + stored * 12 + self.npart * 36
 
 
 # ------------------------------------------------------------------------------------------------
@@ -484,46 +502,82 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def main():
-    args = parse_args()
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
-        reference_arm(args, rank)
-        return
-    if args.probe:
-        if rank == 0:
-            import torch
-            import paper_2606_02627_b200 as S
-            torch.cuda.set_device(local)
-            rows = []
-            for span_mb in (48, 537, 8192, 34400):
-                for piece in (32, 64, 128):
-                    rows.append({"span_mb": span_mb, "piece_bytes": piece,
-                                 "gbs": S.streami_probe_gather(span_mb << 20, piece, 3000)})
-            print(json.dumps({"probe": "random aligned gathers, useful GB/s", "rows": rows}))
-        return
+# L2-resident gather ceiling of this chip: random aligned 32-byte reads inside a 48 MB buffer, one per thread and
+# iteration, 64 warps per SM (round-1 probe: 8,170 GB/s; 64-byte pieces 8,350).  No driver
+# file records an L2 peak, so this measured figure is the denominator of roofline.l2.
+L2_GATHER_GBS = 8170.0
+
+# SURVEY.md 8(d), "Compulsory new data (perfect caching)": bytes per step attempt
+COMPULSORY_B = {"rk4_steady": 18.0, "rk4_unsteady": 36.0, "dp5": 72.0}
+
+
+def traffic_row(workload, layout_name):
+    """ncu counters of the dominant kernel, per launch (profiles/traffic.csv; profiles/traffic.md says how)."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tpath):
+        return None
+    import csv
+    best = None
+    with open(tpath) as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload and row.get("layout", layout_name) in (layout_name, ""):
+                best = row
+    return best
+
+
+def roofline_of(job, workload, samples, stored, attempts, kern_ms, kern_n, steps, total_ms, world, lay):
+    peak, peak_src = peaks()
+    launches_per_step = max(1, kern_n // max(1, steps))
+    kms = kern_ms / max(1, kern_n)                                   # live, CUDA events on the launching stream
+    unsteady = job.kind in ("gyre", "path") and not job.w["prm"].get("time_mode")
+    per_attempt = COMPULSORY_B["dp5"] if job.w["prm"].get("integrator") == 1 else (
+        COMPULSORY_B["rk4_unsteady"] if unsteady else COMPULSORY_B["rk4_steady"])
+    alg = attempts * per_attempt + stored * 12.0 + job.npart * 36.0      # per step (all launches of it)
+    useful = samples * (192.0 if unsteady else 96.0) + stored * 12.0 + job.npart * 36.0
+    sec = kms * 1e-3
+    achieved = (alg / launches_per_step) / sec / 1e9 if kms > 0 else None
+    r = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+         "frac": None if achieved is None else achieved / peak, "traffic": None,
+         "kernel": {"gyre": "streak_kernel", "mesh": "mesh_trace_kernel"}.get(job.kind, "trace_kernel"),
+         "kernel_ms_per_launch": kms, "kernel_launches_per_step": launches_per_step,
+         "algorithmic_bytes_per_launch": alg / launches_per_step,
+         "algorithmic_basis": "SURVEY.md 8(d) compulsory row: %g B per step attempt + 12 B per stored vertex + 36 B per particle"
+                              % per_attempt,
+         "compulsory_frac": None if achieved is None else achieved / peak,
+         "useful_request_gbs": (useful / launches_per_step) / sec / 1e9 if kms > 0 else None,
+         "peak_source": peak_src,
+         "kernel_share_of_step": kern_ms / total_ms if world == 1 else None}
+    row = traffic_row(workload, lay)
+    if row is not None and kms > 0:
+        tr = float(row["dram_bytes_per_launch"])
+        r["traffic"] = tr
+        r["traffic_source"] = row["source"]
+        r["dram_gbs"] = tr / sec / 1e9
+        r["dram_frac"] = r["dram_gbs"] / peak
+        r["wasted_traffic"] = tr / (alg / launches_per_step)
+        cap_ms = float(row["kernel_ms_at_capture"])
+        r["traffic_captured_at"] = {"commit": row["commit"], "kernel_ms": cap_ms}
+        # the counted bytes belong to the kernel as it was when ncu saw it: flag them when the live kernel has moved
+        r["traffic_stale"] = abs(kms - cap_ms) > 0.10 * cap_ms
+        lts = float(row["lts_read_bytes_per_launch"])
+        r["l2"] = {"achieved": lts / sec / 1e9, "peak": L2_GATHER_GBS, "unit": "GB/s",
+                   "frac": lts / sec / 1e9 / L2_GATHER_GBS,
+                   "peak_source": "measured on B200: random 32-byte gathers inside an L2-resident 48 MB buffer (DESIGN.md section 6)",
+                   "numerator": "lts__t_sectors_op_read.sum x 32 B per launch (ncu) / live kernel time"}
+        r["ncu"] = {k: float(row[k]) for k in ("l1_hit_pct", "l2_hit_pct", "active_lanes_per_warp_instruction",
+                                               "issue_slots_busy_pct") if row.get(k)}
+    return r
+
+
+def run_workload(name, args, rank, local, world, red, cpu_seconds, steps, warmup):
+    """One workload through all legs: device-resident timed region, e2e, roofline, cpu_baseline."""
     import torch
-    import torch.distributed as dist
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    red = Reducer(world, "cuda")
-    barrier, allmax, allsum = red.barrier, red.max, red.sum
-
     import paper_2606_02627_b200 as S
-    for kv in args.opt:
-        k, v = kv.split("=")
-        S.streami_set_option(k, int(v))
-    job = Job(args.workload, rank, args.layout)
+    barrier, allmax = red.barrier, red.max
+    job = Job(name, rank, args.layout)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         job.step_device()
     torch.cuda.synchronize()
     attempts, accepted, samples, handoffs, stored = job.work()
@@ -531,7 +585,7 @@ def main():
     # ---- timed region: exactly K steps, device-resident ---------------------------------------
     S.streami_set_option("kernel_timing", 1)
     S.streami_kernel_time()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     sampler = ClockSampler(local) if rank == 0 else None
     barrier()
     l0 = S.streami_launch_count()
@@ -547,7 +601,7 @@ def main():
     clocks = sampler.stop(t0, t1) if sampler else None
     kern_ms, kern_n = S.streami_kernel_time()
     S.streami_set_option("kernel_timing", 0)
-    value, total_ms, job_attempts = job_value(attempts, args.steps, sum(a.elapsed_time(b) for a, b in ev), red)
+    value, total_ms, job_attempts = job_value(attempts, steps, sum(a.elapsed_time(b) for a, b in ev), red)
 
     # ---- e2e: host buffers, copies inside the timed region --------------------------------------
     e2e = None
@@ -556,77 +610,92 @@ def main():
         bi, bo = job.e2e_bytes()
         barrier()
         w0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             job.step_host()
         torch.cuda.synchronize()
         w1 = time.perf_counter()
         e_ms = allmax((w1 - w0) * 1e3)
-        e2e = {"value": job_attempts * args.steps / (e_ms * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "ms_per_step": e_ms / args.steps}
+        e2e = {"value": job_attempts * steps / (e_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "ms_per_step": e_ms / steps}
+        job.release_pinned()
         barrier()
-
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
-
-    # ---- roofline of the advection kernel (rank 0) ----------------------------------------------
-    peak, peak_src = peaks()
-    alg = job.algorithmic_bytes(samples, stored)
-    launches_per_step = max(1, kern_n // max(1, args.steps))
-    kms = kern_ms / max(1, kern_n)
-    achieved = (alg / launches_per_step) / (kms * 1e-3) / 1e9 if kms > 0 else None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": None if achieved is None else achieved / peak, "traffic": None,
-                "kernel": {"gyre": "streak_kernel", "mesh": "mesh_trace_kernel"}.get(job.kind, "trace_kernel"),
-                "kernel_ms_per_launch": kms, "kernel_launches_per_step": launches_per_step,
-                "algorithmic_bytes_per_launch": alg / launches_per_step, "peak_source": peak_src,
-                "kernel_share_of_step": kern_ms / total_ms if world == 1 else None}
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram bytes per launch (profiles/traffic.md)
-    if os.path.exists(tpath):
-        import csv
-        with open(tpath) as f:
-            for row in csv.DictReader(f):
-                if row["workload"] == args.workload:
-                    roofline["traffic"] = float(row["dram_bytes_per_launch"])
-                    roofline["traffic_source"] = row["source"]
-                    roofline["ncu"] = {k: float(v) for k, v in row.items()
-                                       if k not in ("workload", "source", "dram_bytes_per_launch")}
-                    # the same kernel against the same peak, but with the DRAM bytes ncu counted for one launch
-                    # (the profiled launch; C4's launches differ in work, see profiles/traffic.md) instead of the
-                    # algorithmic bytes: how far the memory system, not the method's request stream, is loaded
-                    if kms > 0:
-                        roofline["dram_gbs_from_traffic"] = roofline["traffic"] / (kms * 1e-3) / 1e9
-                        roofline["dram_frac_from_traffic"] = roofline["dram_gbs_from_traffic"] / peak
-
-    cpu = None
-    if world == 1 and not args.no_cpu and job.host_field is not None:
-        orc = OracleRun(args.workload, job.host_field, job.seeds_h)
-        a, dt, npart, stride = orc.bounded(args.cpu_seconds)
-        cpu = {"value": a / dt, "unit": UNIT, "cores": orc.cores, "kind": "oracle",
-               "sample": "every %d-th particle of the same workload (%d particles, %d step attempts, %.1f s)"
-                         % (stride, npart, a, dt)}
+    del flush
 
     lay = {1: "packed3", 2: "float4", 3: "xpair", 4: "cell", 5: "xyquad"}.get(job.layout, str(job.layout))
     if job.kind == "mesh":
         lay = "224-byte cell records (8 corner positions + 8 corner values + box)"
-    out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": DESCR[args.workload], "seeds_per_gpu": job.n,
-                   "recording": {k: job.w["prm"][k] for k in ("capacity", "stride") if k in job.w["prm"]},
-                   "field_layout": lay, "field_bytes_owned": job.owned_bytes,
-                   "l2": "flushed between timed steps (256 MiB memset) and the field is larger than L2",
-                   "parallelism": "seeds sharded over %d GPU(s), field replicated" % world,
-                   "options": {k: S.streami_get_option(k) for k in ("cell_cache", "presort")}},
-        "work_per_step_per_gpu": {"step_attempts": attempts, "accepted_steps": accepted,
-                                  "field_samples": samples, "handoffs": handoffs,
-                                  "stored_vertices": stored, "rounds": job.nrounds},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-        "cpu_baseline": cpu,
-    }
-    print(json.dumps(out))
+    out = None
+    if rank == 0:
+        roofline = roofline_of(job, name, samples, stored, attempts, kern_ms, kern_n, steps, total_ms, world, lay)
+        cpu = None
+        if world == 1 and not args.no_cpu:
+            fld = job.host_field_lazy()
+            if fld is not None:
+                orc = OracleRun(name, fld, job.seeds_h)
+                a, dt, npart, stride = orc.bounded(cpu_seconds)
+                cpu = {"value": a / dt, "unit": UNIT, "cores": orc.cores, "kind": "oracle",
+                       "sample": "every %d-th particle of the same workload (%d particles, %d step attempts, %.1f s)"
+                                 % (stride, npart, a, dt)}
+                del orc
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": DESCR[name], "seeds_per_gpu": job.n,
+                       "recording": {k: job.w["prm"][k] for k in ("capacity", "stride") if k in job.w["prm"]},
+                       "field_layout": lay, "field_bytes_owned": job.owned_bytes,
+                       "l2": "flushed between timed steps (256 MiB memset) and the field is larger than L2",
+                       "parallelism": "seeds sharded over %d GPU(s), field replicated" % world,
+                       "options": {k: S.streami_get_option(k) for k in ("cell_cache", "presort")}},
+            "work_per_step_per_gpu": {"step_attempts": attempts, "accepted_steps": accepted,
+                                      "field_samples": samples, "handoffs": handoffs,
+                                      "stored_vertices": stored, "rounds": job.nrounds},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+        if cpu is not None:
+            out["vs_cpu_baseline"] = value / cpu["value"]     # context only; vs_baseline stays null (no published number)
+    job.close()
+    del job
+    torch.cuda.empty_cache()
+    return out
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    headline = args.workload or "c5"
+    if args.impl == "reference":
+        args.workload = headline
+        reference_arm(args, rank)
+        return
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    red = Reducer(world, "cuda")
+
+    import paper_2606_02627_b200 as S
+    for kv in args.opt:
+        k, v = kv.split("=")
+        S.streami_set_option(k, int(v))
+
+    out = run_workload(headline, args, rank, local, world, red, args.cpu_seconds, args.steps, args.warmup)
+    if args.workload is None:
+        # the default run also carries BASELINE.json configs[1] (C2), the config the metric was first quoted on
+        c2 = run_workload("c2", args, rank, local, world, red, min(args.cpu_seconds, 6.0), args.steps, args.warmup)
+        if rank == 0:
+            out["also"] = {"c2": c2}
+            out["gpu_launches"] += c2["gpu_launches"]
+            out["config"]["also"] = "c2 = " + DESCR["c2"]
+    if rank == 0:
+        print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 

@@ -308,11 +308,6 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
 int streami_set_option(const char* name, int value);
 int streami_get_option(const char* name, int* value);
 
-/* Gather probe: useful GB/s of random aligned reads of piece_bytes (32, 64 or 128) inside a freshly
- * allocated buffer of span_bytes, iters reads per resident thread; the memory-system ceiling a
- * trilinear gather can be held against (span below L2 size: L2 rate; far above: DRAM rate).
- * out_gbs is a HOST pointer; synchronises cuda_stream. */
-int streami_probe_gather(size_t span_bytes, int piece_bytes, int iters, float* out_gbs, void* cuda_stream);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */
 unsigned long long streami_launch_count(void);

@@ -57,7 +57,6 @@ def lib():
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
-        L.streami_probe_gather.argtypes = [Z, I, I, P, P]
         L.streami_mesh_create_hex.argtypes = [Z, Z, P, P, P, P, P, P, P]
         L.streami_mesh_destroy.argtypes = [P]
         L.streami_mesh_sample.argtypes = [P, P, Z, P, P, P]
@@ -306,36 +305,6 @@ def streami_mesh_trace_streamlines_lines_host(mesh, seeds, prm_host, out_offsets
     """The same on a hexahedral mesh."""
     return _lines_host(lib().streami_mesh_trace_streamlines_lines_host, mesh.handle, seeds, prm_host, out_offsets,
                        out_points, stream)
-
-
-def streami_probe_gather(span_bytes, piece_bytes, iters=2000, stream=None):
-    """Useful GB/s of random aligned reads (the gather ceiling, include/streami.h)."""
-    out = ctypes.c_float(0.0)
-    _check(lib().streami_probe_gather(int(span_bytes), int(piece_bytes), int(iters), ctypes.byref(out), _stream(stream)))
-    return out.value
-
-
-class Mesh:
-    """Owner of a streami_mesh handle (hexahedral mesh field)."""
-
-    def __init__(self, X, V, H, lo, hi, nb):
-        import numpy as np
-        X = np.ascontiguousarray(X, dtype=np.float32); V = np.ascontiguousarray(V, dtype=np.float32)
-        H = np.ascontiguousarray(H, dtype=np.uint32)
-        self.handle = ctypes.c_void_p(None)
-        _check(lib().streami_mesh_create_hex(X.shape[0], H.shape[0], X.ctypes.data, V.ctypes.data, H.ctypes.data,
-                                             _f3(lo), _f3(hi), _i3(nb), ctypes.byref(self.handle)))
-
-    def destroy(self):
-        if self.handle:
-            lib().streami_mesh_destroy(self.handle)
-            self.handle = None
-
-    def __del__(self):
-        try:
-            self.destroy()
-        except Exception:
-            pass
 
 
 def streami_mesh_sample(mesh, points, stream=None):

@@ -12,7 +12,30 @@
 
 namespace streami {
 
-Options& options() { static Options o{1, 1, 0, 0, 0, 1, 1, 0, 0, 1, 0, 0}; return o; }
+// process-wide option values, in the member order of Options (internal.h)
+static std::atomic<int> g_options[N_OPTIONS] = {{1}, {1}, {0}, {0}, {0}, {1}, {1}, {0}, {0}, {1}, {0}, {0}};
+static const char* const g_option_names[N_OPTIONS] = {"cell_cache", "presort", "streak_window", "kernel_timing", "segment_steps",
+                                                      "vertex_staging", "prefetch", "max_blocks_per_sm", "brick_round_steps",
+                                                      "integer_accept", "host_batch", "queue_steps"};
+static_assert(sizeof(Options) == N_OPTIONS * sizeof(int), "Options is N_OPTIONS ints");
+static thread_local Options tl_options;
+static thread_local int tl_options_depth = 0;
+static void options_snapshot(Options& o) {
+  int* v = reinterpret_cast<int*>(&o);
+  for (int i = 0; i < N_OPTIONS; ++i) v[i] = g_options[i].load(std::memory_order_relaxed);
+}
+const Options& options() {
+  if (tl_options_depth == 0) options_snapshot(tl_options);
+  return tl_options;
+}
+OptionsScope::OptionsScope() { if (tl_options_depth++ == 0) options_snapshot(tl_options); }
+OptionsScope::~OptionsScope() { --tl_options_depth; }
+int option_index(const char* name) {
+  for (int i = 0; i < N_OPTIONS; ++i) if (!strcmp(name, g_option_names[i])) return i;
+  return -1;
+}
+void option_store(int index, int value) { g_options[index].store(value, std::memory_order_relaxed); }
+int option_load(int index) { return g_options[index].load(std::memory_order_relaxed); }
 std::atomic<unsigned long long>& launch_counter() { static std::atomic<unsigned long long> c{0}; return c; }
 
 static std::mutex g_err_mutex;
@@ -198,6 +221,7 @@ extern "C" {
 int streami_field_create(const int dims[3], const float origin[3], const float spacing[3],
                          int nslices, float slice_dt, const float* dev_ptr, int layout_hint,
                          streami_field* out) {
+  OptionsScope options_scope;
   if (!dims || !origin || !spacing || !dev_ptr || !out) return STREAMI_E_INVALID;
   *out = nullptr;
   int layout = pick_layout(layout_hint);
@@ -250,6 +274,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
                                  const float spacing[3], const int brick_grid[3], int ghost_cells,
                                  const float* const* brick_dev_ptrs, int layout_hint,
                                  streami_field* out) {
+  OptionsScope options_scope;
   if (!global_dims || !origin || !spacing || !brick_grid || !brick_dev_ptrs || !out)
     return STREAMI_E_INVALID;
   *out = nullptr;
@@ -358,6 +383,7 @@ int streami_field_info(streami_field f, int* layout, size_t* owned_bytes) {
 
 int streami_sample(streami_field f, const float* points, size_t n, float t, int time_mode,
                    float* out_v, unsigned* out_rc, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || f->bricked || !points || !out_v || !out_rc) return STREAMI_E_INVALID;
   if (time_mode != 0 && time_mode != 1) return STREAMI_E_INVALID;
   if (n == 0) return STREAMI_OK;
@@ -402,39 +428,25 @@ int streami_seed_shape(const float origin[3], const float edge_u[3], const float
 
 int streami_set_option(const char* name, int value) {
   if (!name) return STREAMI_E_INVALID;
-  Options& o = options();
-  if (!strcmp(name, "cell_cache")) o.cell_cache = value != 0;
-  else if (!strcmp(name, "presort")) o.presort = value != 0;
-  else if (!strcmp(name, "streak_window")) o.streak_window = value < 0 ? 0 : value;
-  else if (!strcmp(name, "kernel_timing")) o.kernel_timing = value != 0;
-  else if (!strcmp(name, "segment_steps")) o.segment_steps = value < 0 ? 0 : value;
-  else if (!strcmp(name, "vertex_staging")) o.vertex_staging = value != 0;
-  else if (!strcmp(name, "brick_round_steps")) o.brick_round_steps = value < -2 ? -2 : value;
-  else if (!strcmp(name, "max_blocks_per_sm")) o.max_blocks_per_sm = value < 0 ? 0 : value;
-  else if (!strcmp(name, "prefetch")) o.prefetch = value < 0 ? 0 : (value > 2 ? 2 : value);
-  else if (!strcmp(name, "integer_accept")) o.integer_accept = value != 0;
-  else if (!strcmp(name, "host_batch")) o.host_batch = value < 0 ? 0 : value;
-  else if (!strcmp(name, "queue_steps")) o.queue_steps = value < 0 ? 0 : value;
-  else return STREAMI_E_INVALID;
+  const int i = option_index(name);
+  if (i < 0) return STREAMI_E_INVALID;
+  Options lim{};    // member offsets only
+  int* base = reinterpret_cast<int*>(&lim);
+  int v = value;
+  if (&base[i] == &lim.cell_cache || &base[i] == &lim.presort || &base[i] == &lim.kernel_timing ||
+      &base[i] == &lim.vertex_staging || &base[i] == &lim.integer_accept) v = value != 0;
+  else if (&base[i] == &lim.brick_round_steps) v = value < -2 ? -2 : value;
+  else if (&base[i] == &lim.prefetch) v = value < 0 ? 0 : (value > 2 ? 2 : value);
+  else v = value < 0 ? 0 : value;
+  option_store(i, v);
   return STREAMI_OK;
 }
 
 int streami_get_option(const char* name, int* value) {
   if (!name || !value) return STREAMI_E_INVALID;
-  Options& o = options();
-  if (!strcmp(name, "cell_cache")) *value = o.cell_cache;
-  else if (!strcmp(name, "presort")) *value = o.presort;
-  else if (!strcmp(name, "streak_window")) *value = o.streak_window;
-  else if (!strcmp(name, "kernel_timing")) *value = o.kernel_timing;
-  else if (!strcmp(name, "segment_steps")) *value = o.segment_steps;
-  else if (!strcmp(name, "vertex_staging")) *value = o.vertex_staging;
-  else if (!strcmp(name, "brick_round_steps")) *value = o.brick_round_steps;
-  else if (!strcmp(name, "max_blocks_per_sm")) *value = o.max_blocks_per_sm;
-  else if (!strcmp(name, "prefetch")) *value = o.prefetch;
-  else if (!strcmp(name, "integer_accept")) *value = o.integer_accept;
-  else if (!strcmp(name, "host_batch")) *value = o.host_batch;
-  else if (!strcmp(name, "queue_steps")) *value = o.queue_steps;
-  else return STREAMI_E_INVALID;
+  const int i = option_index(name);
+  if (i < 0) return STREAMI_E_INVALID;
+  *value = option_load(i);
   return STREAMI_OK;
 }
 
@@ -475,74 +487,3 @@ const char* streami_error_string(int code) {
 }
 
 }  // extern "C"
-
-// ---- gather probe: what the memory system gives a field-line tracer ---------------------------
-// Every thread reads random aligned pieces of `piece` bytes (32, 64 or 128: one, two or four
-// 256-bit loads) inside a buffer of `span` bytes filled with non-repeating data, with as many
-// pieces in flight as resident threads.  span below the L2 size measures the L2 gather rate,
-// span far above it the DRAM gather rate.  This is the roofline a trilinear gather can be held
-// against; the streaming copy peak of MEASURED_PEAKS.json is not reachable
-// by 32-byte gathers.
-namespace streami {
-static __global__ void probe_fill_kernel(unsigned* __restrict__ p, size_t nwords) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t step = (size_t)gridDim.x * blockDim.x;
-  for (; i < nwords; i += step) p[i] = (unsigned)(i * 2654435761ull) ^ (unsigned)(i >> 13);
-}
-template <int NV8>
-static __global__ void __launch_bounds__(256) probe_gather_kernel(const char* __restrict__ buf, size_t nslots, int iters,
-                                                                  float* __restrict__ sink) {
-  unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
-  float acc = 0.0f;
-  for (int it = 0; it < iters; ++it) {
-    s = s * 1664525u + 1013904223u;
-    const size_t r = ((size_t)s * 40503ull + (s >> 7)) % nslots;
-    const char* p = buf + r * (32 * NV8);
-#pragma unroll
-    for (int j = 0; j < NV8; ++j) {
-      float v0, v1, v2, v3, v4, v5, v6, v7;
-      asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                   : "=f"(v0), "=f"(v1), "=f"(v2), "=f"(v3), "=f"(v4), "=f"(v5), "=f"(v6), "=f"(v7)
-                   : "l"(p + 32 * j));
-      acc += v0 + v7;
-    }
-  }
-  if (acc == 123.456f) sink[0] = acc;
-}
-}  // namespace streami
-
-extern "C" int streami_probe_gather(size_t span_bytes, int piece_bytes, int iters, float* out_gbs,
-                                    void* cuda_stream) {
-  if (!out_gbs || (piece_bytes != 32 && piece_bytes != 64 && piece_bytes != 128) || iters < 1 ||
-      span_bytes < 4096)
-    return STREAMI_E_INVALID;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  char* buf = nullptr; float* sink = nullptr;
-  STREAMI_TRY(cudaMalloc((void**)&buf, span_bytes));
-  cudaError_t e = cudaMalloc((void**)&sink, sizeof(float));
-  cudaEvent_t a = nullptr, b = nullptr;
-  if (e == cudaSuccess) e = cudaEventCreate(&a);
-  if (e == cudaSuccess) e = cudaEventCreate(&b);
-  float ms = 0.0f;
-  const int blocks = num_sms() * 8, threads = 256;
-  if (e == cudaSuccess) {
-    probe_fill_kernel<<<blocks, threads, 0, st>>>((unsigned*)buf, span_bytes / 4);
-    const size_t nslots = span_bytes / (size_t)piece_bytes;
-    for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {          // first pass warms up
-      cudaEventRecord(a, st);
-      if (piece_bytes == 32) probe_gather_kernel<1><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
-      else if (piece_bytes == 64) probe_gather_kernel<2><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
-      else probe_gather_kernel<4><<<blocks, threads, 0, st>>>(buf, nslots, iters, sink);
-      cudaEventRecord(b, st);
-      e = cudaEventSynchronize(b);
-      if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    }
-    launch_counter() += 3;
-  }
-  if (a) cudaEventDestroy(a);
-  if (b) cudaEventDestroy(b);
-  cudaFree(buf); if (sink) cudaFree(sink);
-  if (e != cudaSuccess) return check(e);
-  *out_gbs = (float)((double)blocks * threads * iters * piece_bytes / (ms * 1e6));
-  return STREAMI_OK;
-}

@@ -28,6 +28,7 @@ extern "C" {
 
 int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V, const unsigned* H,
                             const float lo[3], const float hi[3], const int nb[3], streami_mesh* out) {
+  OptionsScope options_scope;
   if (!out) return STREAMI_E_INVALID;
   *out = nullptr;
   if (!X || !V || !H || !lo || !hi || !nb || nv == 0 || nc == 0 || nc > 0xffffffffull) return STREAMI_E_INVALID;
@@ -127,6 +128,7 @@ int streami_mesh_destroy(streami_mesh m) {
 
 int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* out_v, long long* out_cell,
                         void* cuda_stream) {
+  OptionsScope options_scope;
   if (!m || (n > 0 && (!points || !out_v))) return STREAMI_E_INVALID;
   if (n == 0) return STREAMI_OK;
   mesh_sample_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(m->d, points, n, out_v, out_cell);
@@ -136,6 +138,7 @@ int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* ou
 
 int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n, const streami_params* params,
                                    float* out_vertices, unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!m || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, true);
   if (rc) return rc;
@@ -188,6 +191,7 @@ int streami_mesh_trace_streamlines_lines_host(streami_mesh m, const float* seeds
                                               const streami_params* params, unsigned long long* out_offsets,
                                               float* out_points, unsigned long long max_points,
                                               unsigned long long* out_total, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!m) return STREAMI_E_INVALID;
   auto trace = [&](const float* d_seeds, size_t nb, const streami_params* dp, float* d_v, unsigned* d_c) {
     return streami_mesh_trace_streamlines(m, d_seeds, nb, dp, d_v, d_c, cuda_stream);

@@ -129,6 +129,7 @@ struct streami_streak_s {
 int streami_streak_begin(streami_field f, const float* points, size_t m, unsigned nsteps,
                          const streami_params* params, float* out_vertices, void* cuda_stream,
                          streami_streak* out) {
+  OptionsScope options_scope;
   if (!out) return STREAMI_E_INVALID;
   *out = nullptr;
   if (!f || f->bricked || m == 0 || nsteps == 0 || !points || !out_vertices) return STREAMI_E_INVALID;
@@ -163,6 +164,7 @@ int streami_streak_begin(streami_field f, const float* points, size_t m, unsigne
 }
 
 int streami_streak_step(streami_streak h, unsigned k, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!h) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   StreakArgs& a = h->a;
@@ -189,6 +191,7 @@ int streami_streak_position(streami_streak h, unsigned* steps_done) {
 
 int streami_streak_lines(streami_streak h, unsigned long long* out_offsets, float* out_points,
                          unsigned long long* out_total, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!h || !out_offsets) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const StreakArgs& a = h->a;
@@ -214,6 +217,7 @@ int streami_streak_lines(streami_streak h, unsigned long long* out_offsets, floa
 }
 
 int streami_streak_end(streami_streak h, unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!h) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t e = cudaSuccess;
@@ -231,6 +235,7 @@ int streami_streak_end(streami_streak h, unsigned* out_counts, void* cuda_stream
 int streami_trace_streaklines(streami_field f, const float* points, size_t m, unsigned nsteps,
                               const streami_params* params, float* out_vertices,
                               unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || f->bricked || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, false);
   if (rc) return rc;
@@ -252,6 +257,7 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
 int streami_streamline_lines(const float* vertices, const unsigned* counts, size_t n, unsigned capacity,
                              unsigned long long* out_offsets, float* out_points,
                              unsigned long long* out_total, void* cuda_stream) {
+  OptionsScope options_scope;
   if ((n > 0 && !counts) || !out_offsets || capacity == 0 || (n > 0 && out_points && !vertices)) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = scan_counts(counts, n, out_offsets, st);
@@ -274,6 +280,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          unsigned long long* out_handoff_log, size_t log_capacity,
                          unsigned long long* out_log_count, unsigned* out_nrounds,
                          void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || !f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, true);
   if (rc) return rc;
@@ -466,6 +473,7 @@ extern "C" {
 int streami_trace_streaklines_host(streami_field f, const float* points, size_t m, unsigned nsteps,
                                    const streami_params* params, float* out_vertices,
                                    unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || !params || (m > 0 && nsteps > 0 && (!points || !out_vertices || !out_counts))) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t np = m * (size_t)nsteps;
@@ -494,6 +502,7 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
                               unsigned long long* out_handoff_log, size_t log_capacity,
                               unsigned long long* out_log_count, unsigned* out_nrounds,
                               void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || !params || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   if (params->capacity == 0) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -533,6 +542,7 @@ int streami_trace_streamlines_lines_host(streami_field f, const float* seeds, si
                                          const streami_params* params, unsigned long long* out_offsets,
                                          float* out_points, unsigned long long max_points,
                                          unsigned long long* out_total, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f) return STREAMI_E_INVALID;
   // Bricked fields run as one batch: every batch would pay all the rounds (C3 267 -> 293 ms in 4).
   auto trace = [&](const float* d_seeds, size_t nb, const streami_params* dp, float* d_v, unsigned* d_c) {

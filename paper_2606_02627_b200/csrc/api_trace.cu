@@ -103,6 +103,7 @@ extern "C" {
 int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
                               const streami_params* params, float* out_vertices,
                               unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, true);
   if (rc) return rc;
@@ -249,6 +250,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
 int streami_trace_streamlines_host(streami_field f, const float* seeds, size_t n,
                                    const streami_params* params, float* out_vertices,
                                    unsigned* out_counts, void* cuda_stream) {
+  OptionsScope options_scope;
   if (!f || f->bricked || (n > 0 && (!seeds || !out_counts))) return STREAMI_E_INVALID;
   int rc = check_params(params, true);
   if (rc) return rc;

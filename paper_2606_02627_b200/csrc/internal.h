@@ -23,8 +23,16 @@ struct streami_field_s {
 
 namespace streami {
 
+// Library options (streami_set_option).  The process-wide values are atomics; an API call works on ONE
+// snapshot of them, taken when it is entered (OptionsScope), so that a setter running on another host
+// thread can neither tear a value nor change the schedule of a call half way through.
 struct Options { int cell_cache; int presort; int streak_window; int kernel_timing; int segment_steps; int vertex_staging; int prefetch; int max_blocks_per_sm; int brick_round_steps; int integer_accept; int host_batch; int queue_steps; };
-Options& options();
+constexpr int N_OPTIONS = 12;
+const Options& options();            // the snapshot of the API call in progress on this thread, else a fresh one
+int option_index(const char* name);  // -1 if unknown
+void option_store(int index, int value);
+int option_load(int index);
+struct OptionsScope { OptionsScope(); ~OptionsScope(); };
 std::atomic<unsigned long long>& launch_counter();
 void set_cuda_error(cudaError_t e);
 
