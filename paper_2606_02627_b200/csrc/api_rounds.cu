@@ -65,7 +65,7 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
     if (perm) cudaFreeAsync(perm, st);
     if (have_sorter) sorter.release();
   };
-  // scratch: [0] work counter u64, [8] ring tail u32, [12] ring head u32, [16] particles done u32, [20] error u32
+  // scratch: [0] work counter u64, [8] ring tail u64, [16] ring head u64, [24] particles done u32, [28] error u32
   cudaError_t e = cudaMallocAsync((void**)&ctr, 32, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(ctr, 0, 32, st);
   if (e == cudaSuccess) e = cudaMallocAsync((void**)&cq, sizeof(QRec) * cap, st);
@@ -94,8 +94,9 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
   fill_integrator(a, params);
   a.verts = out_vertices; a.n = n; a.counts = out_counts;
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
-  a.qout = cq; a.qout_count = (unsigned*)(ctr + 8); a.cq_head = (unsigned*)(ctr + 12);
-  a.cq_done = (unsigned*)(ctr + 16); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 20);
+  a.qout = cq; a.qout_count = nullptr;
+  a.cq_tail = (unsigned long long*)(ctr + 8); a.cq_head = (unsigned long long*)(ctr + 16);
+  a.cq_done = (unsigned*)(ctr + 24); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 28);
   a.cq_mask = (unsigned)(cap - 1); a.cq_shift = shift;
   int grid = 0;
   rc = trace_grid(k, n, block, &grid);
@@ -106,7 +107,7 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
   launch_counter()++;
   e = cudaGetLastError();
   unsigned err = 0;
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&err, ctr + 20, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&err, ctr + 28, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
   cleanup();
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // streami_brick_advect synchronises its stream (streami.h)
   if (e != cudaSuccess) return check(e);
@@ -371,9 +372,9 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
       unsigned shift = 10;
       while ((1ull << shift) < 2ull * nwork) ++shift;
       const size_t cap = (size_t)1 << shift;
-      char* rctr = nullptr; QRec* ring = nullptr;       // [0] ring tail, [4] head, [8] done, [12] error
-      e = cudaMallocAsync((void**)&rctr, 16, st);
-      if (e == cudaSuccess) e = cudaMemsetAsync(rctr, 0, 16, st);
+      char* rctr = nullptr; QRec* ring = nullptr;       // [0] ring tail u64, [8] head u64, [16] done u32, [20] error u32
+      e = cudaMallocAsync((void**)&rctr, 32, st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(rctr, 0, 32, st);
       if (e == cudaSuccess) e = cudaMallocAsync((void**)&ring, sizeof(QRec) * cap, st);
       if (e == cudaSuccess) e = cudaMemsetAsync(ring, 0, sizeof(QRec) * cap, st);
       if (e == cudaSuccess) e = cudaMemsetAsync(d_next, 0, sizeof(unsigned long long), st);
@@ -382,8 +383,8 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
         TraceKernel kr = pick_trace_kernel_inq(f->layout, unit_geometry(f->g), true);
         a.perm = nullptr; a.seeds4 = nullptr; a.rc_this = nullptr; a.rc_next = nullptr;
         a.seg_budget = 0;                               // until the particle leaves its brick
-        a.qout = ring; a.qout_count = (unsigned*)rctr; a.cq_head = (unsigned*)(rctr + 4);
-        a.cq_done = (unsigned*)(rctr + 8); a.cq_error = (unsigned*)(rctr + 12); a.cq_total = (unsigned)nwork;
+        a.qout = ring; a.qout_count = nullptr; a.cq_tail = (unsigned long long*)rctr; a.cq_head = (unsigned long long*)(rctr + 8);
+        a.cq_done = (unsigned*)(rctr + 16); a.cq_error = (unsigned*)(rctr + 20); a.cq_total = (unsigned)nwork;
         a.cq_mask = (unsigned)(cap - 1); a.cq_shift = shift;
         int grid = 0;
         rc = trace_grid(kr, nwork, block, &grid);
@@ -393,7 +394,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
           timing_end(st);
           launch_counter()++;
           e = cudaGetLastError();
-          if (e == cudaSuccess) e = cudaMemcpyAsync(&err, rctr + 12, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+          if (e == cudaSuccess) e = cudaMemcpyAsync(&err, rctr + 20, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
           if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         }
       }

@@ -158,10 +158,11 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   rc = trace_grid(k, n, block, &grid);
   if (rc) { if (cq) cudaFreeAsync(cq, st); return rc; }
 
-  // scratch: [0] work counter u64, [8] queue counts u32 x 2 (INQ: tail, head), [16] INQ: particles terminated
+  // scratch: [0] work counter u64, [8] queue counts u32 x 2, INQ: [16] ring tail u64, [24] ring head u64,
+  // [32] particles terminated u32, [36] error flag u32
   char* ctr = nullptr;
   {
-    cudaError_t ce = cudaMallocAsync((void**)&ctr, 32, st);
+    cudaError_t ce = cudaMallocAsync((void**)&ctr, 48, st);
     if (ce != cudaSuccess) { if (cq) cudaFreeAsync(cq, st); return check(ce); }
   }
   unsigned long long* next = (unsigned long long*)ctr;
@@ -177,7 +178,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
     if (q[1]) cudaFreeAsync(q[1], st);
     if (have_sorter) sorter.release();
   };
-  cudaError_t e = cudaMemsetAsync(ctr, 0, 32, st);
+  cudaError_t e = cudaMemsetAsync(ctr, 0, 48, st);
   if (e == cudaSuccess && sorting) e = cudaMallocAsync((void**)&perm, sizeof(unsigned) * n, st);
   if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[0], sizeof(QRec) * n, st);
   if (e == cudaSuccess && K) e = cudaMallocAsync((void**)&q[1], sizeof(QRec) * n, st);
@@ -204,8 +205,9 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   a.vec_ok = out_vertices && (params->capacity % 8u) == 0u && ((unsigned long long)out_vertices % 32ull) == 0ull;
   a.qout = K ? q[0] : nullptr; a.qout_count = qcount;
   if (Q) {
-    a.seg_budget = Q; a.qout = cq; a.qout_count = qcount; a.cq_head = qcount + 1;
-    a.cq_done = (unsigned*)(ctr + 16); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 20);
+    a.seg_budget = Q; a.qout = cq; a.qout_count = qcount;
+    a.cq_tail = (unsigned long long*)(ctr + 16); a.cq_head = (unsigned long long*)(ctr + 24);
+    a.cq_done = (unsigned*)(ctr + 32); a.cq_total = (unsigned)n; a.cq_error = (unsigned*)(ctr + 36);
     a.cq_mask = (unsigned)(qcap - 1ull); a.cq_shift = qshift;
   }
   timing_begin(st);
@@ -243,7 +245,15 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
       e = cudaGetLastError();
     }
   }
+  unsigned cq_err = 0;
+  if (Q && e == cudaSuccess) {
+    // the in-kernel queue can give up (a lost record would otherwise hang the device): that must not pass for
+    // success, so a call that used it reads the flag back and therefore synchronises its stream
+    e = cudaMemcpyAsync(&cq_err, ctr + 36, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
   cleanup();
+  if (e == cudaSuccess && cq_err) return STREAMI_E_CUDA;
   return check(e);
 }
 

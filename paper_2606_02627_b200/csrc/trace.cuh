@@ -49,7 +49,8 @@ struct TraceArgs {
   // brick outputs
   QRec* qout; unsigned* qout_count;
   // in-kernel continuation queue (trace_kernel.cuh, INQ): qout, zero-initialised, is consumed by the same launch
-  unsigned* cq_head;               // next index to claim
+  unsigned long long* cq_tail;     // next ring position to publish at (64-bit: positions never wrap)
+  unsigned long long* cq_head;     // next ring position to claim
   unsigned* cq_done;               // particles terminated so far
   unsigned cq_total;               // the launch ends when cq_done reaches this (the particles it was given)
   unsigned* cq_error;              // set if a warp gave up waiting (never, unless a record was lost)

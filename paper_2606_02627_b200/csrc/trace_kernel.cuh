@@ -36,28 +36,30 @@ __device__ __forceinline__ void emit_outgoing(const TraceArgs& a, Lane& L, int d
   flush_vertices<trace_block(INTEG)>(a, L);
   int lane = threadIdx.x & 31;
   int leader = __ffs(mask) - 1;
-  unsigned base = 0;
-  if (lane == leader) base = atomicAdd(a.qout_count, (unsigned)__popc(mask));
-  base = __shfl_sync(mask, base, leader);
-  unsigned pos = base + __popc(mask & ((1u << lane) - 1u));
   QRec r; r.px = L.px; r.py = L.py; r.pz = L.pz; r.id = L.id; r.n = L.n; r.brick = (unsigned)dest;
   r.pad0 = 0; r.pad1 = 0;
   if (INTEG == 1) { r.pad0 = __float_as_uint(L.t); r.pad1 = __float_as_uint(L.h); }
   else { r.pad0 = L.slot; r.pad1 = L.rec_cd; }     // RK4: the writer's position, so that the pick-up needs no division
   if (INQ) {
-    // Ring slot pos & mask, two self-validating halves, each ONE aligned 16-byte store: both carry
-    // the tag (pos >> shift) + 1 of this pass through the ring (the memory starts zeroed, tags start
-    // at 1).  No fence: a gpu-scope fence invalidates the SM's L1 and with it the lines the cell
-    // prefetcher has just brought in (measured: L1 hit rate 47 -> 12 %, C2 15.7 -> 18.8 ms with
-    // __threadfence + a flag word).
-    uint4* q = reinterpret_cast<uint4*>(a.qout + (pos & a.cq_mask));
-    const unsigned tag = (pos >> a.cq_shift) + 1u;
-    asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(q), "r"(__float_as_uint(r.px)),
-                 "r"(__float_as_uint(r.py)), "r"(__float_as_uint(r.pz)), "r"(tag) : "memory");
-    asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(q + 1), "r"(r.id), "r"(r.n), "r"(r.brick),
-                 "r"(tag) : "memory");
+    // Ring slot pos & mask.  The payload {px, py, pz, id | n, brick} goes out with plain stores; the
+    // record is PUBLISHED by a release store (gpu scope) of the tag word, (pos >> shift) + 1 = the pass
+    // through the ring (the memory starts zeroed, tags start at 1).  The consumer reads the tag with an
+    // acquire load before it touches the payload (PTX memory model: release / acquire pattern on one
+    // word; nothing relies on the atomicity of a vector store).
+    unsigned long long base = 0;
+    if (lane == leader) base = atomicAdd(a.cq_tail, (unsigned long long)__popc(mask));
+    base = __shfl_sync(mask, base, leader);
+    const unsigned long long pos = base + __popc(mask & ((1u << lane) - 1u));
+    unsigned* q = reinterpret_cast<unsigned*>(a.qout + (pos & (unsigned long long)a.cq_mask));
+    const unsigned tag = (unsigned)(pos >> a.cq_shift) + 1u;
+    *reinterpret_cast<uint4*>(q) = make_uint4(__float_as_uint(r.px), __float_as_uint(r.py), __float_as_uint(r.pz), r.id);
+    *reinterpret_cast<uint2*>(q + 4) = make_uint2(r.n, r.brick);
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(q + 7), "r"(tag) : "memory");
   } else {
-    a.qout[pos] = r;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(a.qout_count, (unsigned)__popc(mask));
+    base = __shfl_sync(mask, base, leader);
+    a.qout[base + __popc(mask & ((1u << lane) - 1u))] = r;
   }
   // |Q_r+1[dest]| counts every queued particle; with a step budget per round (the paper's
   // one-step rounds) that includes particles that stay in their brick.  The log holds brick
@@ -99,14 +101,14 @@ template <> struct TraceCache<true> { typedef CellCacheT type; };
 // the lane keeps its index and looks again in the next iteration, so a warp whose other lanes hold
 // particles (one of which may be the producer) keeps stepping.  The launch ends when every
 // particle has terminated (`cq_done` == `cq_total`).
-__device__ __forceinline__ unsigned ld_volatile_u32(const unsigned* p) {
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {      // strong (L2-coherent) load, no ordering
   unsigned v;
-  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ uint4 ld_volatile_v4(const uint4* p) {
-  uint4 v;
-  asm volatile("ld.volatile.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {      // orders every later access after it
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
 
@@ -126,9 +128,9 @@ trace_kernel(const TraceArgs a) {
   int my_brick = 0;
   bool active = false, exhausted = false;
   unsigned n_samples = 0, n_attempts = 0, n_start = 0, budget = 0;
-  unsigned pend = 0xffffffffu;    // INQ: claimed queue index whose record is not published yet
+  unsigned long long pend = ~0ull; // INQ: claimed ring position whose record is not published yet
   bool term = false;              // INQ: this lane's particle terminated since the last count
-  unsigned spins = 0;             // INQ: polls of a warp with nothing to do
+  unsigned spins = 0, seen_done = 0;   // INQ: polls of an idle warp since the launch last made progress
 
   for (;;) {
     if (INQ) {
@@ -208,26 +210,31 @@ trace_kernel(const TraceArgs a) {
       }
     }
     if (INQ) {
-      // seeds are dry for this lane: claim a queue index (one atomic per warp), take the record once published
-      const unsigned want = __ballot_sync(FULL, !active && exhausted && pend == 0xffffffffu);
+      // seeds are dry for this lane: claim a queue position (one atomic per warp), take the record once published
+      const unsigned want = __ballot_sync(FULL, !active && exhausted && pend == ~0ull);
       if (want) {
         const int leader = __ffs(want) - 1;
-        unsigned base = 0;
-        if (lane == leader) base = atomicAdd(a.cq_head, (unsigned)__popc(want));
+        unsigned long long base = 0;
+        if (lane == leader) base = atomicAdd(a.cq_head, (unsigned long long)__popc(want));
         base = __shfl_sync(FULL, base, leader);
-        if (!active && exhausted && pend == 0xffffffffu) pend = base + __popc(want & ((1u << lane) - 1u));
+        if (!active && exhausted && pend == ~0ull) pend = base + __popc(want & ((1u << lane) - 1u));
       }
-      uint4 r0 = make_uint4(0u, 0u, 0u, 0u), r1 = r0;
-      const bool look = !active && pend != 0xffffffffu;
-      if (look) {
-        const uint4* q = reinterpret_cast<const uint4*>(a.qout + (pend & a.cq_mask));
-        r0 = ld_volatile_v4(q);
-        r1 = ld_volatile_v4(q + 1);
-      }
-      const unsigned tag = (pend >> a.cq_shift) + 1u;
-      if (look && r0.w == tag && r1.w == tag) {        // both halves written in this pass of the ring
+      const bool look = !active && pend != ~0ull;
+      const unsigned* q = reinterpret_cast<const unsigned*>(a.qout + (pend & (unsigned long long)a.cq_mask));
+      const unsigned tag = (unsigned)(pend >> a.cq_shift) + 1u;
+      // Poll with a relaxed load (an acquire load at gpu scope invalidates the SM's L1, and with it the
+      // cells the prefetcher has brought in: not on every poll); once the tag of this pass is there, the
+      // acquire load of the same word orders the payload reads behind the publisher's release store.
+      const unsigned seen = look ? ld_relaxed_u32(q + 7) : 0u;
+      // a tag of a LATER pass means the ring was lapped before this record was read (its size makes that impossible:
+      // at most cq_total records are queued at any time and the ring holds twice that); never read on silently
+      if (look && (int)(seen - tag) > 0) atomicExch(a.cq_error, 1u);
+      if (look && seen == tag && ld_acquire_u32(q + 7) == tag) {
+        uint4 r0; uint2 r1;            // after the acquire: plain (weak) loads are ordered behind it
+        asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r0.x), "=r"(r0.y), "=r"(r0.z), "=r"(r0.w) : "l"(q) : "memory");
+        asm volatile("ld.global.v2.u32 {%0,%1}, [%2];" : "=r"(r1.x), "=r"(r1.y) : "l"(q + 4) : "memory");
         L.px = __uint_as_float(r0.x); L.py = __uint_as_float(r0.y); L.pz = __uint_as_float(r0.z);
-        L.id = r1.x; L.n = r1.y; my_brick = (int)r1.z;
+        L.id = r0.w; L.n = r1.x; my_brick = (int)r1.y;
         if (BRICK) {
           st = a.bricks[my_brick];
           if (!a.brick_fast) { st.fastx = 0u; st.fasty = 0u; st.fastz = 0u; }
@@ -237,20 +244,25 @@ trace_kernel(const TraceArgs a) {
         L.stage0 = L.slot;
         n_samples = 0; n_attempts = 0; n_start = L.n; budget = a.seg_budget;
         cc.invalidate(); L.pf = 0xffffffffu;
-        pend = 0xffffffffu; active = true; spins = 0;
+        pend = ~0ull; active = true;
       }
     }
     if (__all_sync(FULL, !active)) {
       if (__all_sync(FULL, exhausted)) {
         if (!INQ) break;
         unsigned dn = 0;
-        if (lane == 0) dn = ld_volatile_u32(a.cq_done);
+        if (lane == 0) dn = ld_relaxed_u32(a.cq_done);
         dn = __shfl_sync(FULL, dn, 0);
         if (dn >= a.cq_total && !__any_sync(FULL, term)) break;
-        // A warp that has nothing to do polls ~5 times per microsecond; 2^27 polls (half a minute) without the launch
-        // ending means a record was lost (it cannot be, see the ring's size in the host code): give
-        // up loudly instead of hanging the device.
-        if (++spins > (1u << 27)) { if (lane == 0) atomicExch(a.cq_error, 1u); break; }
+        // An idle warp polls ~5 times per microsecond.  2^26 polls (a quarter of a minute) during which NO particle
+        // of the whole launch terminated means a record was lost (it cannot be, see the ring's size in the
+        // host code): give up loudly instead of hanging the device.  Progress anywhere restarts the count, so a
+        // long launch with a few stragglers is never cut short.
+        if (dn != seen_done) { seen_done = dn; spins = 0; }
+        if (++spins > (1u << 26)) { if (lane == 0) atomicExch(a.cq_error, 1u); break; }
+        unsigned er = 0;
+        if (lane == 0) er = ld_relaxed_u32(a.cq_error);
+        if (__shfl_sync(FULL, er, 0)) break;                 // some warp has given up: end the launch, the host reports it
         __nanosleep(200);
       }
       continue;

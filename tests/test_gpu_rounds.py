@@ -246,6 +246,63 @@ def test_bricks_one_launch_ring(S, torch, oracle, wl, nb, N, layout, q, mode):
     assert np.array_equal(totals.cpu().numpy().astype(np.uint64), ref.totals)
 
 
+_RING_STRESS = {}
+
+
+@pytest.mark.parametrize("q", [1, 2, 3, 4])
+def test_ring_stress_many_passes(S, torch, oracle, wl, q):
+    """Stress test of the in-kernel hand-off ring (release / acquire publication, trace_kernel.cuh): one launch,
+    every particle re-queued every q steps, so the ring of 2^19 records is passed through several hundred times
+    (tags run to several hundred) while all SMs publish and claim at once; repeated 20 times, every per-particle
+    output bit-compared with the oracle each time.  A torn or lost record would show as a wrong step count or
+    position, a lapped ring or a stalled launch as an error return."""
+    N, nb, n = 48, (2, 2, 2), 1 << 18
+    # rigid rotation about the vertical axis through the centre (speed 1 at the rim) plus a slow vertical drift that
+    # reverses at mid height: particles circle through the four brick columns until max_steps, so the work is long
+    # and every particle changes brick again and again
+    c = (N - 1) / 2.0
+    z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    data = np.zeros((1, N, N, N, 3), dtype=np.float32)
+    data[0, ..., 0] = -(y - c) / c; data[0, ..., 1] = (x - c) / c; data[0, ..., 2] = 0.05 * np.sin(2 * np.pi * z / (N - 1))
+    fld = wl.Field((N, N, N), (0.0, 0.0, 0.0), (1.0, 1.0, 1.0), data)
+    seeds = wl.seeds_uniform(7, n, [N - 1.0] * 3)
+    kw = dict(integrator=0, h=0.25, max_steps=1600, vmin=1e-6, capacity=16, stride=128)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    if "ref" not in _RING_STRESS:
+        _RING_STRESS["ref"] = oracle.brick_advect(bricks, nb, seeds, oracle.params(**kw), "f32")
+    ref = _RING_STRESS["ref"]
+    assert int(ref.totals[1]) // q > 100 * (1 << 19)            # the ring of 2^19 records is lapped hundreds of times
+    assert int(ref.totals[3]) > 4 * n                           # and real hand-offs are plentiful
+    arrays = [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nb, 1)]
+    f = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, 1, arrays, 0)
+    d_seeds = torch.from_numpy(seeds).cuda()
+    S.streami_set_option("brick_round_steps", -2)
+    S.streami_set_option("queue_steps", q)
+    try:
+        for rep in range(20):
+            verts = torch.full((3, n, 16), float("nan"), dtype=torch.float32, device="cuda")
+            counts = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+            steps = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+            status = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+            final = torch.zeros((3, n), dtype=torch.float32, device="cuda")
+            totals = torch.zeros(4, dtype=torch.int64, device="cuda")
+            prm = S.params(out_steps=steps, out_status=status, out_final=final, out_totals=totals, **kw)
+            nrounds, truncated = S.streami_brick_advect(f, d_seeds, prm, verts, counts)
+            torch.cuda.synchronize()
+            assert nrounds == 1 and not truncated
+            assert np.array_equal(status.cpu().numpy().astype(np.uint32), ref.status), rep
+            assert np.array_equal(steps.cpu().numpy().astype(np.uint32), ref.steps), rep
+            assert np.array_equal(counts.cpu().numpy().astype(np.uint32), ref.counts), rep
+            assert np.array_equal(final.cpu().numpy().view(np.uint32), ref.final.view(np.uint32)), rep
+            assert np.array_equal(verts.cpu().numpy().view(np.uint32), ref.vertices.view(np.uint32)), rep
+            assert np.array_equal(totals.cpu().numpy().astype(np.uint64)[:3], ref.totals[:3]), rep
+    finally:
+        S.streami_set_option("brick_round_steps", 0)
+        S.streami_set_option("queue_steps", 0)
+
+
 @pytest.mark.parametrize("k", [1, 7])
 def test_bricks_paper_step_rounds(S, torch, oracle, wl, k):
     """the paper's schedule (every particle re-queued after every RK step,
