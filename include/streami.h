@@ -68,6 +68,11 @@ extern "C" {
                                       aligned sector per trilinear row */
 #define STREAMI_LAYOUT_XYQUAD  5   /* library-owned copy, 64 B per vertex: the XPAIR rows (x, y) and (x, y+1):
                                       a cell is two aligned 64-byte pieces (4x the packed size) */
+#define STREAMI_LAYOUT_SOA     6   /* library-owned copy, three component planes of fp32 (12 B per vertex); a comparison
+                                      layout: measured and rejected, kept selectable */
+#define STREAMI_LAYOUT_TEX     7   /* library-owned float4 copy read through a texture object in POINT mode (tex1Dfetch,
+                                      lerps in registers); comparison layout, measured and rejected; INVALID for
+                                      stores of more texels than a linear texture holds */
 #define STREAMI_LAYOUT_CELL    4   /* library-owned copy, 128 B per CELL: its 8 corner vertices in one
                                       aligned L2 line (10.7x the packed size) */
 

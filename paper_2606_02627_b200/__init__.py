@@ -307,6 +307,29 @@ def streami_mesh_trace_streamlines_lines_host(mesh, seeds, prm_host, out_offsets
                        out_points, stream)
 
 
+class Mesh:
+    """Owner of a streami_mesh handle (hexahedral mesh field)."""
+
+    def __init__(self, X, V, H, lo, hi, nb):
+        import numpy as np
+        X = np.ascontiguousarray(X, dtype=np.float32); V = np.ascontiguousarray(V, dtype=np.float32)
+        H = np.ascontiguousarray(H, dtype=np.uint32)
+        self.handle = ctypes.c_void_p(None)
+        _check(lib().streami_mesh_create_hex(X.shape[0], H.shape[0], X.ctypes.data, V.ctypes.data, H.ctypes.data,
+                                             _f3(lo), _f3(hi), _i3(nb), ctypes.byref(self.handle)))
+
+    def destroy(self):
+        if self.handle:
+            lib().streami_mesh_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
 def streami_mesh_sample(mesh, points, stream=None):
     _req(points, torch.float32, "points")
     n = points.shape[0]

@@ -117,7 +117,7 @@ static unsigned long long layout_records(int layout, unsigned nx, unsigned ny, u
   return (unsigned long long)nx * ny * nz * nslices;
 }
 static size_t layout_record_bytes(int layout) {
-  return layout == LAYOUT_FLOAT4 ? 16 : (layout == LAYOUT_XPAIR ? 32 : (layout == LAYOUT_CELL ? 128 : (layout == LAYOUT_XYQUAD ? 64 : 12)));
+  return (layout == LAYOUT_FLOAT4 || layout == LAYOUT_TEX) ? 16 : (layout == LAYOUT_XPAIR ? 32 : (layout == LAYOUT_CELL ? 128 : (layout == LAYOUT_XYQUAD ? 64 : 12)));
 }
 
 // Build the library-owned copy of one packed float3 array (stored box nx*ny*nz, nslices slices).
@@ -131,8 +131,10 @@ static int repack(const float* src, unsigned nx, unsigned ny, unsigned nz, unsig
   void* dst = nullptr;
   STREAMI_TRY(cudaMalloc(&dst, rec * nrec + 32));   // +32: FLOAT4 reads p[1] of the last vertex
   int blocks = 148 * 8;
-  if (layout == LAYOUT_FLOAT4)
+  if (layout == LAYOUT_FLOAT4 || layout == LAYOUT_TEX)
     repack_float4_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert);
+  else if (layout == LAYOUT_SOA)
+    repack_soa_kernel<<<blocks, 256>>>(src, (float*)dst, nvert);
   else if (layout == LAYOUT_XPAIR)
     repack_xpair_kernel<<<blocks, 256>>>(src, (float4*)dst, nvert, nx);
   else if (layout == LAYOUT_XYQUAD)
@@ -145,6 +147,24 @@ static int repack(const float* src, unsigned nx, unsigned ny, unsigned nz, unsig
   if (e == cudaSuccess) e = cudaStreamSynchronize(0);
   if (e != cudaSuccess) { cudaFree(dst); return check(e); }
   *out = dst; *bytes = rec * nrec + 32;
+  return STREAMI_OK;
+}
+
+// LAYOUT_TEX: a texture object in point mode over the float4 copy (tex1Dfetch).  A linear texture holds at most
+// maxTexture1DLinear texels; larger stores are refused (INVALID).
+static int make_texture(void* data, unsigned long long nvert, unsigned long long* tex) {
+  int dev = 0, lim = 0;
+  STREAMI_TRY(cudaGetDevice(&dev));
+  STREAMI_TRY(cudaDeviceGetAttribute(&lim, cudaDevAttrMaxTexture1DLinearWidth, dev));
+  if (nvert + 2 > (unsigned long long)lim) return STREAMI_E_INVALID;
+  cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
+  rd.resType = cudaResourceTypeLinear; rd.res.linear.devPtr = data;
+  rd.res.linear.desc = cudaCreateChannelDesc<float4>(); rd.res.linear.sizeInBytes = 16ull * (nvert + 2);
+  cudaTextureDesc td; memset(&td, 0, sizeof(td));
+  td.filterMode = cudaFilterModePoint; td.readMode = cudaReadModeElementType; td.addressMode[0] = cudaAddressModeClamp;
+  cudaTextureObject_t t = 0;
+  STREAMI_TRY(cudaCreateTextureObject(&t, &rd, &td, nullptr));
+  *tex = (unsigned long long)t;
   return STREAMI_OK;
 }
 
@@ -207,7 +227,7 @@ static int scan_tame(const float* dev_ptr, unsigned long long n, bool* tame) {
 static int pick_layout(int hint) {
   if (hint == STREAMI_LAYOUT_AUTO) return 0;              // decided per stored array (auto_layout)
   if (hint == STREAMI_LAYOUT_PACKED3 || hint == STREAMI_LAYOUT_FLOAT4 || hint == STREAMI_LAYOUT_XPAIR ||
-      hint == STREAMI_LAYOUT_CELL || hint == STREAMI_LAYOUT_XYQUAD)
+      hint == STREAMI_LAYOUT_CELL || hint == STREAMI_LAYOUT_XYQUAD || hint == STREAMI_LAYOUT_SOA || hint == STREAMI_LAYOUT_TEX)
     return hint;
   return -1;
 }
@@ -259,13 +279,21 @@ int streami_field_create(const int dims[3], const float origin[3], const float s
   f->layout = layout;
   if (rc) { delete f; return rc; }
   f->tame = false;
-  if (nslices == 1) {                 // only the steady paths ask
+  // PACKED3 reads the caller's BORROWED array live (the in-situ use the paper targets): the
+  // application may write NaN or Inf into it after this scan, so the integer accept is not licensed there.
+  if (nslices == 1 && layout != LAYOUT_PACKED3) {                 // only the steady paths ask
     rc = scan_tame(dev_ptr, 3ull * s.slice_stride, &f->tame);
     if (rc) { if (bytes) cudaFree(data); delete f; return rc; }
   }
   if (layout == LAYOUT_CELL) cell_strides(s, (unsigned)dims[0], (unsigned)dims[1], (unsigned)dims[2]);
   s.data = data;
+  s.plane = s.slice_stride * (unsigned long long)nslices; s.tex = 0ull;
   if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
+  if (layout == LAYOUT_TEX) {
+    rc = make_texture(data, s.slice_stride * (unsigned long long)nslices, &s.tex);
+    if (rc) { cudaFree(data); delete f; return rc; }
+    f->textures.push_back(s.tex);
+  }
   *out = f;
   return STREAMI_OK;
 }
@@ -299,6 +327,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
   m.Bx = global_dims[0] / m.nbx; m.By = global_dims[1] / m.nby; m.Bz = global_dims[2] / m.nbz;
   const int B[3] = {m.Bx, m.By, m.Bz};
   auto fail = [&](int code) {
+    for (unsigned long long t : f->textures) cudaDestroyTextureObject((cudaTextureObject_t)t);
     for (void* p : f->owned) cudaFree(p);
     delete f;
     return code;
@@ -345,10 +374,18 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
         if (rc) return fail(rc);
         if (layout == LAYOUT_CELL) cell_strides(s, bnx, bny, bnz);
         s.data = data;
+        s.plane = s.slice_stride; s.tex = 0ull;
         if (bytes) { f->owned.push_back(data); f->owned_bytes += bytes; }
+        if (layout == LAYOUT_TEX) {
+          rc = make_texture(data, s.slice_stride, &s.tex);
+          if (rc) return fail(rc);
+          f->textures.push_back(s.tex);
+        }
         bool brick_tame = false;
-        rc = scan_tame(src, 3ull * bnx * bny * bnz, &brick_tame);
-        if (rc) return fail(rc);
+        if (layout != LAYOUT_PACKED3) {      // a borrowed array can change after the scan (see streami_field_create)
+          rc = scan_tame(src, 3ull * bnx * bny * bnz, &brick_tame);
+          if (rc) return fail(rc);
+        }
         f->tame = f->tame && brick_tame;
         f->bricks.push_back(s);
       }
@@ -369,6 +406,7 @@ int streami_field_create_bricked(const int global_dims[3], const float origin[3]
 
 int streami_field_destroy(streami_field f) {
   if (!f) return STREAMI_E_INVALID;
+  for (unsigned long long t : f->textures) cudaDestroyTextureObject((cudaTextureObject_t)t);
   for (void* p : f->owned) cudaFree(p);
   delete f;
   return STREAMI_OK;
@@ -402,7 +440,11 @@ int streami_sample(streami_field f, const float* points, size_t n, float t, int 
     case LAYOUT_CELL * 2: GO(LAYOUT_CELL, false); break;
     case LAYOUT_CELL * 2 + 1: GO(LAYOUT_CELL, true); break;
     case LAYOUT_XYQUAD * 2: GO(LAYOUT_XYQUAD, false); break;
-    default: GO(LAYOUT_XYQUAD, true); break;
+    case LAYOUT_XYQUAD * 2 + 1: GO(LAYOUT_XYQUAD, true); break;
+    case LAYOUT_SOA * 2: GO(LAYOUT_SOA, false); break;
+    case LAYOUT_SOA * 2 + 1: GO(LAYOUT_SOA, true); break;
+    case LAYOUT_TEX * 2: GO(LAYOUT_TEX, false); break;
+    default: GO(LAYOUT_TEX, true); break;
   }
 #undef GO
   STREAMI_LAUNCHED();

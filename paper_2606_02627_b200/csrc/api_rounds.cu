@@ -32,6 +32,8 @@ static StreakKernel pick_streak(int layout, bool unsteady, bool tcache) {
     case LAYOUT_FLOAT4: return pick_streak_l<LAYOUT_FLOAT4>(unsteady, tcache);
     case LAYOUT_CELL: return pick_streak_l<LAYOUT_CELL>(unsteady, tcache);
     case LAYOUT_XYQUAD: return pick_streak_l<LAYOUT_XYQUAD>(unsteady, tcache);
+    case LAYOUT_SOA: return pick_streak_l<LAYOUT_SOA>(unsteady, tcache);
+    case LAYOUT_TEX: return pick_streak_l<LAYOUT_TEX>(unsteady, tcache);
     default: return pick_streak_l<LAYOUT_XPAIR>(unsteady, tcache);
   }
 }
@@ -222,7 +224,7 @@ int streami_streak_end(streami_streak h, unsigned* out_counts, void* cuda_stream
   if (!h) return STREAMI_E_INVALID;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t e = cudaSuccess;
-  if (out_counts) {
+  if (out_counts || h->out_status) {       // out_counts may be NULL; params->out_status is written either way
     streak_finalize_kernel<<<(unsigned)((h->a.m + 255) / 256), 256, 0, st>>>(h->a.state, h->a.m, h->a.nsteps, h->done,
                                                                              out_counts, h->out_status);
     launch_counter()++;
@@ -297,7 +299,8 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   const bool cache = options().cell_cache != 0;
   // brick_round_steps = -2: one launch with the in-kernel ring instead of rounds (measured on C3: 158 ms
   // against 157 ms for sorted rounds -- the Morton sort of every round is worth what the rounds cost)
-  if (options().brick_round_steps == -2 && !out_round_counts && !out_handoff_log && params->integrator == 0 && cache)
+  const bool ring_ok = f->layout != LAYOUT_SOA && f->layout != LAYOUT_TEX;    // the comparison layouts have no ring kernels
+  if (options().brick_round_steps == -2 && !out_round_counts && !out_handoff_log && params->integrator == 0 && cache && ring_ok)
     return brick_advect_inq(f, seeds, n, params, out_vertices, out_counts, out_nrounds, st);
   TraceKernel k = pick_trace_kernel(f->layout, params->integrator, false, true, cache, unit_geometry(f->g));
   const int block = trace_block(params->integrator);
@@ -364,7 +367,7 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   // waits for its slowest particle -- is finished by ONE launch that consumes its own hand-off ring
   // (trace_kernel.cuh, INQ).
   const bool ring_finish = options().brick_round_steps == 0 && !out_round_counts && !out_handoff_log &&
-                           params->integrator == 0 && cache;
+                           params->integrator == 0 && cache && ring_ok;
   for (;;) {
     a.round = (int)round; a.nwork = nwork;
     a.qin = round ? q[round & 1] : nullptr; a.qout = q[(round + 1) & 1];
@@ -513,7 +516,8 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
     Mirror mr(st);
     streami_params dp = *params;
     float* d_seeds = (float*)mr.make(seeds, nullptr, 3 * n * sizeof(float));
-    float* d_v = (float*)mr.make(nullptr, out_vertices, 3 * n * (size_t)params->capacity * sizeof(float));
+    // slots beyond out_counts stay untouched (A6): the mirror starts as the caller's array
+    float* d_v = (float*)mr.make(out_vertices, out_vertices, 3 * n * (size_t)params->capacity * sizeof(float));
     unsigned* d_c = (unsigned*)mr.make(nullptr, out_counts, n * sizeof(unsigned));
     // the round table is only partly written by the call: upload the caller's content first
     unsigned* d_rc = (unsigned*)mr.make(out_round_counts, out_round_counts, (size_t)max_rounds * nb * sizeof(unsigned));

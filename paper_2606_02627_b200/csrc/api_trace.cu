@@ -33,6 +33,8 @@ TraceKernel pick_trace_kernel(int layout, int integ, bool unsteady, bool brick, 
     case LAYOUT_FLOAT4: return pick_l<LAYOUT_FLOAT4>(integ, unsteady, brick, cache, unit);
     case LAYOUT_CELL: return pick_l<LAYOUT_CELL>(integ, unsteady, brick, cache, unit);
     case LAYOUT_XYQUAD: return pick_l<LAYOUT_XYQUAD>(integ, unsteady, brick, cache, unit);
+    case LAYOUT_SOA: return pick_l<LAYOUT_SOA>(integ, unsteady, brick, cache, unit);
+    case LAYOUT_TEX: return pick_l<LAYOUT_TEX>(integ, unsteady, brick, cache, unit);
     default: return pick_l<LAYOUT_XPAIR>(integ, unsteady, brick, cache, unit);
   }
 }
@@ -129,7 +131,7 @@ int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
   // is queued at most floor(max_steps / Q) times, which sizes the queue; if that does not fit, the
   // launch runs without.
   unsigned Q = 0;
-  if (!dp5 && !unsteady && cache && K == 0 && options().queue_steps > 0) {
+  if (!dp5 && !unsteady && cache && K == 0 && options().queue_steps > 0 && f->layout != LAYOUT_SOA && f->layout != LAYOUT_TEX) {
     Q = (unsigned)options().queue_steps;
     if (Q >= params->max_steps) Q = 0;
   }
@@ -289,13 +291,14 @@ int streami_trace_streamlines_host(streami_field f, const float* seeds, size_t n
   if (e == cudaSuccess && params->out_final) e = alloc((void**)&d_final, 3 * n * sizeof(float));
   if (e == cudaSuccess && params->out_totals) e = alloc((void**)&d_totals, 4 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_seeds, seeds, 3 * n * sizeof(float), cudaMemcpyHostToDevice, st);
+  // Slots beyond out_counts are "left untouched" (A6): the device mirror starts as a copy of the caller's array, so
+  // that the download below returns the caller's own values there, not whatever the allocator handed out.
+  if (e == cudaSuccess && nv) e = cudaMemcpyAsync(d_verts, out_vertices, nv * sizeof(float), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) { cleanup(); return check(e); }
   streami_params dp = *params;
   dp.out_steps = d_steps; dp.out_status = d_status; dp.out_final = d_final; dp.out_totals = d_totals;
   rc = streami_trace_streamlines(f, d_seeds, n, &dp, d_verts, d_counts, cuda_stream);
   if (rc) { cleanup(); return rc; }
-  // Slots beyond out_counts are "left untouched" on the device copy; the host array receives
-  // the device array as is (its untouched slots hold whatever the allocator returned).
   e = cudaMemcpyAsync(out_counts, d_counts, n * sizeof(unsigned), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess && nv) e = cudaMemcpyAsync(out_vertices, d_verts, nv * sizeof(float), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess && d_steps) e = cudaMemcpyAsync(params->out_steps, d_steps, n * sizeof(unsigned), cudaMemcpyDeviceToHost, st);

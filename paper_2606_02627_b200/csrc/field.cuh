@@ -12,7 +12,7 @@
 
 namespace streami {
 
-enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3, LAYOUT_CELL = 4, LAYOUT_XYQUAD = 5 };
+enum : int { LAYOUT_PACKED3 = 1, LAYOUT_FLOAT4 = 2, LAYOUT_XPAIR = 3, LAYOUT_CELL = 4, LAYOUT_XYQUAD = 5, LAYOUT_SOA = 6, LAYOUT_TEX = 7 };
 enum : unsigned { ST_ALIVE = 0, ST_OUT = 1, ST_MAXSTEPS = 2, ST_STAGNANT = 3, ST_HALO = 4 };
 
 // Global geometry (A1), uniform over the launch.
@@ -47,6 +47,8 @@ struct Store {
   // `self` when wanted instead of staying live (the brick kernel is short of registers).
   const Store* self;
   unsigned long long slice_stride;   // records per slice
+  unsigned long long plane;          // LAYOUT_SOA: floats per component plane (all slices)
+  unsigned long long tex;            // LAYOUT_TEX: cudaTextureObject_t over the float4 copy (point mode, tex1Dfetch)
 };
 
 // A brick grid (A9): owner of an in-domain position.
@@ -141,9 +143,30 @@ template <> struct CellLoad<LAYOUT_XYQUAD> {
   }
 };
 
+// LAYOUT_SOA: three component planes of fp32 (the other layout north_star names): a row is 2 floats from
+// each of three planes, a cell 24 scalar loads from 12 distant sectors.  LAYOUT_TEX: the FLOAT4 copy read
+// through a texture object in POINT mode (tex1Dfetch; the lerps stay in registers, A2 -- hardware filtering
+// has 8-bit weights).  Both exist so that the layout choice is settled by measurement.
+template <int LAYOUT>
+__device__ __forceinline__ void load_row_alt(const Store& s, unsigned long long v, float* o) {
+  if constexpr (LAYOUT == LAYOUT_SOA) {
+    const float* p = reinterpret_cast<const float*>(s.data) + v;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { o[c] = __ldg(p + c * s.plane); o[3 + c] = __ldg(p + c * s.plane + 1); }
+  } else {
+    const float4 a = tex1Dfetch<float4>((cudaTextureObject_t)s.tex, (int)v);
+    const float4 b = tex1Dfetch<float4>((cudaTextureObject_t)s.tex, (int)v + 1);
+    o[0] = a.x; o[1] = a.y; o[2] = a.z; o[3] = b.x; o[4] = b.y; o[5] = b.z;
+  }
+}
+template <int LAYOUT> struct AltLayout { static constexpr bool value = LAYOUT == LAYOUT_SOA || LAYOUT == LAYOUT_TEX; };
+
 template <int LAYOUT>
 __device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, float* V) {
-  if constexpr (LAYOUT == LAYOUT_CELL) {
+  if constexpr (AltLayout<LAYOUT>::value) {
+    load_row_alt<LAYOUT>(s, v, V); load_row_alt<LAYOUT>(s, v + s.nx, V + 6);
+    load_row_alt<LAYOUT>(s, v + s.nxy, V + 12); load_row_alt<LAYOUT>(s, v + s.nxy + s.nx, V + 18);
+  } else if constexpr (LAYOUT == LAYOUT_CELL) {
     CellLoad<LAYOUT_CELL>::template cell<false>(s.data, v, V);
   } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
     CellLoad<LAYOUT_XYQUAD>::template pair<false>(s.data, v, V);
@@ -160,7 +183,9 @@ __device__ __forceinline__ void load_cell(const Store& s, unsigned long long v, 
 // indices fit 32 bits (v + nxy + nx <= nvert - 1) and each address is one 32x32->64 multiply-add.
 template <int LAYOUT, bool NA = false>
 __device__ __forceinline__ void load_cell32(const Store& s, unsigned v, float* V) {
-  if constexpr (LAYOUT == LAYOUT_CELL) {
+  if constexpr (AltLayout<LAYOUT>::value) {
+    load_cell<LAYOUT>(s, (unsigned long long)v, V);
+  } else if constexpr (LAYOUT == LAYOUT_CELL) {
     CellLoad<LAYOUT_CELL>::template cell<NA>(s.data, v, V);
   } else if constexpr (LAYOUT == LAYOUT_XYQUAD) {
     CellLoad<LAYOUT_XYQUAD>::template pair<NA>(s.data, v, V);
@@ -443,7 +468,9 @@ __device__ __forceinline__ void prefetch_sector(const void* gptr, unsigned smem_
 
 template <int LAYOUT>
 __device__ __forceinline__ void prefetch_cell32(const Store& s, unsigned v, unsigned smem_addr) {
-  if constexpr (LAYOUT == LAYOUT_CELL) {
+  if constexpr (AltLayout<LAYOUT>::value) {
+    return;                                  // comparison layouts: no prefetcher
+  } else if constexpr (LAYOUT == LAYOUT_CELL) {
     const char* p = reinterpret_cast<const char*>(s.data) + 128ull * v;
 #pragma unroll
     for (int r = 0; r < 3; ++r) prefetch_sector(p + 32 * r, smem_addr);

@@ -122,8 +122,10 @@ int lines_host(Trace&& trace, bool one_batch, const float* seeds, size_t n, cons
           e = cudaMemcpyAsync(params->out_final + c * n + s0, d_fin + c * nb, nb * sizeof(float), cudaMemcpyDeviceToHost, cs);
         if (e != cudaSuccess) rc = check(e);
       }
-      if (d_pts) cudaFreeAsync(d_pts, cs);
-      if (d_fin) cudaFreeAsync(d_fin, cs);
+      // freed on the copy stream only if that stream was made to wait for the tracing stream above (rc == OK);
+      // on an error path the tracing stream itself frees them, in order behind the kernels that write them
+      if (d_pts) cudaFreeAsync(d_pts, rc == STREAMI_OK ? cs : st);
+      if (d_fin) cudaFreeAsync(d_fin, rc == STREAMI_OK ? cs : st);
       total += tb;
     }
     if (cs != st) {                               // the caller's stream covers the copies as well

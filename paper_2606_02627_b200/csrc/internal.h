@@ -18,6 +18,7 @@ struct streami_field_s {
   streami::Store* d_bricks;          // device table
   streami::BrickMap bm;
   std::vector<void*> owned;          // device allocations owned by the handle
+  std::vector<unsigned long long> textures;   // texture objects owned by the handle (LAYOUT_TEX)
   size_t owned_bytes;
 };
 

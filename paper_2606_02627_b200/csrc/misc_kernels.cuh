@@ -14,6 +14,16 @@ static __global__ void repack_float4_kernel(const float* __restrict__ src, float
     dst[v] = make_float4(src[3 * v], src[3 * v + 1], src[3 * v + 2], 0.0f);
 }
 
+// SOA: three component planes of nvert floats each (nvert = all vertices of all slices).
+static __global__ void repack_soa_kernel(const float* __restrict__ src, float* __restrict__ dst,
+                                         unsigned long long nvert) {
+  unsigned long long v = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
+  for (; v < nvert; v += step) {
+    dst[v] = src[3 * v]; dst[nvert + v] = src[3 * v + 1]; dst[2 * nvert + v] = src[3 * v + 2];
+  }
+}
+
 // Tame scan: *flag |= 1 if any of the n floats is NaN, infinite or above 2^60 in magnitude.
 static __global__ void tame_scan_kernel(const float* __restrict__ src, unsigned long long n, unsigned* flag) {
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -223,7 +233,7 @@ static __global__ void streak_finalize_kernel(const unsigned char* __restrict__ 
     c += (j < released) && (st == ST_MAXSTEPS || st == ST_ALIVE);
     if (status) status[(unsigned long long)j * m + i] = st;
   }
-  counts[i] = c;
+  if (counts) counts[i] = c;
 }
 
 }  // namespace streami

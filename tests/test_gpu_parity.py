@@ -29,7 +29,7 @@ def torch():
     return t
 
 
-LAYOUTS = [1, 2, 3, 4, 5]
+LAYOUTS = [1, 2, 3, 4, 5, 6, 7]
 
 
 # ---- a2-a4: the sampling layer alone -------------------------------------------------------

@@ -157,3 +157,28 @@ def test_integer_accept_keeps_the_domain_test_exact(S, torch, oracle, wl, turb48
             finally:
                 S.streami_set_option("integer_accept", 1)
             assert_same(out, ref, "%s integer_accept=%d %s" % (kind, on, kw))
+
+
+def test_packed3_array_poisoned_after_create(S, torch, oracle, wl, turb48):
+    """PACKED3 traces the caller's BORROWED array in place (the in-situ use).  If the application
+    writes NaN / Inf into it AFTER streami_field_create, the create-time scan is stale: the integer accept
+    must not be licensed for that layout, or a NaN position would be judged inside and run to MAX_STEPS
+    (ADVICE r1).  The trace of the poisoned array must equal the oracle's on the same poisoned bytes."""
+    data = turb48.data.copy()
+    dev = torch.from_numpy(data).cuda()
+    f = S.streami_field_create(turb48.dims, turb48.origin, turb48.spacing, 1, 1.0, dev, 1)
+    rng = np.random.default_rng(9)
+    idx = rng.integers(0, 48, size=(600, 3))
+    data[0, idx[:, 2], idx[:, 1], idx[:, 0], idx[:, 0] % 3] = np.where(idx[:, 1] % 2, np.nan, np.inf)
+    dev.copy_(torch.from_numpy(data))                              # the application overwrites its own array
+    n = 6000
+    seeds = wl.seeds_uniform(33, n, [47.0] * 3)
+    seeds[:400] = idx[:400] + 0.5
+    g = oracle.grid(data, turb48.dims, turb48.origin, turb48.spacing)
+    for kw in (dict(integrator=0, h=0.25, max_steps=80, vmin=1e-6, capacity=16, stride=5),
+               dict(integrator=1, h=0.25, h_min=0.01, h_max=1.0, atol=1e-4, rtol=1e-4, max_steps=60, vmin=1e-6,
+                    capacity=16, stride=5)):
+        ref = oracle.streamlines(g, seeds, oracle.params(**kw), "f32")
+        assert np.count_nonzero(ref.status == oracle.OUT_OF_DOMAIN) > 400
+        out = gpu_streamlines(S, torch, f, seeds, **kw)
+        assert_same(out, ref, "poisoned packed3 %s" % kw)
