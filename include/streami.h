@@ -161,6 +161,17 @@ int streami_trace_streaklines(streami_field f, const float* points, size_t m, un
                               const streami_params* params, float* out_vertices,
                               unsigned* out_counts, void* cuda_stream);
 
+/* Per-destination partition of seeds (A9: Q_0[b] = the seeds owned by brick b; the distribution step of a
+ * data-parallel run, where every rank receives the particles of its macrocell).
+ * out_perm [n] (device): the seed indices ordered by (owner brick, Morton code inside the brick) -- the same
+ * two-level counting sort streami_brick_advect applies to every round's hand-off queue, so that the work
+ * of a round is ONE contiguous segment per destination brick (the "send buffer" of that destination).
+ * out_offsets [nbricks + 1] (device): segment b is out_perm[out_offsets[b] .. out_offsets[b+1]).  Seeds
+ * outside the domain are listed with brick 0.  Order inside a (brick, block) bin is unspecified.
+ * Asynchronous on cuda_stream.  Errors: INVALID (null, not a bricked field, n >= 2^32), NOMEM, CUDA. */
+int streami_partition_seeds(streami_field bricked, const float* seeds, size_t n, unsigned* out_perm,
+                            unsigned long long* out_offsets, void* cuda_stream);
+
 /* Brick advection with hand-off (P1/K1/K3/K4 of SURVEY.md; A9).
  * f must come from streami_field_create_bricked; RK4 or DP5(4).  In round r every particle queued for
  * brick b is advected inside b until it ends or its new position is owned by another brick; it

@@ -54,6 +54,7 @@ def lib():
         L.streami_trace_streamlines_host.argtypes = [P, P, Z, P, P, P, P]
         L.streami_trace_streaklines.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
+        L.streami_partition_seeds.argtypes = [P, P, Z, P, P, P]
         L.streami_trace_streaklines_host.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_streak_begin.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
@@ -223,6 +224,16 @@ def streami_brick_advect(field, seeds, prm, out_vertices, out_counts, out_round_
                                            log_cap, _ptr(out_log_count), ctypes.byref(nrounds),
                                            _stream(stream)), allow=(E_TRUNCATED,))
     return nrounds.value, rc == E_TRUNCATED
+
+
+def streami_partition_seeds(field, seeds, nbricks, stream=None):
+    """(perm [n] int32 cuda, offsets [nbricks+1] int64 cuda): seeds ordered by (owner brick, Morton code)."""
+    _req(seeds, torch.float32, "seeds")
+    n = seeds.shape[0]
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    off = torch.empty(nbricks + 1, dtype=torch.int64, device="cuda")
+    _check(lib().streami_partition_seeds(field.handle, _ptr(seeds), n, _ptr(perm), _ptr(off), _stream(stream)))
+    return perm, off
 
 
 class Streak:

@@ -76,7 +76,7 @@ static int brick_advect_inq(streami_field f, const float* seeds, size_t n, const
   if (e != cudaSuccess) { cleanup(); return check(e); }
   int rc = STREAMI_OK;
   if (sorting) {
-    rc = sorter.init(f, n, st);
+    rc = sorter.init(f, n, st, true);
     if (rc) { cleanup(); return rc; }
     have_sorter = true;
     rc = sorter.sort(f->g, seeds, 3, n, nullptr, perm);
@@ -277,6 +277,22 @@ int streami_streamline_lines(const float* vertices, const unsigned* counts, size
   return rc;
 }
 
+int streami_partition_seeds(streami_field f, const float* seeds, size_t n, unsigned* out_perm,
+                            unsigned long long* out_offsets, void* cuda_stream) {
+  OptionsScope options_scope;
+  if (!f || !f->bricked || !out_offsets || (n > 0 && (!seeds || !out_perm))) return STREAMI_E_INVALID;
+  if (n > 0xffffffffull) return STREAMI_E_INVALID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const unsigned nb = (unsigned)f->bricks.size();
+  if (n == 0) return check(cudaMemsetAsync(out_offsets, 0, sizeof(unsigned long long) * (nb + 1), st));
+  MortonSorter sorter{};
+  int rc = sorter.init(f, n, st, true);
+  if (rc) return rc;
+  rc = sorter.sort(f->g, seeds, 3, n, nullptr, out_perm, out_offsets);
+  sorter.release();
+  return rc;
+}
+
 int streami_brick_advect(streami_field f, const float* seeds, size_t n,
                          const streami_params* params, float* out_vertices, unsigned* out_counts,
                          unsigned* out_round_counts, unsigned max_rounds,
@@ -353,8 +369,9 @@ int streami_brick_advect(streami_field f, const float* seeds, size_t n,
   a.qout_count = d_qcount;
   a.log = out_handoff_log; a.log_cap = log_capacity; a.log_count = d_logc;
 
-  if (sorting) {            // a12: each round's work is processed in Morton order of its positions
-    rc = sorter.init(f, n, st);
+  if (sorting) {            // a12 + a9: each round's work is ONE contiguous segment per destination brick (Q_r[b] of A9:
+                            // what a data-sharded run would send to rank b), in Morton order inside the segment
+    rc = sorter.init(f, n, st, true);
     if (rc) { cleanup(); return rc; }
     have_sorter = true;
   }

@@ -9,6 +9,8 @@
 
 namespace streami {
 
+constexpr unsigned PRESORT_SEG = 1024;   // bins per scan segment (see the scan kernels below)
+
 __device__ __forceinline__ unsigned spread3(unsigned x) {   // 10 bits -> every third bit
   x &= 0x3ffu;
   x = (x | (x << 16)) & 0x030000ffu;
@@ -29,24 +31,64 @@ __device__ __forceinline__ unsigned seed_bin(const Geom& g, int shift, const flo
   return spread3(bx) | (spread3(by) << 1) | (spread3(bz) << 2);
 }
 
+// Brick-major key (a9: per-destination segments): key = brick * 2^(3 lbits) + Morton code of the item's cell
+// block RELATIVE to its brick's owned box, so that the sorted work of a round is one contiguous range per
+// destination brick -- Q_r[b] of A9, the "send buffer" a data-sharded run would hand to rank b (PAPER.md:63-65,
+// 101) -- and Morton-ordered inside it.  The brick of a queue record is its word 5 (written by emit_outgoing),
+// the brick of a seed is its owner (A9).  Items outside the domain go to bin 0.
+__device__ __forceinline__ unsigned brick_bin(const Geom& g, const BrickMap& m, int shift, int lbits, const float* pos,
+                                              unsigned stride, unsigned long long i) {
+  float gx, gy, gz;
+  const float* p = pos + (unsigned long long)stride * i;
+  if (!to_index(g, p[0], p[1], p[2], gx, gy, gz)) return 0u;
+  const int ix = __float2int_rz(gx), iy = __float2int_rz(gy), iz = __float2int_rz(gz);
+  int bx, by, bz;
+  if (stride == 8u) {                        // queue record: destination brick as stored
+    const unsigned b = __float_as_uint(p[5]);
+    bx = (int)(b % (unsigned)m.nbx); by = (int)((b / (unsigned)m.nbx) % (unsigned)m.nby); bz = (int)(b / (unsigned)(m.nbx * m.nby));
+  } else {
+    bx = min(ix / m.Bx, m.nbx - 1); by = min(iy / m.By, m.nby - 1); bz = min(iz / m.Bz, m.nbz - 1);
+  }
+  const unsigned lim = (1u << lbits) - 1u;
+  const unsigned lx = min((unsigned)max(ix - bx * m.Bx, 0) >> shift, lim), ly = min((unsigned)max(iy - by * m.By, 0) >> shift, lim),
+                 lz = min((unsigned)max(iz - bz * m.Bz, 0) >> shift, lim);
+  const unsigned b = (unsigned)((bz * m.nby + by) * m.nbx + bx);
+  return (b << (3 * lbits)) | spread3(lx) | (spread3(ly) << 1) | (spread3(lz) << 2);
+}
+
 // The item count is `n`, or *n_dev when n_dev is set (a queue whose size only the device knows).
-static __global__ void presort_hist_kernel(Geom g, int shift, const float* __restrict__ pos, unsigned stride,
+// lbits > 0: brick-major keys (brick_bin), else plain Morton keys of the global grid.
+static __global__ void presort_hist_kernel(Geom g, BrickMap bm, int shift, int lbits, const float* __restrict__ pos, unsigned stride,
                                     unsigned long long n, const unsigned* __restrict__ n_dev,
                                     unsigned* __restrict__ hist, unsigned* __restrict__ keys) {
   if (n_dev) n = *n_dev;
   unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned long long step = (unsigned long long)gridDim.x * blockDim.x;
   for (; i < n; i += step) {
-    unsigned k = seed_bin(g, shift, pos, stride, i);
+    unsigned k = lbits > 0 ? brick_bin(g, bm, shift, lbits, pos, stride, i) : seed_bin(g, shift, pos, stride, i);
     keys[i] = k;
     atomicAdd(hist + k, 1u);
+  }
+}
+
+// Start of every brick's segment in the sorted order (brick-major keys): offsets[b] for b = 0..nb, read from the
+// exclusive scan BEFORE the scatter advances it.
+static __global__ void presort_segments_kernel(const unsigned* __restrict__ scanned, const unsigned* __restrict__ seg_base,
+                                               unsigned bins_per_brick, unsigned nbricks, unsigned long long n,
+                                               const unsigned* __restrict__ n_dev, unsigned long long* __restrict__ offsets) {
+  if (n_dev) n = *n_dev;
+  const unsigned b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < nbricks) {
+    const unsigned k = b * bins_per_brick;
+    offsets[b] = (unsigned long long)scanned[k] + seg_base[k / PRESORT_SEG];
+  } else if (b == nbricks) {
+    offsets[b] = n;
   }
 }
 
 // Exclusive scan of `hist` in two levels.  Level 1: each block scans one segment of 1024 bins in
 // place (4 consecutive bins per thread, warp shuffles, one shared-memory hop) and writes the
 // segment total.  Level 2: one block scans the <= 2048 segment totals.  The scatter adds both.
-constexpr unsigned PRESORT_SEG = 1024;
 
 static __global__ void __launch_bounds__(256)
 presort_scan_seg_kernel(unsigned* __restrict__ hist, unsigned nbins, unsigned* __restrict__ seg_total) {

@@ -246,6 +246,36 @@ def test_bricks_one_launch_ring(S, torch, oracle, wl, nb, N, layout, q, mode):
     assert np.array_equal(totals.cpu().numpy().astype(np.uint64), ref.totals)
 
 
+@pytest.mark.parametrize("nb,N", [((2, 2, 2), 32), ((3, 2, 1), 31), ((1, 1, 1), 24), ((4, 3, 2), 50)])
+def test_partition_seeds_per_destination_segments(S, torch, oracle, wl, nb, N):
+    """a9 / A9: the two-level counting sort (destination brick, Morton code inside the brick) that orders every
+    round's work.  Through streami_partition_seeds: segment b of the permutation holds exactly the seeds the
+    oracle's Q_0[b] holds (owner of the seed, A9), every seed once, segments contiguous and in brick order."""
+    fld = wl.turb_field_cpu(N, 24, 1, 4)
+    n = 70001
+    seeds = wl.seeds_uniform(5, n, [N - 1.0] * 3)
+    seeds[:50] = np.round(seeds[:50])                       # on vertices: faces belong to the upper brick
+    nbricks = nb[0] * nb[1] * nb[2]
+    arrays = [torch.from_numpy(a).cuda() for a in wl.cut_bricks(fld, nb, 1)]
+    f = S.streami_field_create_bricked(fld.dims, fld.origin, fld.spacing, nb, 1, arrays, 3)
+    perm, off = S.streami_partition_seeds(f, torch.from_numpy(seeds).cuda(), nbricks)
+    torch.cuda.synchronize()
+    perm = perm.cpu().numpy().astype(np.int64); off = off.cpu().numpy().astype(np.int64)
+    assert off[0] == 0 and off[-1] == n and np.all(np.diff(off) >= 0)
+    assert np.array_equal(np.sort(perm), np.arange(n))      # a permutation
+    B = [N // nb[a] for a in range(3)]
+    own = sum(np.minimum(np.floor(seeds[:, a]).astype(int) // B[a], nb[a] - 1) * [1, nb[0], nb[0] * nb[1]][a] for a in range(3))
+    for b in range(nbricks):
+        seg = perm[off[b]:off[b + 1]]
+        assert np.all(own[seg] == b), b
+    # the oracle's Q_0 sizes (round table, row 0)
+    boxes = wl.brick_boxes(fld.dims, nb, 1)
+    bricks = [oracle.grid(a, None, fld.origin, fld.spacing, gdims=fld.dims, lo=lo, hi=hi)
+              for a, (lo, hi) in zip(wl.cut_bricks(fld, nb, 1), boxes)]
+    ref = oracle.brick_advect(bricks, nb, seeds, oracle.params(0, h=0.25, max_steps=1, vmin=0.0, capacity=2), "f32")
+    assert np.array_equal(np.diff(off), ref.round_counts[0])
+
+
 _RING_STRESS = {}
 
 
