@@ -93,6 +93,10 @@ void fill_integrator(TraceArgs& a, const streami_params* p) {
   a.vmin2 = p->vmin * p->vmin; a.t0 = p->t0; a.max_steps = p->max_steps;
   a.cap = p->capacity; a.stride = p->stride; a.vec_ok = 0; a.staging = options().vertex_staging;
   a.prefetch = options().prefetch;
+  // RK4 phase length (trace_kernel.cuh): the largest power of two <= 8 that divides the recording stride (a vertex can
+  // then only fall due on the last step of a phase) and the step budget of a segment / round, if there is one
+  a.phase = 1u;
+  while (a.phase < 8u && p->stride % (2u * a.phase) == 0u && (a.seg_budget == 0u || a.seg_budget % (2u * a.phase) == 0u)) a.phase *= 2u;
   a.steps = p->out_steps; a.status = p->out_status; a.fin = p->out_final; a.totals = p->out_totals;
 }
 

@@ -33,6 +33,7 @@ struct TraceArgs {
   unsigned long long nwork;
   const unsigned* nwork_dev;       // if set, the work count is read from device memory instead
   unsigned seg_budget;             // step attempts per particle per launch, 0 = unlimited
+  unsigned phase;                  // RK4: steps per phase of the advection loop (power of two dividing stride; trace_kernel.cuh)
   unsigned long long* next;        // global work counter
   int round;
   // integrator (host-computed fp32 constants, A4/A8)
@@ -154,13 +155,36 @@ __device__ __forceinline__ void record_vertex(const TraceArgs& a, Lane& L) {
   }
 }
 
+// The phased loop (trace_kernel.cuh) counts rec_cd down inside the step and records at the phase boundary.
+template <int BT = REC_THREADS>
+__device__ __forceinline__ void record_due(const TraceArgs& a, Lane& L) {
+  if (L.rec_cd != 0u) return;
+  L.rec_cd = a.stride;
+  if (L.slot >= a.cap) return;
+  if (a.staging) {
+    float* s = rec_stage<BT>() + (L.slot & (REC_GROUP - 1));
+    s[0] = L.px; s[REC_GROUP] = L.py; s[2 * REC_GROUP] = L.pz;
+    L.slot++;
+    if ((L.slot & (REC_GROUP - 1)) == 0u) flush_vertices<BT>(a, L);
+  } else {
+    if (a.verts) {
+      unsigned long long o = (unsigned long long)L.id * a.cap + L.slot;
+      unsigned long long plane = a.n * a.cap;
+      a.verts[o] = L.px; a.verts[plane + o] = L.py; a.verts[2 * plane + o] = L.pz;
+    }
+    L.slot++; L.stage0 = L.slot;
+  }
+}
+
 // ---- A4 + A5 steps 2-6: one RK4 step.  Returns 0 to continue, else the final status. -------
 // `done` = field samples taken in this call (0..4); the caller derives its counters from it:
 // a call that returns 0 took 4 samples and is one attempt; a call that ends the particle took
 // `done` samples and is an attempt iff done >= 2 or the new position left the domain (A5.3
 // comes before the attempt is counted).  The stage-1 sample does not repeat the domain test:
 // p passed it at the end of the previous step (A5.5) or at the seed (A5.1).
-template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool REC = true, class CC = CellCache>
+// REC: record the new vertex here (record_vertex).  !REC && COUNT: only count rec_cd down; the caller records at
+// its phase boundary (record_due).
+template <int LAYOUT, bool UNSTEADY, bool BRICK, bool CACHE, bool UNIT, bool REC = true, class CC = CellCache, bool COUNT = false>
 __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s, CC& cc,
                                              Lane& L, unsigned& done) {
   done = 0;
@@ -215,6 +239,7 @@ __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s,
     }
     L.px = nx; L.py = ny; L.pz = nz; L.n++;                                     // A5.6
     record_vertex<REC>(a, L);
+    if (!REC && COUNT) L.rec_cd--;
     return 0;
   }
   float tn = 0.0f;
@@ -259,6 +284,7 @@ __device__ __forceinline__ unsigned rk4_step(const TraceArgs& a, const Store& s,
   }
   L.px = nx; L.py = ny; L.pz = nz; L.n++;                                       // A5.6
   record_vertex<REC>(a, L);
+  if (!REC && COUNT) L.rec_cd--;
   return 0;
 }
 

@@ -128,6 +128,8 @@ trace_kernel(const TraceArgs a) {
   int my_brick = 0;
   bool active = false, exhausted = false;
   unsigned n_samples = 0, n_attempts = 0, n_start = 0, budget = 0;
+  constexpr bool PH = INTEG == 0 && !INQ;   // phased loop (below)
+  unsigned skip = 0;              // PH: steps of its first phase a continued particle sits out
   unsigned long long pend = ~0ull; // INQ: claimed ring position whose record is not published yet
   bool term = false;              // INQ: this lane's particle terminated since the last count
   unsigned spins = 0, seen_done = 0;   // INQ: polls of an idle warp since the launch last made progress
@@ -177,6 +179,7 @@ trace_kernel(const TraceArgs a) {
             if (INTEG == 1) { L.t = a.t0; L.h = fminf(fmaxf(a.h, a.hmin), a.hmax); L.rejected = false; }
           }
           n_start = L.n;
+          if (PH) skip = L.n & (a.phase - 1u);
           active = true;
           if (fresh) {
             float gx, gy, gz;
@@ -269,6 +272,40 @@ trace_kernel(const TraceArgs a) {
     }
     // ---- a2-a8: one step (RK4) or one attempt (DP5(4)) --------------------------------------
     bool emit = false, handoff = false; int dest = my_brick;
+    if constexpr (PH) {
+      // Phased loop (RK4): a.phase = U steps between two passes through the warp-level code above and below (refill
+      // ballots, vertex staging, emit), U a power of two that divides `stride`, so a vertex can only fall due on the
+      // last step of a phase and is recorded at the boundary.  Lanes keep n = 0 (mod U) at boundaries: a fresh particle
+      // starts there with n = 0, a continued one (n = r mod U) sits out the first r steps of its first phase.  A lane
+      // that loses its particle inside a phase idles until the boundary (U/2 of ~800 steps on average).  Schedule only.
+      const unsigned U = a.phase;
+#pragma unroll 1
+      for (unsigned u = 0; u < U; ++u) {
+        if (active && u >= skip) {
+          unsigned done = 0;
+          unsigned rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT, false, typename TraceCache<UNSTEADY && CACHE>::type, true>(a, st, cc, L, done);
+          if (BRICK && rc == 0) {                                                 // a8: owner of p_new
+            if (!still_owned<UNIT>(a.g, st, L.px, L.py, L.pz)) dest = owner_of<UNIT>(a.g, a.bm, L.px, L.py, L.pz);
+            if (dest != my_brick) { rc = (L.n == a.max_steps) ? ST_MAXSTEPS : RC_HANDOFF; done = 0; handoff = rc == RC_HANDOFF; }
+          }
+          if (rc == 0 && --budget == 0u) { rc = RC_HANDOFF; done = 0; }           // segment budget spent
+          if (rc) {
+            active = false;
+            // a vertex that fell due on this very step (n = 0 mod stride) is recorded before the particle goes
+            record_due<trace_block(INTEG)>(a, L);
+            if (rc == RC_HANDOFF) emit = true; else { finish_particle<trace_block(INTEG)>(a, L, rc); term = true; }
+            n_attempts = (L.n - n_start) + (done >= 2u ? 1u : 0u);
+            n_samples = 4u * (L.n - n_start) + min(done, 4u);
+            atomicAdd(&s_tot[0], (unsigned long long)n_attempts);
+            atomicAdd(&s_tot[1], (unsigned long long)(L.n - n_start));
+            atomicAdd(&s_tot[2], (unsigned long long)n_samples);
+            if (handoff) atomicAdd(&s_tot[3], 1ull);
+          }
+        }
+      }
+      skip = 0u;
+      if (active) record_due<trace_block(INTEG)>(a, L);
+    } else
     if (active) {
       unsigned rc, done = 0;
       if (INTEG == 0) rc = rk4_step<LAYOUT, UNSTEADY, BRICK, CACHE, UNIT>(a, st, cc, L, done);
