@@ -308,7 +308,10 @@ int streami_brick_advect_host(streami_field f, const float* seeds, size_t n,
  *   "presort"           0/1   process work items in Morton order of their 4^3-cell block
  *   "segment_steps"     K     streamlines: K step attempts per particle per launch, survivors are
  *                             re-sorted between launches (0 = one launch; DP5(4) then synchronises)
- *   "prefetch"          0/1/2 RK4: request the predicted next cell one step ahead (2: two points)
+ *   "prefetch"          0..4  RK4: request the cell the NEXT step is predicted to end in, a step ahead.  3 (default):
+ *                             early form, issued right after stage 2 from p + 2 h k2; 4: also the next step's mid
+ *                             point; 1: issued at the end of the step from p_new + (p_new - p) (2: plus the half-step
+ *                             point); 0: off.  Bricked fields use the end-of-step form for every value > 0
  *   "integer_accept"    0/1   steady RK4 on a field of finite values: decide "inside" from floor(g)
  *   "vertex_staging"    0/1   stage vertices in shared memory and store full 32-byte sectors
  *   "max_blocks_per_sm" B     limit resident blocks per SM (0 = as many as fit)

@@ -13,7 +13,7 @@
 namespace streami {
 
 // process-wide option values, in the member order of Options (internal.h)
-static std::atomic<int> g_options[N_OPTIONS] = {{1}, {1}, {0}, {0}, {0}, {1}, {1}, {0}, {0}, {1}, {0}, {0}};
+static std::atomic<int> g_options[N_OPTIONS] = {{1}, {1}, {0}, {0}, {0}, {1}, {3}, {0}, {0}, {1}, {0}, {0}};
 static const char* const g_option_names[N_OPTIONS] = {"cell_cache", "presort", "streak_window", "kernel_timing", "segment_steps",
                                                       "vertex_staging", "prefetch", "max_blocks_per_sm", "brick_round_steps",
                                                       "integer_accept", "host_batch", "queue_steps"};
@@ -478,7 +478,7 @@ int streami_set_option(const char* name, int value) {
   if (&base[i] == &lim.cell_cache || &base[i] == &lim.presort || &base[i] == &lim.kernel_timing ||
       &base[i] == &lim.vertex_staging || &base[i] == &lim.integer_accept) v = value != 0;
   else if (&base[i] == &lim.brick_round_steps) v = value < -2 ? -2 : value;
-  else if (&base[i] == &lim.prefetch) v = value < 0 ? 0 : (value > 2 ? 2 : value);
+  else if (&base[i] == &lim.prefetch) v = value < 0 ? 0 : (value > 4 ? 4 : value);
   else v = value < 0 ? 0 : value;
   option_store(i, v);
   return STREAMI_OK;

@@ -32,7 +32,7 @@ def turb48(wl):
     return wl.turb_field_cpu(48, 64, 1, 12)
 
 
-DEFAULTS = dict(segment_steps=0, prefetch=1, vertex_staging=1, max_blocks_per_sm=0, presort=1, queue_steps=0)
+DEFAULTS = dict(segment_steps=0, prefetch=3, vertex_staging=1, max_blocks_per_sm=0, presort=1, queue_steps=0)
 
 
 def _with(S, opts, fn):
@@ -47,7 +47,7 @@ def _with(S, opts, fn):
 
 @pytest.mark.parametrize("layout", [1, 3, 4, 5])
 @pytest.mark.parametrize("opts", [dict(segment_steps=16), dict(segment_steps=37, prefetch=0),
-                                  dict(vertex_staging=0), dict(prefetch=2, max_blocks_per_sm=1),
+                                  dict(vertex_staging=0), dict(prefetch=2, max_blocks_per_sm=1), dict(prefetch=1), dict(prefetch=4),
                                   dict(segment_steps=5, vertex_staging=0, presort=1),
                                   dict(queue_steps=16), dict(queue_steps=7, vertex_staging=0),
                                   dict(queue_steps=50, prefetch=0, max_blocks_per_sm=1)])
