@@ -558,7 +558,8 @@ def roofline_of(job, workload, samples, stored, attempts, kern_ms, kern_n, steps
         cap_ms = float(row["kernel_ms_at_capture"])
         r["traffic_captured_at"] = {"commit": row["commit"], "kernel_ms": cap_ms}
         # the counted bytes belong to the kernel as it was when ncu saw it: flag them when the live kernel has moved
-        r["traffic_stale"] = abs(kms - cap_ms) > 0.10 * cap_ms
+        # (one captured launch cannot be compared with the mean of several launches of different work: C4's windows)
+        r["traffic_stale"] = (abs(kms - cap_ms) > 0.10 * cap_ms) if launches_per_step == 1 else None
         lts = float(row["lts_read_bytes_per_launch"])
         r["l2"] = {"achieved": lts / sec / 1e9, "peak": L2_GATHER_GBS, "unit": "GB/s",
                    "frac": lts / sec / 1e9 / L2_GATHER_GBS,
