@@ -45,6 +45,7 @@ extern "C" {
 #define STREAMI_E_NOMEM      (-2)  /* out of device memory */
 #define STREAMI_E_CUDA       (-3)  /* CUDA error; text behind streami_error_string(-3) */
 #define STREAMI_E_TRUNCATED  (-4)  /* hand-off log or round table overflowed; results still valid */
+#define STREAMI_E_TOO_LARGE  (-5)  /* streami_trace_streamlines_noalloc: more seeds than its static scratch holds */
 
 /* termination reasons (A5) written to out_status */
 #define STREAMI_ALIVE          0u  /* never final */
@@ -142,6 +143,26 @@ int streami_sample(streami_field f, const float* points, size_t n, float t, int 
 int streami_trace_streamlines(streami_field f, const float* seeds, size_t n,
                               const streami_params* params, float* out_vertices,
                               unsigned* out_counts, void* cuda_stream);
+
+/* The same call for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): identical arguments, identical outputs (the same kernels run), but ALL
+ * scratch -- the persistent kernel's work counter and, from 65,536 seeds on, the Morton presort's histogram, keys,
+ * permutation and gathered seeds -- lives in one static device array of the library (7,341,312 bytes, held by
+ * every GPU that loads the library until exit) instead of coming from the stream-ordered allocator.  The call
+ * makes no cudaMalloc / cudaMallocAsync / cudaFree and creates no events or streams.  Limits and rules:
+ *   - n <= STREAMI_NOALLOC_MAX_SEEDS, else STREAMI_E_TOO_LARGE (nothing is enqueued);
+ *   - monolithic fields; one launch to the end (options "segment_steps", "queue_steps" and "kernel_timing"
+ *     are ignored);
+ *   - every call on a device shares the array: the call clears what must start at zero itself, on cuda_stream,
+ *     but two calls that OVERLAP on the GPU (different streams without an ordering between them) race on it and
+ *     give undefined results.  Calls on one stream, or ordered by events, are fine;
+ *   - the first call on a device resolves the array's device address (cudaGetSymbolAddress, no allocation); make
+ *     one call per device before capturing a graph.
+ * Asynchronous on cuda_stream.  Errors: as streami_trace_streamlines, plus TOO_LARGE. */
+#define STREAMI_NOALLOC_MAX_SEEDS 262144
+int streami_trace_streamlines_noalloc(streami_field f, const float* seeds, size_t n,
+                                      const streami_params* params, float* out_vertices,
+                                      unsigned* out_counts, void* cuda_stream);
 
 /* The same call with HOST buffers: seeds, out_vertices, out_counts and the optional outputs in
  * params are host pointers (pinned memory makes the copies faster but is not required).  Copies

@@ -14,7 +14,8 @@ from . import build as _build
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 
-OK, E_INVALID, E_NOMEM, E_CUDA, E_TRUNCATED = 0, -1, -2, -3, -4
+OK, E_INVALID, E_NOMEM, E_CUDA, E_TRUNCATED, E_TOO_LARGE = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_SEEDS = 262144
 OUT_OF_DOMAIN, MAX_STEPS, STAGNANT, HALO_MISS = 1, 2, 3, 4
 LAYOUT_AUTO, LAYOUT_PACKED3, LAYOUT_FLOAT4, LAYOUT_XPAIR, LAYOUT_CELL, LAYOUT_XYQUAD = 0, 1, 2, 3, 4, 5
 
@@ -52,6 +53,7 @@ def lib():
         L.streami_sample.argtypes = [P, P, Z, F, I, P, P, P]
         L.streami_trace_streamlines.argtypes = [P, P, Z, P, P, P, P]
         L.streami_trace_streamlines_host.argtypes = [P, P, Z, P, P, P, P]
+        L.streami_trace_streamlines_noalloc.argtypes = [P, P, Z, P, P, P, P]
         L.streami_trace_streaklines.argtypes = [P, P, Z, U, P, P, P, P]
         L.streami_brick_advect.argtypes = [P, P, Z, P, P, P, P, U, P, Z, P, P, P]
         L.streami_partition_seeds.argtypes = [P, P, Z, P, P, P]
@@ -188,6 +190,16 @@ def streami_trace_streamlines(field, seeds, prm, out_vertices, out_counts, strea
     _check(lib().streami_trace_streamlines(field.handle, _ptr(seeds), seeds.shape[0],
                                            ctypes.byref(prm), _ptr(out_vertices), _ptr(out_counts),
                                            _stream(stream)))
+
+
+def streami_trace_streamlines_noalloc(field, seeds, prm, out_vertices, out_counts, stream=None):
+    """streami_trace_streamlines with all scratch in the library's static device array (no allocation);
+    at most NOALLOC_MAX_SEEDS seeds, calls must not overlap on the GPU (include/streami.h)."""
+    _req(seeds, torch.float32, "seeds"); _req(out_vertices, torch.float32, "out_vertices")
+    _req(out_counts, torch.int32, "out_counts")
+    _check(lib().streami_trace_streamlines_noalloc(field.handle, _ptr(seeds), seeds.shape[0],
+                                                   ctypes.byref(prm), _ptr(out_vertices), _ptr(out_counts),
+                                                   _stream(stream)))
 
 
 def streami_trace_streamlines_host(field, seeds, prm_host, out_vertices, out_counts, stream=None):

@@ -11,7 +11,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libstreami_b200.so")
-UNITS = ["api_field.cu", "api_trace.cu", "api_rounds.cu", "api_mesh.cu"]
+UNITS = ["api_field.cu", "api_trace.cu", "api_rounds.cu", "api_mesh.cu", "api_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off"]
 

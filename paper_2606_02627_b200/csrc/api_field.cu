@@ -518,6 +518,7 @@ const char* streami_error_string(int code) {
     case STREAMI_E_INVALID: return "invalid argument";
     case STREAMI_E_NOMEM: return "out of device memory";
     case STREAMI_E_TRUNCATED: return "hand-off log or round table truncated (results valid)";
+    case STREAMI_E_TOO_LARGE: return "too many seeds for the static scratch of streami_trace_streamlines_noalloc (max 262,144)";
     case STREAMI_E_CUDA: {
       static thread_local std::string copy;
       std::lock_guard<std::mutex> lk(g_err_mutex);
