@@ -235,6 +235,15 @@ typedef struct streami_mesh_s* streami_mesh;
 int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V, const unsigned* H,
                             const float lo[3], const float hi[3], const int nb[3], streami_mesh* out);
 int streami_mesh_destroy(streami_mesh m);
+/* Host-only helpers (no device work).  _reorder_vtk_hex: H_vtk [nc][8] in VTK_HEXAHEDRON node order (0-3 the bottom
+ * face counter-clockwise, 4-7 the top face above them) -> H_out [nc][8] in the corner order of this library
+ * (l = dx + 2 dy + 4 dz); H_out may be H_vtk.  _check_hex: counts the cells whose Jacobian determinant at the cell
+ * centre or at one of the 8 corners is not positive (inverted, degenerate or wrongly ordered cells: U3's Newton iteration does not converge in
+ * them and their points report OUT_OF_DOMAIN) or that name a vertex >= nv; *out_first_bad = the first such cell or -1
+ * (may be NULL).  Call it before _create_hex when the mesh comes from elsewhere.  Errors: INVALID (null). */
+int streami_mesh_reorder_vtk_hex(size_t nc, const unsigned* H_vtk, unsigned* H_out);
+int streami_mesh_check_hex(size_t nv, size_t nc, const float* X, const unsigned* H, unsigned long long* out_bad,
+                           long long* out_first_bad);
 int streami_mesh_sample(streami_mesh m, const float* points, size_t n, float* out_v, long long* out_cell,
                         void* cuda_stream);
 int streami_mesh_trace_streamlines(streami_mesh m, const float* seeds, size_t n, const streami_params* params,

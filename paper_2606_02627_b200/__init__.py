@@ -62,6 +62,8 @@ def lib():
         L.streami_seed_shape.argtypes = [P, P, P, P, U, U, U, I, ctypes.c_ulonglong, P, P]
         L.streami_mesh_create_hex.argtypes = [Z, Z, P, P, P, P, P, P, P]
         L.streami_mesh_destroy.argtypes = [P]
+        L.streami_mesh_reorder_vtk_hex.argtypes = [Z, P, P]
+        L.streami_mesh_check_hex.argtypes = [Z, Z, P, P, P, P]
         L.streami_mesh_sample.argtypes = [P, P, Z, P, P, P]
         L.streami_mesh_trace_streamlines.argtypes = [P, P, Z, P, P, P, P]
         L.streami_mesh_trace_streamlines_lines_host.argtypes = [P, P, Z, P, P, P, ctypes.c_ulonglong, P, P]
@@ -328,6 +330,24 @@ def streami_mesh_trace_streamlines_lines_host(mesh, seeds, prm_host, out_offsets
     """The same on a hexahedral mesh."""
     return _lines_host(lib().streami_mesh_trace_streamlines_lines_host, mesh.handle, seeds, prm_host, out_offsets,
                        out_points, stream)
+
+
+def streami_mesh_reorder_vtk_hex(H_vtk):
+    """[nc][8] uint32 in VTK_HEXAHEDRON node order -> the library's corner order (numpy, host)."""
+    import numpy as np
+    H = np.ascontiguousarray(H_vtk, dtype=np.uint32)
+    out = np.empty_like(H)
+    _check(lib().streami_mesh_reorder_vtk_hex(H.shape[0], H.ctypes.data, out.ctypes.data))
+    return out
+
+
+def streami_mesh_check_hex(X, H):
+    """(number of cells with a non-positive centre Jacobian or a bad vertex index, first such cell or -1)."""
+    import numpy as np
+    X = np.ascontiguousarray(X, dtype=np.float32); H = np.ascontiguousarray(H, dtype=np.uint32)
+    bad = ctypes.c_ulonglong(0); first = ctypes.c_longlong(-1)
+    _check(lib().streami_mesh_check_hex(X.shape[0], H.shape[0], X.ctypes.data, H.ctypes.data, ctypes.byref(bad), ctypes.byref(first)))
+    return bad.value, first.value
 
 
 class Mesh:

@@ -26,6 +26,51 @@ using namespace streami;
 
 extern "C" {
 
+// Host-only helpers for applications that hold their hexahedra in another corner order or are not sure of their
+// orientation (a cell with a non-positive Jacobian never converges in U3: its points would silently report
+// OUT_OF_DOMAIN).  VTK_HEXAHEDRON order: nodes 0-3 = the bottom face counter-clockwise, 4-7 = the top face above them.
+int streami_mesh_reorder_vtk_hex(size_t nc, const unsigned* H_vtk, unsigned* H_out) {
+  if (!H_vtk || !H_out) return STREAMI_E_INVALID;
+  static const int from_vtk[8] = {0, 1, 3, 2, 4, 5, 7, 6};        // lattice corner l = dx + 2 dy + 4 dz <- VTK node
+  for (size_t c = 0; c < nc; ++c) {
+    unsigned t[8];
+    for (int l = 0; l < 8; ++l) t[l] = H_vtk[8 * c + from_vtk[l]];
+    for (int l = 0; l < 8; ++l) H_out[8 * c + l] = t[l];          // in place is fine
+  }
+  return STREAMI_OK;
+}
+
+int streami_mesh_check_hex(size_t nv, size_t nc, const float* X, const unsigned* H, unsigned long long* out_bad,
+                           long long* out_first_bad) {
+  if (!X || !H || !out_bad || nv == 0) return STREAMI_E_INVALID;
+  unsigned long long bad = 0; long long first = -1;
+  for (size_t c = 0; c < nc; ++c) {
+    bool ok = true;
+    for (int l = 0; l < 8 && ok; ++l) ok = H[8 * c + l] < nv;
+    // Jacobian determinant of the trilinear map at the centre and at the 8 corners (the usual validity test of a
+    // hexahedron): dX_a/dxi_b = sum_l X_l[a] dN_l/dxi_b with N_l = prod_b (bit b of l ? xi_b : 1 - xi_b)
+    for (int q = 0; q < 9 && ok; ++q) {
+      const double xi[3] = {q == 8 ? 0.5 : (double)(q & 1), q == 8 ? 0.5 : (double)((q >> 1) & 1), q == 8 ? 0.5 : (double)((q >> 2) & 1)};
+      double J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+      for (int l = 0; l < 8; ++l) {
+        const float* x = X + 3 * (size_t)H[8 * c + l];
+        for (int b = 0; b < 3; ++b) {
+          double w = ((l >> b) & 1) ? 1.0 : -1.0;
+          for (int o = 0; o < 3; ++o) if (o != b) w *= ((l >> o) & 1) ? xi[o] : 1.0 - xi[o];
+          for (int a = 0; a < 3; ++a) J[a][b] += w * (double)x[a];
+        }
+      }
+      const double det = J[0][0] * (J[1][1] * J[2][2] - J[1][2] * J[2][1]) - J[0][1] * (J[1][0] * J[2][2] - J[1][2] * J[2][0]) +
+                         J[0][2] * (J[1][0] * J[2][1] - J[1][1] * J[2][0]);
+      ok = det > 0.0;                                             // NaN -> bad
+    }
+    if (!ok) { if (first < 0) first = (long long)c; ++bad; }
+  }
+  *out_bad = bad;
+  if (out_first_bad) *out_first_bad = first;
+  return STREAMI_OK;
+}
+
 int streami_mesh_create_hex(size_t nv, size_t nc, const float* X, const float* V, const unsigned* H,
                             const float lo[3], const float hi[3], const int nb[3], streami_mesh* out) {
   OptionsScope options_scope;

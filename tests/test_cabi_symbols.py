@@ -107,3 +107,25 @@ def test_argument_validation_without_a_gpu():
         assert S.streami_get_option(name) == v, name
         S.streami_set_option(name, old)
     assert L.streami_error_string(-4).startswith(b"hand-off log")
+
+
+def test_mesh_host_helpers(wl=None):
+    """streami_mesh_reorder_vtk_hex / streami_mesh_check_hex are host-only: VTK node order -> lattice corner order,
+    and the orientation check flags inverted, degenerate and wrongly ordered cells."""
+    import numpy as np
+    import workloads
+    import paper_2606_02627_b200 as S
+    X, V, H, lo, hi = workloads.hexmesh_from_grid((5, 4, 3), (0.0, 0.0, 0.0), (1.0, 0.5, 2.0), None, jitter=0.2, seed=3,
+                                                  value_fn=lambda P: P)
+    assert S.streami_mesh_check_hex(X, H) == (0, -1)
+    # the same cells in VTK order: the check sees the wrong order, the reorder restores the library's
+    to_vtk = [0, 1, 3, 2, 4, 5, 7, 6]
+    H_vtk = H[:, to_vtk]
+    bad, first = S.streami_mesh_check_hex(X, H_vtk)
+    assert bad == H.shape[0] and first == 0
+    assert np.array_equal(S.streami_mesh_reorder_vtk_hex(H_vtk), H)
+    # one mirrored cell (x corners swapped) and one degenerate cell
+    H2 = H.copy(); H2[7] = H2[7][[1, 0, 3, 2, 5, 4, 7, 6]]; H2[11] = H2[11, 0]
+    assert S.streami_mesh_check_hex(X, H2) == (2, 7)
+    H3 = H.copy(); H3[2, 5] = X.shape[0] + 5                                # index out of range
+    assert S.streami_mesh_check_hex(X, H3) == (1, 2)
