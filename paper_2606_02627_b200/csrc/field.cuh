@@ -393,7 +393,7 @@ __device__ __forceinline__ unsigned sample(const Geom& g, const Store& s, CC& cc
     } else { vx = ux; vy = uy; vz = uz; }
   } else if constexpr (CACHE && !IsTimeCache<CC>::value) {
     const unsigned v32 = (unsigned)v;
-    if (v32 != cc.key) { load_cell32<LAYOUT>(s, v32, cc.V); cc.key = v32; }
+    if (v32 != cc.key) { load_cell32<LAYOUT, (LAYOUT == LAYOUT_CELL && !BRICK)>(s, v32, cc.V); cc.key = v32; }
     interp_cell<LayoutTraits<LAYOUT>::DIFF>(cc.V, fx, fy, fz, vx, vy, vz);
   } else {
     float V[24];
